@@ -1,0 +1,39 @@
+"""Seeded synthetic one-/two-electron integrals (BASELINE.json `configs`).
+
+h_pq = h_qp ~ N(0,1)*exp(-|p-q|/4) (p != q), h_pp = -2 - 0.5 p;
+g_pqrs: ONE draw N(0, 0.1^2)*exp(-(|p-q|+|r-s|)/3) per 8-fold orbit
+(g_pqrs = g_qprs = g_pqsr = g_rspq = ...), g_pppp = 0.5 + U(0, 0.5).
+"N(0,0.1)" is read as standard deviation 0.1 (reading R-gen1).
+
+Pure input recipe: numpy PCG64, no method arithmetic.
+"""
+import numpy as np
+
+
+def make_integrals(n_spatial: int, seed: int):
+    """Return (h [N,N] float64 symmetric, g [N,N,N,N] float64 8-fold symmetric, chemists' (pq|rs))."""
+    N = int(n_spatial)
+    rng = np.random.default_rng(seed)
+    idx = np.arange(N)
+
+    # one-body
+    z = rng.standard_normal((N, N))
+    z = np.tril(z, -1)
+    z = z + z.T
+    h = z * np.exp(-np.abs(idx[:, None] - idx[None, :]) / 4.0)
+    h[idx, idx] = -2.0 - 0.5 * idx
+
+    # two-body: one draw per canonical (pq >= rs) compound-index pair
+    M = N * (N + 1) // 2
+    ztab = rng.standard_normal((M, M))
+    diag_u = rng.uniform(0.0, 0.5, size=N)
+    a = np.maximum(idx[:, None], idx[None, :])
+    b = np.minimum(idx[:, None], idx[None, :])
+    pair = a * (a + 1) // 2 + b                      # [N,N] compound index of (p,q)
+    hi = np.maximum(pair[:, :, None, None], pair[None, None, :, :])
+    lo = np.minimum(pair[:, :, None, None], pair[None, None, :, :])
+    dist = np.abs(idx[:, None] - idx[None, :]).astype(np.float64)
+    decay = np.exp(-(dist[:, :, None, None] + dist[None, None, :, :]) / 3.0)
+    g = 0.1 * ztab[hi, lo] * decay
+    g[idx, idx, idx, idx] = 0.5 + diag_u
+    return np.ascontiguousarray(h), np.ascontiguousarray(g)
