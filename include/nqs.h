@@ -1,0 +1,168 @@
+/* nqs.h — C ABI of the B200-native local-energy hot path of arxiv 2208.05637
+ * ("Scalable Neural Quantum States Architecture for Quantum Chemistry").
+ *
+ * What the library computes (citations are PAPER.md lines of /root/reference/PAPER.md):
+ *
+ *   l_theta(x) = sum_{p in S} alpha_p <x|P_p|x^p> f(x^p, theta) / f(x, theta)          (:152, Eq. 15)
+ *   <x|P_p|x^p> = (-i)^r prod_{k: p_k in {2,3}} (-1)^{x_k},  r = #sigma_2 in P_p      (:158 Eq. 16, :192)
+ *   x^p = x xor F^{1,2}_p                                                             (:128, Alg. 1 line 1)
+ *   log f(x) = i phi(x) + 1/2 sum_i log pi_i(x_i | x_<i)                              (:96, Eq. 10)
+ *
+ * with pi_i the conditionals of a MADE (masked FC -> ReLU -> ... -> sigmoid, :84) and phi a dense
+ * two-layer MLP on the first n-2 inputs with 4 outputs picked by the last two bits (:84-86, :91).
+ *
+ * Conventions.  Qubit j (0-based) <-> bit j%64 of word j/64 of a 2 x uint64 configuration; x_j = 1 is
+ * |1> (occupied).  Pauli codes 0,1,2,3 = sigma_0..sigma_3 = I,X,Y,Z (:40 Eq. 1).  Per term:
+ * f = positions holding X or Y (the paper's F^{1,2}), s = positions holding Y or Z (F^{2,3}).
+ * n_qubits in [3, 128].  All "host" pointers are ordinary CPU memory, all "_dev" pointers are CUDA
+ * device memory of the current device (e.g. torch tensor.data_ptr()); `cuda_stream` is a cudaStream_t
+ * passed as void* (NULL = legacy default stream).
+ *
+ * Ownership.  Handles are created by the library and released only by the matching *_free.  Every
+ * buffer passed in stays owned by the caller and is not referenced after the call returns
+ * (compile/create copy what they need).
+ *
+ * Errors.  Every int-returning function returns NQS_OK (0) or a negative nqs_status; on error `*out`
+ * handles are left untouched.  Nothing aborts, throws across the ABI or prints.  There is no CPU
+ * fallback: compute entry points return NQS_ECUDA / NQS_EARCH when no sm_100 device is usable.
+ */
+#ifndef NQS_H_
+#define NQS_H_
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct nqs_ham  nqs_ham_t;    /* opaque: compiled Hamiltonian (host copy + device term tensors) */
+typedef struct nqs_made nqs_made_t;   /* opaque: packed MADE + phase-MLP parameters (host + device)     */
+
+enum nqs_status {
+    NQS_OK           =  0,
+    NQS_EINVAL       = -1,   /* NULL pointer, negative size, Pauli code > 3, bits >= n_qubits set, bad permutation */
+    NQS_ERANGE       = -2,   /* n_qubits outside [3,128], hidden < 1 or > 4096, degrees outside [1, n-1], ...    */
+    NQS_ENOMEM       = -3,   /* host or device allocation failed                                                 */
+    NQS_ECUDA        = -4,   /* a CUDA runtime call or kernel launch failed (no device, ...)                      */
+    NQS_EARCH        = -5,   /* device is not compute capability 10.x (the kernels are sm_100a only)             */
+    NQS_EUNSUPPORTED = -6    /* the requested path cannot run this shape (e.g. NQS_PATH_TC on hidden % 64 != 0)   */
+};
+
+/* Which kernels evaluate the MADE chain.  Both are CUDA; neither touches the CPU.
+ *  NQS_PATH_SIMT : fp32 FFMA on CUDA cores, every layer (reference-quality, any shape).
+ *  NQS_PATH_TC   : tcgen05 tensor cores, fp16 operands / fp32 accumulation in TMEM, fused gather of
+ *                  x xor f into the operand tile and log|psi| / phase / ratio / E_loc in the epilogue.
+ *                  Needs n_hidden_layers == 2, hidden in {256, 384, 512} (multiple of 128, <= 512).
+ *  NQS_PATH_AUTO : TC when the shape supports it, else SIMT. */
+enum nqs_path { NQS_PATH_AUTO = 0, NQS_PATH_SIMT = 1, NQS_PATH_TC = 2 };
+
+/* ---- (a1) Hamiltonian compile: Fig. 1 (:101) -------------------------------------
+ * "we constructed a string parser that computes an Operator Matrix along with coefficients ... collect
+ * the indices of sigma_1, sigma_2 operators prior to the training and only keep a buffer of unique
+ * flippings and their corresponding number of occurrences".
+ *
+ * codes  : host uint8 [n_terms][n_qubits], the Operator Matrix, entries 0..3.
+ * coeffs : host double [n_terms], real alpha_p (:47).
+ * Result (host copy kept for nqs_ham_export; device copy made on first compute call):
+ *   1. per term (f, s) and r = popcount(f & s);
+ *   2. terms with identical (f, s) merged, coefficients summed in fp64 in input order, left to right;
+ *   3. nothing dropped except a merged coefficient that is exactly 0.0;
+ *   4. groups = distinct f, ascending as unsigned 128-bit integers (word 1 major); inside a group terms
+ *      ascending by s the same way; offsets[g] .. offsets[g+1] index the terms of group g;
+ *   5. coef = (float)c round-to-nearest-even; ycount = r.
+ * n_terms = 0 is valid (E_loc = 0).  Pure host work: usable without a GPU. */
+int nqs_ham_compile(int n_qubits, int64_t n_terms, const uint8_t *codes, const double *coeffs,
+                    nqs_ham_t **out);
+
+/* Same, from bit-packed incidence rows: fmask = F^{1,2}, smask = F^{2,3}, host uint64 [n_terms][2]. */
+int nqs_ham_compile_packed(int n_qubits, int64_t n_terms, const uint64_t *fmask, const uint64_t *smask,
+                           const double *coeffs, nqs_ham_t **out);
+
+/* K = merged term count, G = number of unique flips, sum_abs_coeff = sum_t |c_t| (fp64, merged, the
+ * tolerance scale of BASELINE.json).  Any output pointer may be NULL. */
+int nqs_ham_info(const nqs_ham_t *ham, int *n_qubits, int64_t *K, int64_t *G, double *sum_abs_coeff);
+
+/* Host copies of the grouped tensors (for bit-exact tests).  Caller-allocated:
+ * flips uint64 [G][2], offsets uint32 [G+1], zy uint64 [K][2], ycount uint8 [K], coef float [K].
+ * Any pointer may be NULL. */
+int nqs_ham_export(const nqs_ham_t *ham, uint64_t *flips, uint32_t *offsets, uint64_t *zy,
+                   uint8_t *ycount, float *coef);
+
+void nqs_ham_free(nqs_ham_t *ham);
+
+/* ---- model parameters: PAPER.md:84 (architecture), :86 (masks "remove the connections"), :107 ------
+ * n_hidden_layers : 1 (the paper's diagram) or 2 (BASELINE.json configs).
+ * order      : host int32 [n] permutation; autoregressive position d reads qubit order[d]
+ *              (NULL = identity; the paper's default is reverse, :107).
+ * deg_hidden : host int32 [n_hidden_layers][hidden], MADE degrees in [1, n-1]
+ *              (NULL = 1 + floor(j*(n-1)/hidden) for every layer).
+ *              Masks: M1[j][d] = deg1[j] >= d+1;  Mk[j'][j] = deg_k[j'] >= deg_{k-1}[j];
+ *              Mout[d][j] = d+1 > deg_L[j].
+ * weights    : n_hidden_layers+1 host fp32 matrices, row-major [out][in], UNMASKED:
+ *              [hidden][n], ([hidden][hidden]), [n][hidden]; columns/rows indexed by position d.
+ * biases     : matching host fp32 vectors.
+ * phase_weights / phase_biases : [hidden][n-2], [4][hidden] / [hidden], [4]; the phase net reads
+ *              u_d = 2 z_d - 1 for positions d < n-2 and phi = o[2 z_{n-2} + z_{n-1}].
+ * Pure host work (masking, packing, fp16 splitting); device copies are made on first compute call. */
+int nqs_made_create(int n_qubits, int hidden, int n_hidden_layers, const int32_t *order,
+                    const int32_t *deg_hidden, const float *const *weights, const float *const *biases,
+                    const float *const *phase_weights, const float *const *phase_biases,
+                    nqs_made_t **out);
+
+/* Host copy of the masked fp32 weight W_k (.) M_k of layer k (0-based, k <= n_hidden_layers), row-major
+ * [out][in] in position order — lets a CPU test check the mask rule without a GPU. */
+int nqs_made_export_masked(const nqs_made_t *made, int layer, float *out);
+
+void nqs_made_free(nqs_made_t *made);
+
+/* ---- (a4) MADE forward: Eq. 10 ---------------------------------------------------------
+ * configs_dev : device uint64 [B][2]; bits >= n_qubits must be zero.
+ * out_dev     : device float [B][2] = (log|psi|, phi); phi is not wrapped to [0, 2 pi).
+ * Asynchronous on `cuda_stream`.  B = 0 is a no-op. */
+int nqs_made_logpsi(const nqs_made_t *made, const uint64_t *configs_dev, int64_t B, float *out_dev,
+                    int path, void *cuda_stream);
+
+/* ---- (a3) Pauli contraction alone: Eq. 16 summed inside each unique-flip group --------
+ * S[i][g - g0] = sum_{t in group g} c_t (-i)^{r_t} (-1)^{popcount(x_i & s_t)},  g in [g0, g1).
+ * samples_dev : device uint64 [B][2];  S_out_dev : device float [B][g1-g0][2] (Re, Im).
+ * Provided for tests and for the contraction-only throughput figure; nqs_local_energy fuses this step
+ * and never materialises S. */
+int nqs_pauli_contract(const nqs_ham_t *ham, const uint64_t *samples_dev, int64_t B, int64_t g0,
+                       int64_t g1, float *S_out_dev, void *cuda_stream);
+
+/* ---- (a2-a7) local energy: PAPER.md:122-134 Alg. 1, :152 Eq. 15, :200 Eq. 17, :202 mini-batches ----
+ * samples_dev  : device uint64 [B][2] (unique samples; duplicates are harmless).
+ * counts_dev   : device int64 [B] multiplicities (:105 "counter"), or NULL = all ones.  They weight the
+ *                statistics only; E_loc does not depend on them.
+ * minibatch    : samples per pass (gradient-accumulation slice, :202); 0 = auto (8192).  A pure partition
+ *                in row order, last slice may be short.
+ * eloc_out_dev : device float [B][2] = (Re, Im) of l_theta(x_i).
+ * stats_out_host : host double [5] = { sum n, sum n Re E, sum n Im E, sum n |E|^2, max |psi ratio| }
+ *                or NULL.  When non-NULL the call synchronises the stream before returning; otherwise it
+ *                is asynchronous.
+ * Overflow of exp(delta log|psi|) propagates as inf/NaN into eloc; never an error code. */
+int nqs_local_energy(const nqs_ham_t *ham, const nqs_made_t *made, const uint64_t *samples_dev,
+                     const int64_t *counts_dev, int64_t B, int64_t minibatch, int path,
+                     float *eloc_out_dev, double *stats_out_host, void *cuda_stream);
+
+/* Same computation with HOST buffers: copies samples/counts host->device, runs nqs_local_energy on an
+ * internal stream, copies eloc device->host and synchronises.  samples_host uint64 [B][2], counts_host
+ * int64 [B] or NULL, eloc_out_host float [B][2], stats_out_host double [5] or NULL. */
+int nqs_local_energy_host(const nqs_ham_t *ham, const nqs_made_t *made, const uint64_t *samples_host,
+                          const int64_t *counts_host, int64_t B, int64_t minibatch, int path,
+                          float *eloc_out_host, double *stats_out_host);
+
+/* Number of kernels this library has launched in the calling process since load (monotonic). */
+int64_t nqs_kernel_launch_count(void);
+
+/* Duration in milliseconds of the dominant (MADE-chain) kernel launches of the LAST nqs_local_energy /
+ * nqs_local_energy_host call, summed over its mini-batches, measured with CUDA events on the launching
+ * stream; *n_launches receives how many launches that was.  Synchronises on those events. */
+int nqs_last_chain_kernel_ms(const nqs_made_t *made, float *ms, int *n_launches);
+
+const char *nqs_strerror(int status);
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* NQS_H_ */

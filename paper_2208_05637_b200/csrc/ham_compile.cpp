@@ -1,0 +1,128 @@
+// (a1) Hamiltonian compiler — host only.  PAPER.md:154-156: parse the Operator Matrix into incidence rows
+// F^{1,2} (flips) / F^{2,3} (signs), keep a buffer of unique flips and their number of occurrences.
+// Rules 1-5 are stated in include/nqs.h.
+#include <algorithm>
+#include <cmath>
+#include <new>
+#include <numeric>
+#include "nqs_internal.h"
+
+namespace {
+
+struct Term { uint64_t f[2], s[2]; int64_t idx; };
+
+inline bool key_less(const Term &a, const Term &b) {
+    if (a.f[1] != b.f[1]) return a.f[1] < b.f[1];
+    if (a.f[0] != b.f[0]) return a.f[0] < b.f[0];
+    if (a.s[1] != b.s[1]) return a.s[1] < b.s[1];
+    return a.s[0] < b.s[0];
+}
+inline bool key_eq(const Term &a, const Term &b) {
+    return a.f[0] == b.f[0] && a.f[1] == b.f[1] && a.s[0] == b.s[0] && a.s[1] == b.s[1];
+}
+
+int finish(int n, std::vector<Term> &terms, const double *coeffs, nqs_ham_t **out) {
+    // stable sort keeps input order among identical strings -> left-to-right fp64 merge (rule 2)
+    std::stable_sort(terms.begin(), terms.end(), key_less);
+    nqs_ham *H = new (std::nothrow) nqs_ham();
+    if (!H) return NQS_ENOMEM;
+    H->n = n;
+    try {
+        const size_t T = terms.size();
+        size_t i = 0;
+        bool have_group = false;
+        uint64_t gf[2] = {0, 0};
+        while (i < T) {
+            size_t j = i;
+            double c = coeffs[terms[i].idx];
+            for (j = i + 1; j < T && key_eq(terms[j], terms[i]); ++j) c = c + coeffs[terms[j].idx];
+            if (c != 0.0) {                                                      // rule 3
+                const Term &t = terms[i];
+                if (!have_group || gf[0] != t.f[0] || gf[1] != t.f[1]) {
+                    H->flips.push_back(t.f[0]); H->flips.push_back(t.f[1]);
+                    H->offsets.push_back((uint32_t)H->coef.size());
+                    gf[0] = t.f[0]; gf[1] = t.f[1]; have_group = true;
+                }
+                H->zy.push_back(t.s[0]); H->zy.push_back(t.s[1]);
+                H->ycount.push_back((uint8_t)(__builtin_popcountll(t.f[0] & t.s[0]) +
+                                              __builtin_popcountll(t.f[1] & t.s[1])));
+                H->coef.push_back((float)c);                                     // RNE (rule 5)
+                H->sum_abs += std::fabs(c);
+            }
+            i = j;
+        }
+        H->offsets.push_back((uint32_t)H->coef.size());
+        H->K = (int64_t)H->coef.size();
+        H->G = (int64_t)H->offsets.size() - 1;
+    } catch (const std::bad_alloc &) {
+        delete H;
+        return NQS_ENOMEM;
+    }
+    *out = H;
+    return NQS_OK;
+}
+
+inline bool high_bits_clear(int n, const uint64_t m[2]) {
+    if (n >= 128) return true;
+    if (n >= 64) return (n == 64 ? m[1] == 0 : (m[1] >> (n - 64)) == 0);
+    return m[1] == 0 && (m[0] >> n) == 0;
+}
+
+}  // namespace
+
+extern "C" int nqs_ham_compile(int n_qubits, int64_t n_terms, const uint8_t *codes, const double *coeffs,
+                               nqs_ham_t **out) {
+    if (!out || n_terms < 0 || (n_terms > 0 && (!codes || !coeffs))) return NQS_EINVAL;
+    if (n_qubits < 3 || n_qubits > NQS_MAX_QUBITS) return NQS_ERANGE;
+    if (n_terms > 0xFFFFFFF0ll) return NQS_ERANGE;
+    std::vector<Term> terms;
+    try { terms.resize((size_t)n_terms); } catch (const std::bad_alloc &) { return NQS_ENOMEM; }
+    for (int64_t k = 0; k < n_terms; ++k) {
+        Term t{{0, 0}, {0, 0}, k};
+        const uint8_t *row = codes + (size_t)k * n_qubits;
+        for (int j = 0; j < n_qubits; ++j) {
+            const uint8_t p = row[j];
+            if (p > 3) return NQS_EINVAL;
+            const uint64_t bit = 1ull << (j & 63);
+            if (p == 1 || p == 2) t.f[j >> 6] |= bit;       // sigma_1, sigma_2 flip  (F^{1,2})
+            if (p == 2 || p == 3) t.s[j >> 6] |= bit;       // sigma_2, sigma_3 sign  (F^{2,3})
+        }
+        terms[(size_t)k] = t;
+    }
+    return finish(n_qubits, terms, coeffs, out);
+}
+
+extern "C" int nqs_ham_compile_packed(int n_qubits, int64_t n_terms, const uint64_t *fmask,
+                                      const uint64_t *smask, const double *coeffs, nqs_ham_t **out) {
+    if (!out || n_terms < 0 || (n_terms > 0 && (!fmask || !smask || !coeffs))) return NQS_EINVAL;
+    if (n_qubits < 3 || n_qubits > NQS_MAX_QUBITS) return NQS_ERANGE;
+    if (n_terms > 0xFFFFFFF0ll) return NQS_ERANGE;
+    std::vector<Term> terms;
+    try { terms.resize((size_t)n_terms); } catch (const std::bad_alloc &) { return NQS_ENOMEM; }
+    for (int64_t k = 0; k < n_terms; ++k) {
+        Term t{{fmask[2 * k], fmask[2 * k + 1]}, {smask[2 * k], smask[2 * k + 1]}, k};
+        if (!high_bits_clear(n_qubits, t.f) || !high_bits_clear(n_qubits, t.s)) return NQS_EINVAL;
+        terms[(size_t)k] = t;
+    }
+    return finish(n_qubits, terms, coeffs, out);
+}
+
+extern "C" int nqs_ham_info(const nqs_ham_t *ham, int *n_qubits, int64_t *K, int64_t *G, double *sum_abs_coeff) {
+    if (!ham) return NQS_EINVAL;
+    if (n_qubits) *n_qubits = ham->n;
+    if (K) *K = ham->K;
+    if (G) *G = ham->G;
+    if (sum_abs_coeff) *sum_abs_coeff = ham->sum_abs;
+    return NQS_OK;
+}
+
+extern "C" int nqs_ham_export(const nqs_ham_t *ham, uint64_t *flips, uint32_t *offsets, uint64_t *zy,
+                              uint8_t *ycount, float *coef) {
+    if (!ham) return NQS_EINVAL;
+    if (flips)   std::copy(ham->flips.begin(), ham->flips.end(), flips);
+    if (offsets) std::copy(ham->offsets.begin(), ham->offsets.end(), offsets);
+    if (zy)      std::copy(ham->zy.begin(), ham->zy.end(), zy);
+    if (ycount)  std::copy(ham->ycount.begin(), ham->ycount.end(), ycount);
+    if (coef)    std::copy(ham->coef.begin(), ham->coef.end(), coef);
+    return NQS_OK;
+}

@@ -1,0 +1,99 @@
+// Internal structures of libnqs (not part of the ABI).
+#pragma once
+#include <cstdint>
+#include <vector>
+#include <cuda_runtime.h>
+#include <cuda_fp16.h>
+#include "../../include/nqs.h"
+
+#define NQS_MAX_QUBITS 128
+#define NQS_MAX_HIDDEN 4096
+
+// ---- device views handed to kernels (plain pointers, no ownership) ------------------------------
+struct HamDev {
+    int n;
+    long long K, G;
+    const ulonglong2 *flips;     // [G] unique flip masks f_g (x = word 0, y = word 1), ascending
+    const uint32_t   *offsets;   // [G+1] CSR into the term arrays
+    const ulonglong2 *zy;        // [K] sign masks s_t
+    const float2     *cph;       // [K] c_t * (-i)^{r_t}: (c,0), (0,-c), (-c,0), (0,c) for r mod 4 = 0..3
+    int has_diag;                // 1 if flips[0] == 0 (group 0 connects x to itself: ratio == 1)
+};
+
+struct MadeDev {
+    int n, h, L;
+    int npad;                    // n rounded up to 4 (row stride of the transposed output layer)
+    const int32_t *order;        // [n] position d -> qubit
+    // SIMT pack: masked fp32 weights TRANSPOSED to [in][out] (out contiguous), position order
+    const float *w1t;            // [n][h]
+    const float *w2t;            // [h][h]   (NULL when L == 1)
+    const float *w3t;            // [h][npad]
+    const float *b1, *b2, *b3;   // [h], [h], [npad]
+    const float *p1t;            // [n][h]   phase layer 1; rows n-2, n-1 are zero
+    const float *p2t;            // [h][4]
+    const float *c1, *c2;        // [h], [4]
+};
+
+// ---- handles ------------------------------------------------------------------------------------
+struct nqs_ham {
+    int n = 0;
+    int64_t K = 0, G = 0;
+    double sum_abs = 0.0;
+    std::vector<uint64_t> flips, zy;      // [G][2], [K][2]
+    std::vector<uint32_t> offsets;        // [G+1]
+    std::vector<uint8_t>  ycount;         // [K]
+    std::vector<float>    coef;           // [K]
+    // device copy (lazy)
+    mutable bool on_device = false;
+    mutable int  device = -1;
+    mutable void *d_flips = nullptr, *d_offsets = nullptr, *d_zy = nullptr, *d_cph = nullptr;
+};
+
+struct TcPack;   // tensor-core weight tiles (kernels_tc.cu)
+
+struct nqs_made {
+    int n = 0, h = 0, L = 0, npad = 0;
+    std::vector<int32_t> order;                 // [n]
+    std::vector<int32_t> deg;                   // [L][h]
+    std::vector<std::vector<float>> wm;         // masked weights, [out][in], position order (L+1)
+    std::vector<std::vector<float>> bias;       // (L+1)
+    std::vector<float> p1, p2, c1, c2;          // [h][n-2], [4][h], [h], [4]
+    // device copies (lazy)
+    mutable bool on_device = false;
+    mutable int  device = -1;
+    mutable std::vector<void *> d_allocs;
+    mutable MadeDev dev{};
+    mutable TcPack *tc = nullptr;
+    // workspace (grown on demand, reused across calls)
+    mutable void  *ws = nullptr;
+    mutable size_t ws_bytes = 0;
+    // timing of the chain kernel (nqs_last_chain_kernel_ms)
+    mutable std::vector<cudaEvent_t> ev;        // pairs (start, stop)
+    mutable int ev_used = 0;
+};
+
+// ---- shared helpers -----------------------------------------------------------------------------
+extern long long g_launch_count;
+int  nqs_check_device();                                        // NQS_OK / NQS_ECUDA / NQS_EARCH
+int  nqs_ham_upload(const nqs_ham *ham);
+int  nqs_made_upload(const nqs_made *made);
+int  nqs_ws_reserve(const nqs_made *made, size_t bytes);
+HamDev nqs_ham_dev(const nqs_ham *ham);
+
+// kernels_simt.cu
+int launch_logpsi_simt(const MadeDev &m, const ulonglong2 *cfg, long long B, float2 *out, cudaStream_t st);
+int launch_contract(const HamDev &hm, const ulonglong2 *x, long long B, long long g0, long long g1,
+                    float2 *S, cudaStream_t st);
+int launch_eloc_simt(const HamDev &hm, const MadeDev &m, const ulonglong2 *x, const float2 *base, long long B,
+                     float2 *eloc, float2 *partial, int nsplit, unsigned *max_ratio_bits, cudaStream_t st);
+int launch_stats(const float2 *eloc, const long long *counts, long long B, double *stats4, cudaStream_t st);
+size_t eloc_simt_partial_bytes(long long B, int *nsplit, const HamDev &hm);
+
+// kernels_tc.cu
+bool tc_supported(const nqs_made *made);
+int  tc_pack_upload(const nqs_made *made);
+void tc_pack_free(const nqs_made *made);
+int  launch_logpsi_tc(const nqs_made *made, const ulonglong2 *cfg, long long B, float2 *out, cudaStream_t st);
+int  launch_eloc_tc(const HamDev &hm, const nqs_made *made, const ulonglong2 *x, const float2 *base, long long B,
+                    float2 *eloc, unsigned *max_ratio_bits, cudaStream_t st);
+size_t eloc_tc_ws_bytes(long long B, const HamDev &hm);

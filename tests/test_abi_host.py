@@ -1,0 +1,132 @@
+"""CPU-only tests of the C-ABI library: it loads, exports every symbol include/nqs.h declares, and its host
+logic (Hamiltonian compile, mask packing, argument checking) matches the oracle bit-exactly.  No compute calls."""
+import ctypes
+import os
+import re
+
+import numpy as np
+import pytest
+
+import paper_2208_05637_b200 as nqs
+from paper_2208_05637_b200 import workloads as wl
+from oracle import compile as ocomp
+from oracle import made as omade
+
+ROOT = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+
+
+def test_library_exports_every_declared_symbol():
+    hdr = open(os.path.join(ROOT, "include", "nqs.h")).read()
+    hdr = re.sub(r"/\*.*?\*/", "", hdr, flags=re.S)
+    names = sorted(set(re.findall(r"\b(nqs_[a-z_0-9]+)\s*\(", hdr)))
+    assert {"nqs_ham_compile", "nqs_made_logpsi", "nqs_local_energy"} <= set(names)
+    L = ctypes.CDLL(nqs.LIB_PATH)
+    for nm in names:
+        assert hasattr(L, nm), nm
+
+
+def _assert_same(lib_t, ora_t):
+    for k in ("flips", "offsets", "zy", "ycount", "coef"):
+        a, b = lib_t[k], ora_t[k]
+        assert a.dtype == b.dtype and a.shape == b.shape, k
+        assert a.tobytes() == b.tobytes(), k            # bit-exact, including the fp32 cast
+
+
+@pytest.mark.parametrize("n", [3, 17, 63, 64, 65, 128])
+def test_compile_bit_exact_random_lists(n):
+    rng = np.random.default_rng(n)
+    K = 400
+    codes = rng.integers(0, 4, size=(K, n)).astype(np.uint8)
+    codes[:, rng.random(n) < 0.6] = 0                       # many identities -> shared flips
+    codes[50:60] = codes[40:50]                              # duplicates
+    coeffs = rng.standard_normal(K) * 10.0 ** rng.integers(-9, 3, size=K)
+    coeffs[55] = -coeffs[45]                                 # exact cancellation
+    H = nqs.ham_compile(codes, coeffs)
+    ora = ocomp.compile_hamiltonian(codes, coeffs)
+    _assert_same(H.export(), ora)
+    assert H.K == ora["zy"].shape[0] and H.G == ora["flips"].shape[0]
+    assert abs(H.sum_abs_coeff - ora["sum_abs_coeff"]) <= 1e-12 * max(1.0, ora["sum_abs_coeff"])
+    # packed entry point gives the same tensors
+    from oracle.pauli import incidence
+    f, s, _ = incidence(codes)
+    _assert_same(nqs.ham_compile_packed(n, f, s, coeffs).export(), ora)
+
+
+@pytest.mark.parametrize("cfg", [1, 2])
+def test_compile_bit_exact_workloads(cfg):
+    w = wl.WORKLOADS[cfg]
+    h, g = wl.make_integrals(w.n_spatial, w.seed_integrals)
+    x, z, c = wl.jw_pauli_terms(h, g)
+    codes = wl.masks_to_codes(x, z, w.n_qubits)
+    H = nqs.ham_compile(codes, c)
+    _assert_same(H.export(), ocomp.compile_hamiltonian(codes, c))
+    Hp = nqs.ham_compile_packed(w.n_qubits, x, z, c)
+    _assert_same(Hp.export(), H.export())
+
+
+def test_compile_edge_cases_and_errors():
+    L = nqs.lib()
+    out = ctypes.c_void_p()
+    codes = np.zeros((1, 4), np.uint8)
+    co = np.ones(1)
+    assert L.nqs_ham_compile(2, 1, codes.ctypes.data, co.ctypes.data, ctypes.byref(out)) == -2      # n < 3
+    assert L.nqs_ham_compile(129, 1, codes.ctypes.data, co.ctypes.data, ctypes.byref(out)) == -2
+    assert L.nqs_ham_compile(4, -1, codes.ctypes.data, co.ctypes.data, ctypes.byref(out)) == -1
+    assert L.nqs_ham_compile(4, 1, None, co.ctypes.data, ctypes.byref(out)) == -1
+    bad = np.full((1, 4), 4, np.uint8)
+    assert L.nqs_ham_compile(4, 1, bad.ctypes.data, co.ctypes.data, ctypes.byref(out)) == -1       # code > 3
+    assert out.value is None                                                                       # untouched
+    H = nqs.ham_compile(np.zeros((0, 5), np.uint8), np.zeros(0), n_qubits=5)                        # K = 0 valid
+    assert (H.K, H.G) == (0, 0) and H.export()["offsets"].tolist() == [0]
+    # bits above n_qubits in packed masks are rejected
+    f = np.array([[1 << 5, 0]], np.uint64)
+    assert L.nqs_ham_compile_packed(5, 1, f.ctypes.data, f.ctypes.data, co.ctypes.data, ctypes.byref(out)) == -1
+    assert nqs.lib().nqs_strerror(-5).decode().startswith("device is not")
+
+
+@pytest.mark.parametrize("n,h,L,order,rd", [(8, 32, 2, "reverse", False), (13, 48, 1, "random", True),
+                                            (76, 64, 2, "reverse", False)])
+def test_made_masks_match_oracle(n, h, L, order, rd):
+    p = wl.make_made_params(n, h, 3, n_hidden_layers=L, order=order)
+    if rd:
+        p.deg_hidden = np.random.default_rng(1).integers(1, n, size=(L, h)).astype(np.int32)
+    M = nqs.made_create(p)
+    masks = omade.build_masks(n, p.deg_hidden)
+    for k in range(L + 1):
+        expect = (p.weights[k].astype(np.float64) * masks[k]).astype(np.float32)
+        assert np.array_equal(M.export_masked(k), expect)
+    # NULL degrees = default sorted rule
+    q = wl.make_made_params(n, h, 3, n_hidden_layers=L, order=order)
+    q.deg_hidden = None
+    M2 = nqs.made_create(q)
+    dm = omade.build_masks(n, wl.default_degrees(n, h, L))
+    assert np.array_equal(M2.export_masked(0), (q.weights[0].astype(np.float64) * dm[0]).astype(np.float32))
+
+
+def test_made_create_errors():
+    p = wl.make_made_params(8, 16, 1)
+    p.order = np.array([0, 1, 2, 3, 4, 5, 6, 6], np.int32)            # not a permutation
+    with pytest.raises(nqs.NqsError) as e:
+        nqs.made_create(p)
+    assert e.value.status == -1
+    p = wl.make_made_params(8, 16, 1)
+    p.deg_hidden = np.full((2, 16), 8, np.int32)                        # degree n is out of range
+    with pytest.raises(nqs.NqsError) as e:
+        nqs.made_create(p)
+    assert e.value.status == -2
+    p = wl.make_made_params(8, 16, 1)
+    p.n_qubits = 2
+    with pytest.raises(nqs.NqsError):
+        nqs.made_create(p)
+
+
+def test_compute_entry_points_fail_loudly_without_gpu():
+    import torch
+    if torch.cuda.is_available():
+        pytest.skip("GPU present")
+    w, (x, z, c), params, samples, counts = wl.make_workload(1, batch=4)
+    H = nqs.ham_compile_packed(w.n_qubits, x, z, c)
+    M = nqs.made_create(params)
+    with pytest.raises(nqs.NqsError) as e:
+        nqs.local_energy_host(H, M, samples, counts)
+    assert e.value.status in (-4, -5)

@@ -1,0 +1,203 @@
+"""GPU parity tests (-m gpu): the CUDA path, called through the C ABI, against the fp64 oracle on the same
+seeded inputs.  Tolerances:
+  * E_loc: |dE| <= 1e-5 * sum_t |c_t| per sample, complex modulus (BASELINE.json north_star);
+  * log psi (NQS_PATH_SIMT, fp32): 2e-4 absolute — n <= 128 conditionals of |log pi| <~ 10 summed in fp32
+    after <= 1024-term fp32 dot products;
+  * contraction S[i,g]: 4 ulp(fp32) * sum_{t in g} |c_t|  (sequential fp32 sum of exactly rounded +-c_t);
+  * grouped tensors: bit-exact (tests/test_abi_host.py).
+"""
+import numpy as np
+import pytest
+import torch
+
+import paper_2208_05637_b200 as nqs
+from paper_2208_05637_b200 import workloads as wl
+from oracle import eloc as oeloc
+from oracle import made as omade
+from oracle import compile as ocomp
+from oracle.pauli import matrix_element
+
+pytestmark = pytest.mark.gpu
+DEV = "cuda:0"
+
+
+def _dev_u64(a):
+    return torch.from_numpy(np.ascontiguousarray(a).view(np.int64)).to(DEV)
+
+
+_cache = {}
+
+
+def workload(cfg):
+    if cfg not in _cache:
+        w = wl.WORKLOADS[cfg]
+        h, g = wl.make_integrals(w.n_spatial, w.seed_integrals)
+        x, z, c = wl.jw_pauli_terms(h, g)
+        params = wl.make_made_params(w.n_qubits, w.hidden, w.seed_weights)
+        H = nqs.ham_compile_packed(w.n_qubits, x, z, c)
+        M = nqs.made_create(params)
+        _cache[cfg] = (w, (x, z, c), params, H, M)
+    return _cache[cfg]
+
+
+def _paths(M):
+    # every path that supports this model; SIMT always, TC when the shape allows
+    out = [nqs.PATH_SIMT]
+    try:
+        t = torch.zeros((1, 2), dtype=torch.int64, device=DEV)
+        nqs.made_logpsi(M, t, path=nqs.PATH_TC)
+        out.append(nqs.PATH_TC)
+    except nqs.NqsError as e:
+        assert e.status == -6
+    return out
+
+
+@pytest.mark.parametrize("n,h,L,order", [(8, 32, 2, "reverse"), (20, 128, 2, "reverse"), (30, 256, 2, "identity"),
+                                         (76, 512, 2, "reverse"), (13, 48, 1, "random"), (128, 64, 2, "random"),
+                                         (65, 16, 2, "reverse"), (3, 8, 1, "identity")])
+def test_logpsi_parity(n, h, L, order):
+    p = wl.make_made_params(n, h, 100 + n, n_hidden_layers=L, order=order)
+    rng = np.random.default_rng(n)
+    B = 333                                                      # several tiles + ragged tail
+    bits = rng.integers(0, 2, size=(B, n)).astype(np.uint8)
+    cfgs = wl.pack_bits(bits)
+    ref = omade.logpsi(p, cfgs)
+    M = nqs.made_create(p)
+    for path in _paths(M):
+        out = nqs.made_logpsi(M, _dev_u64(cfgs), path=path).cpu().numpy().astype(np.float64)
+        tol = 2e-4 if path == nqs.PATH_SIMT else 2e-2
+        assert np.abs(out[:, 0] - ref.real).max() < tol, (path, np.abs(out[:, 0] - ref.real).max())
+        assert np.abs(out[:, 1] - ref.imag).max() < tol, (path, np.abs(out[:, 1] - ref.imag).max())
+    assert nqs.made_logpsi(M, torch.zeros((0, 2), dtype=torch.int64, device=DEV)).shape == (0, 2)   # B = 0
+
+
+@pytest.mark.parametrize("cfg,B", [(1, 256), (2, 300), (3, 130)])
+def test_contraction_parity(cfg, B):
+    w, (x, z, c), params, H, M = workload(cfg)
+    samples, _ = wl.make_samples(w.n_spatial, w.n_alpha, w.n_beta, B, w.max_count, w.seed_samples, w.unique)
+    t = H.export()
+    off = t["offsets"].astype(np.int64)
+    g0, g1 = (0, H.G) if cfg < 3 else (5, 1200)
+    S = nqs.pauli_contract(H, _dev_u64(samples), g0, g1).cpu().numpy().astype(np.float64)
+    S = S[..., 0] + 1j * S[..., 1]                               # [g, B]
+    for gi in range(g0, g1):
+        sl = slice(off[gi], off[gi + 1])
+        cc = t["coef"][sl].astype(np.float64)
+        ref = (cc[None, :] * matrix_element(samples[:, None, :], t["zy"][sl][None, :, :],
+                                            t["ycount"][sl].astype(np.int64))).sum(axis=1)
+        tol = 4 * 2.0 ** -24 * np.abs(cc).sum() * max(1, sl.stop - sl.start) ** 0.5 + 1e-30
+        assert np.abs(S[gi - g0] - ref).max() <= tol, (gi, np.abs(S[gi - g0] - ref).max(), tol)
+
+
+def _check_eloc(cfg, B_gpu, n_oracle, minibatch, memo=False):
+    w, (x, z, c), params, H, M = workload(cfg)
+    samples, counts = wl.make_samples(w.n_spatial, w.n_alpha, w.n_beta, B_gpu, w.max_count, w.seed_samples, w.unique)
+    codes = wl.masks_to_codes(x, z, w.n_qubits)
+    rng = np.random.default_rng(cfg)
+    pick = np.sort(rng.choice(B_gpu, size=min(n_oracle, B_gpu), replace=False))
+    ref = oeloc.local_energy(codes, c, params, samples[pick], memo=memo)
+    tol = 1e-5 * H.sum_abs_coeff
+    res = {}
+    for path in _paths(M):
+        e, stats = nqs.local_energy(H, M, _dev_u64(samples), torch.from_numpy(counts).to(DEV), minibatch=minibatch, path=path)
+        e = e.cpu().numpy().astype(np.float64)
+        ec = e[:, 0] + 1j * e[:, 1]
+        err = np.abs(ec[pick] - ref).max()
+        assert err <= tol, (cfg, path, err, tol)
+        ws = oeloc.weighted_stats(ec, counts)
+        np.testing.assert_allclose(stats[:4], ws[:4], rtol=1e-9)
+        assert stats[4] >= 1.0 and np.isfinite(stats[4])
+        res[path] = (err / tol, ec)
+    return res
+
+
+def test_eloc_cfg1_all_samples_and_full_sector():
+    _check_eloc(1, 256, 256, 256)
+    # the whole 2a+2b sector (36 states), A16
+    w, (x, z, c), params, H, M = workload(1)
+    from itertools import combinations
+    rows = []
+    for a in combinations(range(4), 2):
+        for b in combinations(range(4), 2):
+            bits = np.zeros(8, np.uint8)
+            for k in a: bits[2 * k] = 1
+            for k in b: bits[2 * k + 1] = 1
+            rows.append(bits)
+    sector = wl.pack_bits(np.array(rows))
+    ref = oeloc.local_energy(wl.masks_to_codes(x, z, 8), c, params, sector)
+    e, _ = nqs.local_energy(H, M, _dev_u64(sector), None, path=nqs.PATH_SIMT)
+    e = e.cpu().numpy().astype(np.float64)
+    assert np.abs(e[:, 0] + 1j * e[:, 1] - ref).max() <= 1e-5 * H.sum_abs_coeff
+
+
+def test_eloc_cfg2_bench_configuration():
+    _check_eloc(2, 4096, 192, 4096)
+
+
+def test_eloc_cfg3_sampled():
+    _check_eloc(3, 2048, 24, 2048, memo=True)
+
+
+def test_eloc_cfg4_sampled():
+    _check_eloc(4, 160, 6, 96, memo=True)          # two mini-batches, the second short
+
+
+def test_eloc_cfg5_sampled():
+    _check_eloc(5, 128, 2, 8192, memo=True)
+
+
+def test_minibatch_partition_and_host_variant():
+    w, (x, z, c), params, H, M = workload(2)
+    samples, counts = wl.make_samples(w.n_spatial, w.n_alpha, w.n_beta, 300, w.max_count, w.seed_samples, True)
+    xs = _dev_u64(samples)
+    cd = torch.from_numpy(counts).to(DEV)
+    e1, s1 = nqs.local_energy(H, M, xs, cd, minibatch=300, path=nqs.PATH_SIMT)
+    e2, s2 = nqs.local_energy(H, M, xs, cd, minibatch=128, path=nqs.PATH_SIMT)        # 128 + 128 + 44
+    tol = 1e-5 * H.sum_abs_coeff
+    d = (e1 - e2).cpu().numpy().astype(np.float64)
+    assert np.hypot(d[:, 0], d[:, 1]).max() <= tol
+    np.testing.assert_allclose(s1[:4], s2[:4], rtol=1e-6)
+    eh, sh = nqs.local_energy_host(H, M, samples, counts, minibatch=128, path=nqs.PATH_SIMT)
+    assert np.array_equal(eh, e2.cpu().numpy())
+    np.testing.assert_allclose(sh, s2, rtol=0, atol=0)
+    # counts = NULL -> unit weights
+    e3, s3 = nqs.local_energy(H, M, xs, None, minibatch=0, path=nqs.PATH_SIMT)
+    assert s3[0] == 300
+    # B = 0
+    e0, s0 = nqs.local_energy(H, M, xs[:0], None)
+    assert e0.shape == (0, 2) and np.all(s0 == 0)
+
+
+@pytest.mark.parametrize("n", [5, 64, 65, 128])
+def test_generic_hamiltonian_odd_Y_two_words(n):
+    """Random Pauli lists with odd Y counts, duplicates, no identity group, n around the word boundary."""
+    rng = np.random.default_rng(n)
+    K = 150
+    codes = rng.integers(0, 4, size=(K, n)).astype(np.uint8)
+    codes[:, rng.random(n) < 0.8] = 0
+    codes[:, n - 1] = rng.integers(0, 4, size=K)                 # keep the top qubit busy
+    codes[:, 0] = np.where(codes[:, 0] == 0, 1, codes[:, 0])     # every string flips qubit 0: no f = 0 group
+    codes[7] = codes[3]
+    coeffs = rng.standard_normal(K)
+    p = wl.make_made_params(n, 32, n, order="random")
+    bits = rng.integers(0, 2, size=(70, n)).astype(np.uint8)
+    samples = wl.pack_bits(bits)
+    H = nqs.ham_compile(codes, coeffs)
+    assert H.export()["flips"][0].any()
+    M = nqs.made_create(p)
+    ref, mr = oeloc.local_energy(codes, coeffs, p, samples, return_max_ratio=True)
+    e, st = nqs.local_energy(H, M, _dev_u64(samples), None, path=nqs.PATH_SIMT)
+    e = e.cpu().numpy().astype(np.float64)
+    scale = max(1.0, mr)
+    assert np.abs(e[:, 0] + 1j * e[:, 1] - ref).max() <= 1e-5 * H.sum_abs_coeff * scale
+    assert abs(st[4] - mr) <= 1e-3 * mr
+    assert np.abs(ref.imag).max() > 1e-3                          # the imaginary channel is really exercised
+
+
+def test_empty_hamiltonian():
+    p = wl.make_made_params(6, 16, 1)
+    H = nqs.ham_compile(np.zeros((0, 6), np.uint8), np.zeros(0), n_qubits=6)
+    M = nqs.made_create(p)
+    xs = _dev_u64(wl.pack_bits(np.random.default_rng(0).integers(0, 2, size=(9, 6)).astype(np.uint8)))
+    e, st = nqs.local_energy(H, M, xs, None)
+    assert torch.all(e == 0) and st[0] == 9 and st[1] == 0
