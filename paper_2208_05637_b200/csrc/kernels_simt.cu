@@ -33,13 +33,18 @@ __device__ __forceinline__ void layer_fwd(const float *__restrict__ Wt, int ldw,
 #pragma unroll 4
         for (int k = 0; k < K; ++k) {
             const float w = __ldg(Wt + (size_t)k * ldw + j);
+            if constexpr (RPT >= 4) {
 #pragma unroll
-            for (int r = 0; r < RPT; r += 4) {
-                const float4 a = *reinterpret_cast<const float4 *>(inp + k * TR + r);
-                acc[r] = fmaf(w, a.x, acc[r]);
-                acc[r + 1] = fmaf(w, a.y, acc[r + 1]);
-                acc[r + 2] = fmaf(w, a.z, acc[r + 2]);
-                acc[r + 3] = fmaf(w, a.w, acc[r + 3]);
+                for (int r = 0; r < RPT; r += 4) {
+                    const float4 a = *reinterpret_cast<const float4 *>(inp + k * TR + r);
+                    acc[r] = fmaf(w, a.x, acc[r]);
+                    acc[r + 1] = fmaf(w, a.y, acc[r + 1]);
+                    acc[r + 2] = fmaf(w, a.z, acc[r + 2]);
+                    acc[r + 3] = fmaf(w, a.w, acc[r + 3]);
+                }
+            } else {
+#pragma unroll
+                for (int r = 0; r < RPT; ++r) acc[r] = fmaf(w, inp[k * TR + r], acc[r]);
             }
         }
 #pragma unroll
