@@ -122,6 +122,8 @@ def main():
     ap.add_argument("--cfg", type=int, default=5)
     ap.add_argument("--oracle-samples", type=int, default=0, help="samples for the cpu_baseline leg (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--mb-samples", type=int, default=0,
+                    help="profiling aid: samples per step instead of the configured mini-batch (labelled in config)")
     args = ap.parse_args()
 
     rank = int(os.environ.get("RANK", "0"))
@@ -130,8 +132,8 @@ def main():
     from paper_2208_05637_b200 import workloads as wl
     w = wl.WORKLOADS[args.cfg]
     n_oracle = args.oracle_samples or {1: 256, 2: 64, 3: 16, 4: 2, 5: 1}[args.cfg]
-    workload_name = (f"cfg{args.cfg}: {w.n_qubits} qubits, h={w.hidden}, one {w.minibatch}-sample mini-batch x all "
-                     f"unique-flip groups per step")
+    workload_name = (f"cfg{args.cfg}: {w.n_qubits} qubits, h={w.hidden}, one {args.mb_samples or w.minibatch}-sample "
+                     f"mini-batch x all unique-flip groups per step" + (" [REDUCED mini-batch: profiling run]" if args.mb_samples else ""))
 
     # ---------------- reference arm: the oracle on the host cores (rank 0 only) ----------------
     if args.impl == "reference":
@@ -173,7 +175,7 @@ def main():
     H = nqs.ham_compile_packed(wq.n_qubits, x, z, c)
     M = nqs.made_create(params)
     path = {"auto": nqs.PATH_AUTO, "simt": nqs.PATH_SIMT, "tc": nqs.PATH_TC}[args.path]
-    mb = wq.minibatch
+    mb = args.mb_samples or wq.minibatch
     n_mb = wq.batch // mb
     xs_all = torch.from_numpy(samples.view(np.int64)).to(dev)
     cnt_all = torch.from_numpy(counts).to(dev)
@@ -247,8 +249,7 @@ def main():
 
     # ---- roofline of the dominant kernel (the MADE-chain / fused E_loc kernel) ----
     peaks = load_peaks()
-    used_tc = (args.path == "tc") or (args.path == "auto" and M.hidden % 128 == 0 and 256 <= M.hidden <= 512
-                                       and M.n_hidden_layers == 2)
+    used_tc = M.resolved_path(path) == nqs.PATH_TC
     flops_eval = algorithmic_flops_per_eval(params)
     evals_per_launch = mb * (G - 1)                       # rows the chain kernel evaluates (f = 0 group has ratio 1)
     k_ms = chain_ms / max(chain_launches, 1)

@@ -41,7 +41,7 @@ typedef struct nqs_made nqs_made_t;   /* opaque: packed MADE + phase-MLP paramet
 enum nqs_status {
     NQS_OK           =  0,
     NQS_EINVAL       = -1,   /* NULL pointer, negative size, Pauli code > 3, bits >= n_qubits set, bad permutation */
-    NQS_ERANGE       = -2,   /* n_qubits outside [3,128], hidden < 1 or > 4096, degrees outside [1, n-1], ...    */
+    NQS_ERANGE       = -2,   /* n_qubits outside [3,128], hidden < 1 or > 1024, degrees outside [1, n-1], ...    */
     NQS_ENOMEM       = -3,   /* host or device allocation failed                                                 */
     NQS_ECUDA        = -4,   /* a CUDA runtime call or kernel launch failed (no device, ...)                      */
     NQS_EARCH        = -5,   /* device is not compute capability 10.x (the kernels are sm_100a only)             */
@@ -52,8 +52,9 @@ enum nqs_status {
  *  NQS_PATH_SIMT : fp32 FFMA on CUDA cores, every layer (reference-quality, any shape).
  *  NQS_PATH_TC   : tcgen05 tensor cores, fp16 operands / fp32 accumulation in TMEM, fused gather of
  *                  x xor f into the operand tile and log|psi| / phase / ratio / E_loc in the epilogue.
- *                  Needs n_hidden_layers == 2, hidden in {256, 384, 512} (multiple of 128, <= 512).
- *  NQS_PATH_AUTO : TC when the shape supports it, else SIMT. */
+ *                  Needs n_hidden_layers == 2, hidden a multiple of 64 in [64, 512], n_qubits <= 112.
+ *  NQS_PATH_AUTO : TC when the shape supports it and hidden >= 384 (where single-pass fp16 operands keep
+ *                  |dE_loc| several times below 1e-5 sum|c|), else SIMT. */
 enum nqs_path { NQS_PATH_AUTO = 0, NQS_PATH_SIMT = 1, NQS_PATH_TC = 2 };
 
 /* ---- (a1) Hamiltonian compile: Fig. 1 (:101) -------------------------------------
@@ -114,6 +115,10 @@ int nqs_made_create(int n_qubits, int hidden, int n_hidden_layers, const int32_t
 int nqs_made_export_masked(const nqs_made_t *made, int layer, float *out);
 
 void nqs_made_free(nqs_made_t *made);
+
+/* Which kernels `path` resolves to for this model: NQS_PATH_SIMT or NQS_PATH_TC, or a negative status
+ * (NQS_EUNSUPPORTED when NQS_PATH_TC is forced on an unsupported shape).  Host only. */
+int nqs_made_path(const nqs_made_t *made, int path);
 
 /* ---- (a4) MADE forward: Eq. 10 ---------------------------------------------------------
  * configs_dev : device uint64 [B][2]; bits >= n_qubits must be zero.

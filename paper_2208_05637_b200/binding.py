@@ -42,6 +42,7 @@ def lib():
                                       c_void_p, ctypes.POINTER(c_void_p)]
         L.nqs_made_export_masked.argtypes = [c_void_p, c_int, c_void_p]
         L.nqs_made_free.argtypes = [c_void_p]
+        L.nqs_made_path.argtypes = [c_void_p, c_int]
         L.nqs_made_free.restype = None
         L.nqs_made_logpsi.argtypes = [c_void_p, c_void_p, c_int64, c_void_p, c_int, c_void_p]
         L.nqs_pauli_contract.argtypes = [c_void_p, c_void_p, c_int64, c_int64, c_int64, c_void_p, c_void_p]
@@ -119,6 +120,12 @@ class Made:
         out = np.zeros(shape, np.float32)
         _chk(lib().nqs_made_export_masked(self._h, layer, out.ctypes.data), "nqs_made_export_masked")
         return out
+
+    def resolved_path(self, path=PATH_AUTO):
+        r = lib().nqs_made_path(self._h, path)
+        if r < 0:
+            raise NqsError(r, "nqs_made_path")
+        return r
 
     def last_chain_kernel_ms(self):
         ms, k = ctypes.c_float(), c_int()

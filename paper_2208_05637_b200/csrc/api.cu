@@ -134,8 +134,15 @@ extern "C" void nqs_made_free(nqs_made_t *M) {
 static int resolve_path(const nqs_made *M, int path, bool *use_tc) {
     if (path == NQS_PATH_SIMT) { *use_tc = false; return NQS_OK; }
     if (path == NQS_PATH_TC) { if (!tc_supported(M)) return NQS_EUNSUPPORTED; *use_tc = true; return NQS_OK; }
-    if (path == NQS_PATH_AUTO) { *use_tc = tc_supported(M); return NQS_OK; }
+    if (path == NQS_PATH_AUTO) { *use_tc = tc_supported(M) && M->h >= 384; return NQS_OK; }
     return NQS_EINVAL;
+}
+
+extern "C" int nqs_made_path(const nqs_made_t *M, int path) {
+    if (!M) return NQS_EINVAL;
+    bool use_tc = false;
+    const int rc = resolve_path(M, path, &use_tc);
+    return rc ? rc : (use_tc ? NQS_PATH_TC : NQS_PATH_SIMT);
 }
 
 extern "C" int nqs_made_logpsi(const nqs_made_t *M, const uint64_t *configs_dev, int64_t B, float *out_dev,

@@ -7,7 +7,7 @@
 #include "../../include/nqs.h"
 
 #define NQS_MAX_QUBITS 128
-#define NQS_MAX_HIDDEN 4096
+#define NQS_MAX_HIDDEN 1024
 
 // ---- device views handed to kernels (plain pointers, no ownership) ------------------------------
 struct HamDev {
