@@ -1,15 +1,19 @@
 // Tensor-core path (NQS_PATH_TC): ONE persistent, warp-specialised sm_100a kernel that runs, per tile of
 // 128 samples x 1 unique-flip group g,
-//   (a2) x' = x xor f_g expanded to a +-1 fp16 operand tile in shared memory,
-//   (a4) the MADE chain and the phase MLP as tcgen05 MMAs (fp16 operands, fp32 accumulation in TMEM):
-//          phase hidden  P = relu(A0 . P1^T + c1)      SS-mode, 64-unit chunks -> smem -> D3p += P . P2^T
-//          layer 1       A1 = relu(A0 . W1^T + b1)     SS-mode, 64-unit chunks -> TMEM (fp16, A operand)
-//          layer 2       A2 = relu(A1 . W2^T + b2)     TS-mode (A from TMEM), all-zero 64x64 mask tiles skipped
-//          layer 3       D3 += A2 . W3^T               SS-mode from the smem staging chunk
+//   (a2) x' = x xor f_g expanded to a +-1 fp16 operand tile A0 in shared memory (double-buffered),
+//   (a4) the MADE chain and the phase MLP as tcgen05 MMAs (fp16 operands, fp32 accumulation in TMEM), in
+//        64-unit hidden CHUNKS that ping-pong between two TMEM accumulators D[0] / D[1]:
+//          layer 1   D = A0 . W1c^T        SS   -> epilogue: +b1, ReLU, fp16 -> A1 (TMEM, A operand of layer 2)
+//          phase     D = A0 . P1c^T        SS   -> epilogue: +c1, ReLU, fp16 IN PLACE -> D3 += D . P2c^T   (TS)
+//          layer 2   D = A1 . W2c^T        TS   -> epilogue: +b2, ReLU, fp16 IN PLACE -> D3 += D . W3c^T   (TS)
+//        all-zero 64x16 blocks of the masked weights are never issued (exact: they contribute 0),
 //   (a3) the Pauli contraction S[i,g] over the group's terms (popcount parity, (-i)^r folded into c),
 //   (a5) ratio = exp(dlog|psi|) cis(dphi), E_i += S * ratio, kept in registers per sample.
-// Weight tiles are pre-packed on the host into the exact shared-memory images (128B-swizzled / core-matrix
-// K-major) in consumption order and streamed by the TMA engine (1-D bulk copies) through a ring of slots.
+// Warp roles (14 warps): 0 = weight producer (TMA 1-D bulk copies into a ring of smem slots), 1 = MMA issuer
+// (table-driven: walks a host-built program of MMA groups), 2-5 / 6-9 = two chunk-epilogue groups (one per
+// accumulator), 10-13 = tile warps (build A0 of the NEXT tile, then the final epilogue of the current one).
+// The weight tiles are pre-packed on the host into the exact shared-memory images (128B-swizzled / core-matrix
+// K-major) in consumption order.
 // PAPER.md:122-134 (Alg. 1), :84-96 (architecture, Eq. 8-10), :152-158 (Eq. 15-16).
 #include <cstring>
 #include <new>
@@ -22,25 +26,62 @@ using namespace tc;
 namespace {
 
 constexpr int TILE_M = 128;
-constexpr int CH = 64;                   // hidden-unit chunk (= D buffer columns = staging K-block)
-constexpr int NTHREADS = 320;            // warp 0 producer, warp 1 MMA, warps 2..9 epilogue
-constexpr int NEPI_WARPS = 8;
+constexpr int CH = 64;                   // hidden-unit chunk = accumulator columns
+constexpr int NTHREADS = 448;
 constexpr int MAX_NC = 8;                // hidden <= 512
-// TMEM column map (512 columns allocated)
-constexpr uint32_t TM_A1 = 0;            // fp16 A1[128][H] packed 2/column: H/2 <= 256 columns
-constexpr uint32_t TM_D0 = 256, TM_D1 = 320;   // two 64-column fp32 accumulators
-constexpr uint32_t TM_D3 = 384;          // layer-3 logits, KO <= 112 columns
-constexpr uint32_t TM_D3P = 496;         // phase outputs, 16 columns
+constexpr int MAX_OPS = 4 * MAX_NC + MAX_NC * MAX_NC;
+constexpr int MAX_SLOTS = 16;
+
+// barrier ids
+enum { BAR_A0FULL = 0, BAR_DFULL = 2, BAR_DFREE = 4, BAR_INPL = 6, BAR_D3FULL = 8, BAR_D3EMPTY = 9,
+       BAR_WFULL = 10, BAR_WEMPTY = 10 + MAX_SLOTS, BAR_COUNT = 10 + 2 * MAX_SLOTS };
+constexpr uint32_t W_NONE = 0xFF, W_A0 = 0xFE;
+
+// One MMA group = one weight sub-tile: up to 8 K-steps (K = 16 each) into one accumulator.
+struct __align__(16) MmaOp {
+    uint32_t a;        // A operand: TS -> TMEM column offset; SS -> byte offset inside the A0 buffer
+    uint32_t b;        // B operand: byte offset inside the current ring slot (or from the smem base if F_B_RES)
+    uint32_t d;        // accumulator TMEM column offset
+    uint32_t idesc;
+    uint32_t w;        // kmask[0:8] | flags[8:16] | wait0[16:24] | wait1[24:32]
+    uint32_t c;        // commit0[0:8] | commit1[8:16]
+    uint32_t pad0, pad1;
+};
+enum { F_A_TMEM = 1, F_B_RES = 2, F_NEW_SLOT = 4, F_END_SLOT = 8, F_ACC0 = 16, F_B_NOSWZ = 32 };
+
+struct ChunkOp { uint16_t bias_off; uint16_t dst_col; uint32_t kind; };   // kind 0: -> A1 at dst_col; 1: in place
+
+struct SmemLayout { uint32_t a0, a0_bytes, res, bias, prog, chunks, bars, slots, total; };
+
+__host__ __device__ inline SmemLayout smem_layout(int KI, int H, int KO, int NC, uint32_t slot_bytes, int nslots) {
+    SmemLayout L;
+    uint32_t off = 0;
+    L.a0_bytes = (uint32_t)TILE_M * KI * 2;                      // [128][KI] fp16 core-matrix layout
+    L.a0 = off; off += 2 * L.a0_bytes;
+    off = (off + 1023) & ~1023u;
+    L.res = off; off += (uint32_t)NC * 2048;                     // resident P2 tiles (16 rows x 64 K, 128B swizzle)
+    L.bias = off; off += (uint32_t)(3 * H + KO + 4) * 4;
+    off = (off + 15) & ~15u;
+    L.prog = off; off += MAX_OPS * (uint32_t)sizeof(MmaOp);
+    L.chunks = off; off += 3 * MAX_NC * (uint32_t)sizeof(ChunkOp);
+    L.bars = off; off += BAR_COUNT * 8;
+    off = (off + 1023) & ~1023u;
+    L.slots = off; off += slot_bytes * (uint32_t)nslots;
+    L.total = off;
+    return L;
+}
 
 struct TcParams {
     int n, H, NC, KI, KO;
-    const uint8_t *wimg;                 // packed weight tiles
-    const uint2 *prog;                   // per-tile weight program: (byte offset, bytes), consumption order
-    int nprog;
-    uint32_t slot_bytes;
-    int nslots;
+    uint32_t tm_d, tm_d3;                // TMEM columns: A1 at 0, D[0] at tm_d, D[1] at tm_d + 64, D3 at tm_d3
+    const uint8_t *wimg;                 // packed streamed weight tiles
+    const uint2 *fills;                  // per-tile ring fills: (byte offset, bytes), consumption order
+    int nfills;
+    const MmaOp *prog; int nprog;        // per-tile MMA program
+    const ChunkOp *chunks; int nchunks;  // per-tile accumulator chunks, in MMA order
+    const uint8_t *resimg; uint32_t res_bytes;   // resident P2 tiles
+    uint32_t slot_bytes; int nslots;
     const float *bias;                   // [c1 H | b1 H | b2 H | b3 KO | c2 4] fp32
-    uint8_t nzmask[MAX_NC];              // layer-2 non-empty 64x64 tiles: bit kb of nzmask[c']
     int mode;                            // 0 = logpsi, 1 = local energy
     const ulonglong2 *xpos;              // [B] configurations, bits in autoregressive POSITION order
     long long B;
@@ -54,35 +95,6 @@ struct TcParams {
     long long g_begin;                   // first group that needs a forward pass (1 if group 0 is f = 0)
 };
 
-struct SmemLayout {
-    uint32_t a0, t0, t1, bias, bars, slots, total;
-};
-
-__host__ __device__ inline SmemLayout smem_layout(int KI, int H, int KO, uint32_t slot_bytes, int nslots) {
-    SmemLayout L;
-    uint32_t off = 0;
-    L.a0 = off; off += (uint32_t)KI * 256;                      // [128][KI] fp16 core-matrix layout
-    off = (off + 1023) & ~1023u;
-    L.t0 = off; off += 16384;
-    L.t1 = off; off += 16384;
-    L.bias = off; off += (uint32_t)(3 * H + KO + 4) * 4;
-    off = (off + 15) & ~15u;
-    L.bars = off; off += 64 * 8;
-    off = (off + 1023) & ~1023u;
-    L.slots = off; off += slot_bytes * (uint32_t)nslots;
-    L.total = off;
-    return L;
-}
-
-// barrier indices inside the bars block
-enum { BAR_A0 = 0, BAR_FINAL = 1, BAR_DFULL = 2, BAR_DEMPTY = 4, BAR_TFULL = 6, BAR_TEMPTY = 8, BAR_A1 = 10,
-       BAR_WFULL = 18, BAR_WEMPTY = 40 };   // up to 22 slots
-
-__device__ __forceinline__ uint32_t pack_relu_half2(float a, float b) {
-    __half2 h = __floats2half2_rn(fmaxf(a, 0.0f), fmaxf(b, 0.0f));
-    return *reinterpret_cast<uint32_t *>(&h);
-}
-
 __device__ __forceinline__ unsigned long long shr128(ulonglong2 a, int s) {      // low 64 bits of a >> s, 0 <= s < 128
     if (s == 0) return a.x;
     if (s < 64) return (a.x >> s) | (a.y << (64 - s));
@@ -93,38 +105,37 @@ __device__ __forceinline__ float log_sigmoid_fast(float t) {
     return fminf(t, 0.0f) - __logf(1.0f + __expf(-fabsf(t)));
 }
 
-__device__ __forceinline__ void tmem_ld8(uint32_t taddr, uint32_t (&v)[8]) {
-    asm volatile("tcgen05.ld.sync.aligned.32x32b.x8.b32 {%0,%1,%2,%3,%4,%5,%6,%7}, [%8];\n"
-                 : "=r"(v[0]), "=r"(v[1]), "=r"(v[2]), "=r"(v[3]), "=r"(v[4]), "=r"(v[5]), "=r"(v[6]), "=r"(v[7])
-                 : "r"(taddr));
-}
-
-__global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const TcParams p) {
+__global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_constant__ TcParams p) {
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t s_tmem_base;
-    __shared__ float s_xchg[TILE_M][2];                 // ch=1 -> ch=0 hand-over of (partial log-sum, phi)
-    const SmemLayout L = smem_layout(p.KI, p.H, p.KO, p.slot_bytes, p.nslots);
+    const SmemLayout L = smem_layout(p.KI, p.H, p.KO, p.NC, p.slot_bytes, p.nslots);
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + L.bars);
     float *s_bias = reinterpret_cast<float *>(smem + L.bias);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
-    const int NC = p.NC, KI = p.KI, KO = p.KO, H = p.H;
+    const int KI = p.KI, KO = p.KO, H = p.H;
 
     // ---- one-time setup ----
     if (threadIdx.x == 0) {
-        mbar_init(&bars[BAR_A0], NEPI_WARPS);
-        mbar_init(&bars[BAR_FINAL], 1);
+        mbar_init(&bars[BAR_A0FULL], 4); mbar_init(&bars[BAR_A0FULL + 1], 4);
         for (int b = 0; b < 2; ++b) {
             mbar_init(&bars[BAR_DFULL + b], 1);
-            mbar_init(&bars[BAR_DEMPTY + b], NEPI_WARPS);
-            mbar_init(&bars[BAR_TFULL + b], NEPI_WARPS);
-            mbar_init(&bars[BAR_TEMPTY + b], 1);
+            mbar_init(&bars[BAR_DFREE + b], 4);
+            mbar_init(&bars[BAR_INPL + b], 4);
         }
-        for (int c = 0; c < MAX_NC; ++c) mbar_init(&bars[BAR_A1 + c], NEPI_WARPS);
+        mbar_init(&bars[BAR_D3FULL], 1);
+        mbar_init(&bars[BAR_D3EMPTY], 4);
         for (int s = 0; s < p.nslots; ++s) { mbar_init(&bars[BAR_WFULL + s], 1); mbar_init(&bars[BAR_WEMPTY + s], 1); }
         fence_mbar_init();
     }
     if (warp == 1) tmem_alloc(&s_tmem_base, 512);
     for (int i = threadIdx.x; i < 3 * H + KO + 4; i += NTHREADS) s_bias[i] = p.bias[i];
+    for (int i = threadIdx.x; i < p.nprog * (int)(sizeof(MmaOp) / 16); i += NTHREADS)
+        reinterpret_cast<uint4 *>(smem + L.prog)[i] = reinterpret_cast<const uint4 *>(p.prog)[i];
+    for (int i = threadIdx.x; i < p.nchunks * (int)(sizeof(ChunkOp) / 8); i += NTHREADS)
+        reinterpret_cast<uint2 *>(smem + L.chunks)[i] = reinterpret_cast<const uint2 *>(p.chunks)[i];
+    for (int i = threadIdx.x; i < (int)(p.res_bytes / 16); i += NTHREADS)
+        reinterpret_cast<uint4 *>(smem + L.res)[i] = reinterpret_cast<const uint4 *>(p.resimg)[i];
+    fence_proxy_async();                                  // resident tiles are read by the tensor core (async proxy)
     tc_fence_before();
     __syncthreads();
     tc_fence_after();
@@ -137,271 +148,241 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const TcParams p) 
     const long long t_lo = ntiles * blockIdx.x / gridDim.x, t_hi = ntiles * (blockIdx.x + 1) / gridDim.x;
 
     if (warp == 0) {
-        // =========================== weight-tile producer (TMA engine, 1-D bulk copies) ===========================
+        // =========================== weight producer (TMA engine, 1-D bulk copies) ===========================
         if (lane == 0) {
-            uint32_t it = 0;                                   // running weight-tile index
+            uint32_t slot = 0, par = 1;                         // a fresh barrier passes a parity-1 wait
             for (long long t = t_lo; t < t_hi; ++t) {
-                for (int e = 0; e < p.nprog; ++e, ++it) {
-                    const uint2 pe = __ldg(&p.prog[e]);
-                    const uint32_t slot = it % (uint32_t)p.nslots, rnd = it / (uint32_t)p.nslots;
-                    mbar_wait(&bars[BAR_WEMPTY + slot], (rnd & 1) ^ 1);
+                for (int e = 0; e < p.nfills; ++e) {
+                    const uint2 pe = __ldg(&p.fills[e]);
+                    mbar_wait(&bars[BAR_WEMPTY + slot], par);
                     mbar_arrive_expect_tx(&bars[BAR_WFULL + slot], pe.y);
                     bulk_g2s(smem + L.slots + slot * p.slot_bytes, p.wimg + pe.x, pe.y, &bars[BAR_WFULL + slot]);
+                    if (++slot == (uint32_t)p.nslots) { slot = 0; par ^= 1; }
                 }
             }
         }
     } else if (warp == 1) {
-        // =========================== MMA issuer (one thread) ===========================
-        if (lane == 0) {
-            const uint32_t a0_addr = smem_u32(smem + L.a0);
-            const uint32_t a0_sbo = (uint32_t)(KI / 8) * 128;
-            const uint32_t t_addr[2] = {smem_u32(smem + L.t0), smem_u32(smem + L.t1)};
-            const uint32_t slots_addr = smem_u32(smem + L.slots);
-            const uint32_t id64 = idesc_f16(128, 64), idKO = idesc_f16(128, KO), id16 = idesc_f16(128, 16);
-            const uint32_t dcol[2] = {TM_D0, TM_D1};
-            uint32_t it = 0, jd = 0, jt_c = 0, tcount = 0;    // weight tiles, D chunks, staging chunks (consumer side), tiles
-            auto wait_w = [&]() -> uint32_t {
-                const uint32_t slot = it % (uint32_t)p.nslots, rnd = it / (uint32_t)p.nslots;
-                mbar_wait(&bars[BAR_WFULL + slot], rnd & 1);
-                tc_fence_after();
-                return slot;
-            };
-            auto done_w = [&](uint32_t slot) { mma_commit(&bars[BAR_WEMPTY + slot]); ++it; };
-            // input layer chunk (SS, A0 core-matrix layout x weight tile core-matrix layout) -> D buffer
-            auto input_chunk = [&]() {
-                const uint32_t b = jd & 1, rnd = jd >> 1;
-                mbar_wait(&bars[BAR_DEMPTY + b], (rnd & 1) ^ 1);
-                tc_fence_after();
-                const uint32_t slot = wait_w();
-                const uint32_t w_addr = slots_addr + slot * p.slot_bytes;
-                for (int ks = 0; ks < KI / 16; ++ks)
-                    mma_ss(tmem + dcol[b], desc_noswz(a0_addr + ks * 256, 128, a0_sbo),
-                           desc_noswz(w_addr + ks * 256, 128, a0_sbo), id64, ks > 0);
-                done_w(slot);
-                mma_commit(&bars[BAR_DFULL + b]);
-                ++jd;
-            };
-            // consume one staging chunk (64 hidden units, smem, 128B swizzle): dst += T . W^T, N = KO or 16
-            auto staged_chunk = [&](uint32_t dst_col, uint32_t idesc, bool accumulate) {
-                const uint32_t tb = jt_c & 1, rnd = jt_c >> 1;
-                mbar_wait(&bars[BAR_TFULL + tb], rnd & 1);
-                tc_fence_after();
-                const uint32_t slot = wait_w();
-                const uint32_t w_addr = slots_addr + slot * p.slot_bytes;
-                for (int ks = 0; ks < 4; ++ks)
-                    mma_ss(tmem + dst_col, desc_sw128(t_addr[tb] + ks * 32), desc_sw128(w_addr + ks * 32), idesc,
-                           accumulate || ks > 0);
-                done_w(slot);
-                mma_commit(&bars[BAR_TEMPTY + tb]);
-                ++jt_c;
-            };
-            for (long long t = t_lo; t < t_hi; ++t, ++tcount) {
-                mbar_wait(&bars[BAR_A0], tcount & 1);
-                tc_fence_after();
-                // ---- phase MLP: hidden chunks, then (one chunk behind) P2 ----
-                for (int c = 0; c < NC; ++c) {
-                    input_chunk();
-                    if (c >= 1) staged_chunk(TM_D3P, id16, c - 1 > 0);
-                }
-                staged_chunk(TM_D3P, id16, NC - 1 > 0);
-                // ---- layer 1 -> A1 in TMEM (written by the epilogue warps) ----
-                for (int c = 0; c < NC; ++c) input_chunk();
-                // ---- layer 2 (TS) with layer 3 one chunk behind ----
-                for (int c2 = 0; c2 < NC; ++c2) {
-                    const uint32_t b = jd & 1, rnd = jd >> 1;
-                    mbar_wait(&bars[BAR_DEMPTY + b], (rnd & 1) ^ 1);
-                    tc_fence_after();
-                    bool first = true;
-                    for (int kb = 0; kb < NC; ++kb) {
-                        if (!((p.nzmask[c2] >> kb) & 1)) continue;
-                        mbar_wait(&bars[BAR_A1 + kb], tcount & 1);
-                        tc_fence_after();
-                        const uint32_t slot = wait_w();
-                        const uint32_t w_addr = slots_addr + slot * p.slot_bytes;
-                        for (int ks = 0; ks < 4; ++ks) {
-                            mma_ts(tmem + dcol[b], tmem + TM_A1 + kb * 32 + ks * 8, desc_sw128(w_addr + ks * 32), id64,
-                                   !first || ks > 0);
-                        }
-                        first = false;
-                        done_w(slot);
+        // =========================== MMA issuer: convergent warp, lane 0 issues ===========================
+        const uint32_t smem_base = smem_u32(smem);
+        const uint32_t a0_addr = smem_base + L.a0, slots_addr = smem_base + L.slots;
+        // descriptor high words: version 1 (bit 46); no-swizzle: lbo = 128 B, sbo = KI/8 * 128 B; 128B swizzle: sbo = 1024 B
+        const uint64_t hi_noswz = ((uint64_t)(128 >> 4) << 16) | ((uint64_t)(((uint32_t)(KI / 8) * 128) >> 4) << 32) | (1ull << 46);
+        const uint64_t hi_sw128 = ((uint64_t)(16 >> 4) << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
+        const MmaOp *prog = reinterpret_cast<const MmaOp *>(smem + L.prog);
+        unsigned long long ph = 0;                             // expected parity per barrier id (bit id)
+        uint32_t slot = 0, wpar = 0, tcount = 0;
+        for (long long t = t_lo; t < t_hi; ++t, ++tcount) {
+            const uint32_t a0_cur = a0_addr + (tcount & 1u) * L.a0_bytes;
+            for (int e = 0; e < p.nprog; ++e) {
+                const uint4 o0 = *reinterpret_cast<const uint4 *>(&prog[e]);
+                const uint2 o1 = *reinterpret_cast<const uint2 *>(&prog[e].w);
+                const uint32_t flags = (o1.x >> 8) & 0xFFu;
+                uint32_t kmask = o1.x & 0xFFu;
+#pragma unroll
+                for (int k = 0; k < 2; ++k) {
+                    uint32_t id = (o1.x >> (16 + 8 * k)) & 0xFFu;
+                    if (id != W_NONE) {
+                        if (id == W_A0) id = BAR_A0FULL + (tcount & 1u);
+                        mbar_wait(&bars[id], (uint32_t)(ph >> id) & 1u);
+                        ph ^= 1ull << id;
                     }
-                    mma_commit(&bars[BAR_DFULL + b]);
-                    ++jd;
-                    if (c2 >= 1) staged_chunk(TM_D3, idKO, c2 - 1 > 0);
                 }
-                staged_chunk(TM_D3, idKO, NC - 1 > 0);
-                mma_commit(&bars[BAR_FINAL]);
+                if (flags & F_NEW_SLOT) mbar_wait(&bars[BAR_WFULL + slot], wpar);
+                tc_fence_after();
+                const uint32_t b_addr = (flags & F_B_RES) ? (smem_base + o0.y) : (slots_addr + slot * p.slot_bytes + o0.y);
+                const uint32_t d_addr = tmem + o0.z;
+                uint32_t acc = (flags & F_ACC0) ? 0u : 1u;
+                const uint64_t b_hi = (flags & F_B_NOSWZ) ? hi_noswz : hi_sw128;
+                const uint32_t b_step = (flags & F_B_NOSWZ) ? 16u : 2u;      // 256 B / 32 B per K-step, in 16 B units
+                uint32_t b_lo = (b_addr >> 4) & 0x3FFFu;
+                if (elect_one()) {
+                    if (flags & F_A_TMEM) {
+                        uint32_t a_t = tmem + o0.x;
+#pragma unroll
+                        for (int ks = 0; ks < 4; ++ks) {
+                            if (kmask & 1u) { mma_ts(d_addr, a_t, b_hi | b_lo, o0.w, acc != 0); acc = 1u; }
+                            kmask >>= 1; a_t += 8; b_lo += b_step;
+                        }
+                    } else {
+                        uint32_t a_lo = ((a0_cur + o0.x) >> 4) & 0x3FFFu;
+#pragma unroll 1
+                        for (; kmask; kmask >>= 1, a_lo += 16, b_lo += b_step)
+                            if (kmask & 1u) { mma_ss(d_addr, hi_noswz | a_lo, b_hi | b_lo, o0.w, acc != 0); acc = 1u; }
+                    }
+                    if (flags & F_END_SLOT) mma_commit(&bars[BAR_WEMPTY + slot]);
+                    const uint32_t c0 = o1.y & 0xFFu, c1 = (o1.y >> 8) & 0xFFu;
+                    if (c0 != W_NONE) mma_commit(&bars[c0]);
+                    if (c1 != W_NONE) mma_commit(&bars[c1]);
+                }
+                __syncwarp();
+                if (flags & F_END_SLOT) { if (++slot == (uint32_t)p.nslots) { slot = 0; wpar ^= 1u; } }
             }
         }
-    } else {
-        // =========================== epilogue warps (256 threads) ===========================
-        const int ew = warp - 2;
-        const int q = warp & 3;                    // TMEM lane quadrant this warp may access
-        const int ch = ew >> 2;                    // column half
-        const int row = q * 32 + lane;
-        const uint32_t lane_base = (uint32_t)(q * 32) << 16;
-        const uint32_t dcol[2] = {TM_D0, TM_D1};
-        uint8_t *a0 = smem + L.a0;
-        uint8_t *tbuf[2] = {smem + L.t0, smem + L.t1};
-        const uint32_t a0_sbo = (uint32_t)(KI / 8) * 128;
-        const float *s_c1 = s_bias, *s_b1 = s_bias + H, *s_b2 = s_bias + 2 * H, *s_b3 = s_bias + 3 * H, *s_c2 = s_bias + 3 * H + KO;
-        uint32_t jd = 0, jt_p = 0, tcount = 0;
-        long long cur_sb = -1;
-        ulonglong2 xp = make_ulonglong2(0, 0), xq = make_ulonglong2(0, 0);
-        float2 b0 = make_float2(0.f, 0.f), E = make_float2(0.f, 0.f);
-        float mr = (p.mode == 1 && p.hm.has_diag) ? 1.0f : 0.0f;     // the f = 0 group has ratio exactly 1
-        long long my_i = -1;
-
-        // one hidden chunk: TMEM accumulator -> +bias, ReLU, fp16 -> (to_tmem ? A1 in TMEM : staging smem)
-        auto hidden_chunk = [&](const float *bias_vec, int c, bool to_tmem) {
-            const uint32_t b = jd & 1, rnd = jd >> 1;
-            mbar_wait(&bars[BAR_DFULL + b], rnd & 1);
-            tc_fence_after();
-            uint32_t v[32];
-            tmem_ld32(tmem + lane_base + dcol[b] + ch * 32, v);
-            tmem_wait_ld();
-            tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive(&bars[BAR_DEMPTY + b]);
-            ++jd;
-            uint32_t w[16];
-            const float4 *bp = reinterpret_cast<const float4 *>(bias_vec + c * CH + ch * 32);
+    } else if (warp < 10) {
+        // =========================== chunk epilogue groups: group g owns accumulator D[g] ===========================
+        const int grp = (warp - 2) >> 2;
+        const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;     // TMEM lane quadrant of this warp
+        const uint32_t d_addr = tmem + lane_base + p.tm_d + (uint32_t)grp * CH;
+        const ChunkOp *chunks = reinterpret_cast<const ChunkOp *>(smem + L.chunks);
+        uint32_t uses = 0;
+        for (long long t = t_lo; t < t_hi; ++t) {
+            for (int j = grp; j < p.nchunks; j += 2, ++uses) {
+                const ChunkOp co = chunks[j];
+                mbar_wait(&bars[BAR_DFULL + grp], uses & 1u);
+                tc_fence_after();
+                uint32_t v[64];
+                tmem_ld32p(d_addr, v);
+                tmem_ld32p(d_addr + 32, v + 32);
+                tmem_wait_ld();
+                const float4 *bp = reinterpret_cast<const float4 *>(s_bias + co.bias_off);
+                uint32_t w[32];
 #pragma unroll
-            for (int j = 0; j < 8; ++j) {
-                const float4 bb = bp[j];
-                w[2 * j] = pack_relu_half2(__uint_as_float(v[4 * j]) + bb.x, __uint_as_float(v[4 * j + 1]) + bb.y);
-                w[2 * j + 1] = pack_relu_half2(__uint_as_float(v[4 * j + 2]) + bb.z, __uint_as_float(v[4 * j + 3]) + bb.w);
-            }
-            if (to_tmem) {
-                tmem_st16(tmem + lane_base + TM_A1 + c * 32 + ch * 16, w);
+                for (int j4 = 0; j4 < 16; ++j4) {
+                    const float4 bb = bp[j4];
+                    w[2 * j4] = cvt_relu_f16x2(__uint_as_float(v[4 * j4]) + bb.x, __uint_as_float(v[4 * j4 + 1]) + bb.y);
+                    w[2 * j4 + 1] = cvt_relu_f16x2(__uint_as_float(v[4 * j4 + 2]) + bb.z, __uint_as_float(v[4 * j4 + 3]) + bb.w);
+                }
+                const bool inplace = co.kind != 0;
+                tmem_st32(inplace ? d_addr : (tmem + lane_base + co.dst_col), w);
                 tmem_wait_st();
                 tc_fence_before();
                 __syncwarp();
-                if (lane == 0) mbar_arrive(&bars[BAR_A1 + c]);
-            } else {
-                const uint32_t tb = jt_p & 1, trnd = jt_p >> 1;
-                mbar_wait(&bars[BAR_TEMPTY + tb], (trnd & 1) ^ 1);
-                uint8_t *T = tbuf[tb];
-#pragma unroll
-                for (int j = 0; j < 4; ++j)
-                    *reinterpret_cast<uint4 *>(T + sw128_offset(row, ch * 32 + j * 8)) =
-                        make_uint4(w[4 * j], w[4 * j + 1], w[4 * j + 2], w[4 * j + 3]);
-                fence_proxy_async();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&bars[BAR_TFULL + tb]);
-                ++jt_p;
+                if (lane == 0) mbar_arrive(&bars[(inplace ? BAR_INPL : BAR_DFREE) + grp]);
             }
+        }
+    } else {
+        // =========================== tile warps: A0 of the next tile, final epilogue of the current ===========================
+        const int q = warp & 3;
+        const int row = q * 32 + lane;
+        const uint32_t lane_base = (uint32_t)(q * 32) << 16;
+        const uint32_t d3_addr = tmem + lane_base + p.tm_d3;
+        const uint32_t a0_sbo = (uint32_t)(KI / 8) * 128;
+        const float *s_b3 = s_bias + 3 * H, *s_c2 = s_bias + 3 * H + KO;
+        const uint32_t zero16[16] = {0};
+
+        struct RowState { long long sb, i; ulonglong2 xp, xq; float2 b0; };
+        auto load_row = [&](long long sb, RowState &r) {
+            r.sb = sb; r.i = sb * TILE_M + row;
+            if (r.i < p.B) {
+                r.xp = p.xpos[r.i];
+                if (p.mode == 1) { r.xq = p.x[r.i]; r.b0 = p.base[r.i]; }
+                else { r.xq = make_ulonglong2(0, 0); r.b0 = make_float2(0.f, 0.f); }
+            } else { r.xp = make_ulonglong2(0, 0); r.xq = r.xp; r.b0 = make_float2(0.f, 0.f); }
+        };
+        // (a2) A0: +-1 fp16 tile, core-matrix K-major layout, one row per thread
+        auto build_a0 = [&](uint32_t buf, ulonglong2 zp) {
+            uint8_t *a0 = smem + L.a0 + buf * L.a0_bytes + (row >> 3) * a0_sbo + (row & 7) * 16;
+            for (int kc = 0; kc < KI / 8; ++kc) {
+                const uint32_t bits = (uint32_t)(shr128(zp, kc * 8) & 0xFFull);
+                uint4 w;
+                w.x = 0xBC00BC00u ^ ((bits & 1u) << 15) ^ ((bits & 2u) << 30);
+                w.y = 0xBC00BC00u ^ ((bits & 4u) << 13) ^ ((bits & 8u) << 28);
+                w.z = 0xBC00BC00u ^ ((bits & 16u) << 11) ^ ((bits & 32u) << 26);
+                w.w = 0xBC00BC00u ^ ((bits & 64u) << 9) ^ ((bits & 128u) << 24);
+                *reinterpret_cast<uint4 *>(a0 + kc * 128) = w;
+            }
+            fence_proxy_async();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars[BAR_A0FULL + buf]);
+        };
+        auto flip_of = [&](long long t) -> ulonglong2 {
+            if (p.mode != 1) return make_ulonglong2(0, 0);
+            return __ldg(&p.fpos[p.g_begin + (t % Gnd)]);
         };
 
+        // D3 accumulates from zero (every MMA into it has accumulate = 1)
+        for (int c = 0; c < KO; c += 16) tmem_st16(d3_addr + c, zero16);
+        tmem_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive(&bars[BAR_D3EMPTY]);
+
+        RowState cur{}, nxt{};
+        ulonglong2 zp = make_ulonglong2(0, 0), zp_n = zp;
+        float2 E = make_float2(0.f, 0.f);
+        float mr = (p.mode == 1 && p.hm.has_diag) ? 1.0f : 0.0f;     // the f = 0 group has ratio exactly 1
+        uint32_t tcount = 0;
+        if (t_lo < t_hi) {
+            load_row(t_lo / Gnd, cur);
+            const ulonglong2 f = flip_of(t_lo);
+            zp = make_ulonglong2(cur.xp.x ^ f.x, cur.xp.y ^ f.y);
+            build_a0(0, zp);
+        }
         for (long long t = t_lo; t < t_hi; ++t, ++tcount) {
-            const long long sb = t / Gnd, g = p.g_begin + (t % Gnd);
-            if (sb != cur_sb) {
-                if (p.mode == 1 && ch == 0 && my_i >= 0 && my_i < p.B) {
-                    atomicAdd(&p.eloc[2 * my_i], E.x);
-                    atomicAdd(&p.eloc[2 * my_i + 1], E.y);
-                }
-                cur_sb = sb;
-                my_i = sb * TILE_M + row;
-                E = make_float2(0.f, 0.f);
-                if (my_i < p.B) {
-                    xp = p.xpos[my_i];
-                    if (p.mode == 1) { xq = p.x[my_i]; b0 = p.base[my_i]; }
-                } else {
-                    xp = make_ulonglong2(0, 0); xq = xp; b0 = make_float2(0.f, 0.f);
+            const long long g = p.g_begin + (t % Gnd);
+            // ---- operand tile of the NEXT tile (its buffer was last read by tile t-1, whose D3FULL we have seen) ----
+            const bool has_next = t + 1 < t_hi;
+            if (has_next) {
+                const long long sbn = (t + 1) / Gnd;
+                if (sbn != cur.sb) load_row(sbn, nxt); else nxt = cur;
+                const ulonglong2 f = flip_of(t + 1);
+                zp_n = make_ulonglong2(nxt.xp.x ^ f.x, nxt.xp.y ^ f.y);
+                build_a0((tcount + 1) & 1u, zp_n);
+            }
+            // ---- (a3) S = sum_{t in g} c_t (-i)^{r_t} (-1)^{popcount(x & s_t)}: independent of the MMAs, done while they run ----
+            float2 S = make_float2(0.f, 0.f);
+            if (p.mode == 1 && cur.i < p.B) {
+                const uint32_t t1 = __ldg(&p.hm.offsets[g + 1]);
+                for (uint32_t tt = __ldg(&p.hm.offsets[g]); tt < t1; ++tt) {
+                    const ulonglong2 zy = __ldg(&p.hm.zy[tt]);
+                    const float2 c = __ldg(&p.hm.cph[tt]);
+                    const bool neg = ((__popcll(cur.xq.x & zy.x) + __popcll(cur.xq.y & zy.y)) & 1) != 0;
+                    S.x += neg ? -c.x : c.x;
+                    S.y += neg ? -c.y : c.y;
                 }
             }
-            ulonglong2 zp = xp;
-            if (p.mode == 1) { const ulonglong2 f = __ldg(&p.fpos[g]); zp.x ^= f.x; zp.y ^= f.y; }
-
-            // ---- (a2) A0: +-1 fp16 tile, core-matrix K-major layout; this thread fills its half of the K chunks ----
-            {
-                const int nkc = KI / 8, kc0 = ch * ((nkc + 1) / 2), kc1 = ch ? nkc : (nkc + 1) / 2;
-                for (int kc = kc0; kc < kc1; ++kc) {
-                    const uint32_t bits = (uint32_t)(shr128(zp, kc * 8) & 0xFFull);
-                    uint4 w;
-                    w.x = 0xBC00BC00u ^ ((bits & 1u) << 15) ^ ((bits & 2u) << 30);
-                    w.y = 0xBC00BC00u ^ ((bits & 4u) << 13) ^ ((bits & 8u) << 28);
-                    w.z = 0xBC00BC00u ^ ((bits & 16u) << 11) ^ ((bits & 32u) << 26);
-                    w.w = 0xBC00BC00u ^ ((bits & 64u) << 9) ^ ((bits & 128u) << 24);
-                    *reinterpret_cast<uint4 *>(a0 + (row >> 3) * a0_sbo + kc * 128 + (row & 7) * 16) = w;
-                }
-                fence_proxy_async();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&bars[BAR_A0]);
-            }
-            // ---- (a4) hidden chunks, in the MMA warp's order ----
-            for (int c = 0; c < NC; ++c) hidden_chunk(s_c1, c, false);      // phase hidden -> staging -> P2
-            for (int c = 0; c < NC; ++c) hidden_chunk(s_b1, c, true);       // layer 1 -> A1 (TMEM)
-            for (int c = 0; c < NC; ++c) hidden_chunk(s_b2, c, false);      // layer 2 -> staging -> layer 3
-
             // ---- final epilogue: log|psi| = 1/2 sum_d log sigmoid(+-a_d), phi = o[2 z_{n-2} + z_{n-1}] ----
-            mbar_wait(&bars[BAR_FINAL], tcount & 1);
+            mbar_wait(&bars[BAR_D3FULL], tcount & 1u);
             tc_fence_after();
             float part = 0.0f, phi = 0.0f;
-            {
-                const int half = KO / 2;                         // KO is a multiple of 16
-                const int d0 = ch * half;
-                for (int j = 0; j < half; j += 8) {
-                    uint32_t v[8];
-                    tmem_ld8(tmem + lane_base + TM_D3 + d0 + j, v);
-                    tmem_wait_ld();
-#pragma unroll
-                    for (int k = 0; k < 8; ++k) {
-                        const int d = d0 + j + k;
-                        if (d < p.n) {
-                            const float a = __uint_as_float(v[k]) + s_b3[d];
-                            const bool z = (shr128(zp, d) & 1ull) != 0;
-                            part += log_sigmoid_fast(z ? a : -a);
-                        }
-                    }
-                }
-                if (ch == 1) {
-                    uint32_t v[8];
-                    tmem_ld8(tmem + lane_base + TM_D3P, v);
-                    tmem_wait_ld();
+            for (int c0 = 0; c0 < KO; c0 += 16) {
+                uint32_t v[16];
+                tmem_ld16p(d3_addr + c0, v);
+                tmem_wait_ld();
+                tmem_st16(d3_addr + c0, zero16);              // D3 restarts from zero for the next tile
+                if (c0 + 16 >= KO) {
                     const int sel = (int)((shr128(zp, p.n - 2) & 1ull) * 2 + (shr128(zp, p.n - 1) & 1ull));
-                    const float o0 = __uint_as_float(v[0]) + s_c2[0], o1 = __uint_as_float(v[1]) + s_c2[1];
-                    const float o2 = __uint_as_float(v[2]) + s_c2[2], o3 = __uint_as_float(v[3]) + s_c2[3];
+                    const float o0 = __uint_as_float(v[12]) + s_c2[0], o1 = __uint_as_float(v[13]) + s_c2[1];
+                    const float o2 = __uint_as_float(v[14]) + s_c2[2], o3 = __uint_as_float(v[15]) + s_c2[3];
                     phi = sel == 0 ? o0 : (sel == 1 ? o1 : (sel == 2 ? o2 : o3));
-                    s_xchg[row][0] = part;
-                    s_xchg[row][1] = phi;
                 }
-            }
-            tc_fence_before();
-            asm volatile("bar.sync 1, 256;\n" ::: "memory");                  // the 8 epilogue warps only
-            if (ch == 0) {
-                const float lp = 0.5f * (part + s_xchg[row][0]);
-                phi = s_xchg[row][1];
-                if (p.mode == 0) {
-                    if (my_i < p.B) p.out[my_i] = make_float2(lp, phi);
-                } else if (my_i < p.B) {
-                    // (a3) S = sum_{t in g} c_t (-i)^{r_t} (-1)^{popcount(x & s_t)}
-                    float2 S = make_float2(0.f, 0.f);
-                    const uint32_t t1 = __ldg(&p.hm.offsets[g + 1]);
-                    for (uint32_t tt = __ldg(&p.hm.offsets[g]); tt < t1; ++tt) {
-                        const ulonglong2 zy = __ldg(&p.hm.zy[tt]);
-                        const float2 c = __ldg(&p.hm.cph[tt]);
-                        const bool neg = ((__popcll(xq.x & zy.x) + __popcll(xq.y & zy.y)) & 1) != 0;
-                        S.x += neg ? -c.x : c.x;
-                        S.y += neg ? -c.y : c.y;
+                const unsigned long long zb = shr128(zp, c0);
+#pragma unroll
+                for (int k = 0; k < 16; ++k) {
+                    const int d = c0 + k;
+                    if (d < p.n) {
+                        const float a = __uint_as_float(v[k]) + s_b3[d];
+                        part += log_sigmoid_fast(((zb >> k) & 1ull) ? a : -a);
                     }
-                    // (a5)
-                    const float mag = __expf(lp - b0.x);
-                    float sn, cs;
-                    __sincosf(phi - b0.y, &sn, &cs);
-                    const float rr = mag * cs, ri = mag * sn;
-                    mr = fmaxf(mr, mag);
-                    E.x += S.x * rr - S.y * ri;
-                    E.y += S.x * ri + S.y * rr;
                 }
             }
-            asm volatile("bar.sync 1, 256;\n" ::: "memory");                  // s_xchg reusable
+            tmem_wait_st();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive(&bars[BAR_D3EMPTY]);
+            const float lp = 0.5f * part;
+            if (p.mode == 0) {
+                if (cur.i < p.B) p.out[cur.i] = make_float2(lp, phi);
+            } else if (cur.i < p.B) {
+                // (a5)
+                const float mag = __expf(lp - cur.b0.x);
+                float sn, cs;
+                __sincosf(phi - cur.b0.y, &sn, &cs);
+                const float rr = mag * cs, ri = mag * sn;
+                mr = fmaxf(mr, mag);
+                E.x += S.x * rr - S.y * ri;
+                E.y += S.x * ri + S.y * rr;
+            }
+            if (!has_next || nxt.sb != cur.sb) {
+                if (p.mode == 1 && cur.i < p.B) {
+                    atomicAdd(&p.eloc[2 * cur.i], E.x);
+                    atomicAdd(&p.eloc[2 * cur.i + 1], E.y);
+                }
+                E = make_float2(0.f, 0.f);
+            }
+            cur = nxt; zp = zp_n;
         }
-        if (p.mode == 1 && ch == 0 && my_i >= 0 && my_i < p.B) {
-            atomicAdd(&p.eloc[2 * my_i], E.x);
-            atomicAdd(&p.eloc[2 * my_i + 1], E.y);
-            atomicMax(p.max_ratio_bits, __float_as_uint(mr));
-        }
+        if (p.mode == 1) atomicMax(p.max_ratio_bits, __float_as_uint(mr));
     }
     tc_fence_before();
     __syncthreads();
@@ -446,18 +427,36 @@ __global__ void diag_init_kernel(HamDev hm, const ulonglong2 *__restrict__ x, lo
 
 // ------------------------------------------------------------------------------------------------------------
 struct TcPack {
-    int KI = 0, KO = 0, NC = 0, nprog = 0, nslots = 0;
-    uint32_t slot_bytes = 0;
-    uint8_t nzmask[MAX_NC] = {0};
-    void *d_wimg = nullptr, *d_prog = nullptr, *d_bias = nullptr;
+    int KI = 0, KO = 0, NC = 0, nprog = 0, nchunks = 0, nfills = 0, nslots = 0;
+    uint32_t slot_bytes = 0, res_bytes = 0, tm_d = 0, tm_d3 = 0;
+    void *d_wimg = nullptr, *d_fills = nullptr, *d_prog = nullptr, *d_chunks = nullptr, *d_res = nullptr, *d_bias = nullptr;
     void *d_fpos = nullptr; size_t fpos_cap = 0; const void *fpos_for = nullptr; long long fpos_G = -1;
     void *d_xpos = nullptr; size_t xpos_cap = 0;
     SmemLayout L{};
     int sms = 148;
+    long long mma_issued = 0, mma_dense = 0;                   // K-steps issued / K-steps of the dense chain, per tile
 };
 
+static inline int round16(int v) { return (v + 15) / 16 * 16; }
+
+static bool tc_shape(const nqs_made *M, int *KI_, int *KO_, uint32_t *slot_, int *nslots_) {
+    if (M->L != 2 || M->h % (2 * CH) != 0 || M->h < 2 * CH || M->h > CH * MAX_NC) return false;
+    const int KI = round16(M->n), KO = round16(M->n + 4), NC = M->h / CH;
+    if (KI > 128 || KO > 128 || M->h / 2 + 2 * CH + KO > 512) return false;
+    uint32_t slot = (uint32_t)CH * KI * 2;                                  // input sub-tile (64 rows x KI)
+    if ((uint32_t)CH * 128 > slot) slot = CH * 128;                          // layer-2 sub-tile (64 x 64)
+    if ((uint32_t)KO * 128 > slot) slot = (uint32_t)KO * 128;                // layer-3 sub-tile (KO x 64)
+    slot = ((2 * slot) + 1023) & ~1023u;                                     // two sub-tiles per fill
+    int ns = MAX_SLOTS;
+    while (ns > 0 && smem_layout(KI, M->h, KO, NC, slot, ns).total > 227 * 1024 - 1024) --ns;
+    if (ns < 3) return false;
+    *KI_ = KI; *KO_ = KO; *slot_ = slot; *nslots_ = ns;
+    return true;
+}
+
 bool tc_supported(const nqs_made *M) {
-    return M->L == 2 && M->h % CH == 0 && M->h >= 64 && M->h <= 512 && ((M->n + 15) / 16) * 16 <= 112;
+    int KI, KO, ns; uint32_t slot;
+    return tc_shape(M, &KI, &KO, &slot, &ns);
 }
 
 static inline uint32_t noswz_offset(uint32_t r, uint32_t k, uint32_t KI) {
@@ -466,116 +465,224 @@ static inline uint32_t noswz_offset(uint32_t r, uint32_t k, uint32_t KI) {
 
 int tc_pack_upload(const nqs_made *M) {
     if (M->tc) return NQS_OK;
+    int KI, KO, ns; uint32_t slot;
+    if (!tc_shape(M, &KI, &KO, &slot, &ns)) return NQS_EUNSUPPORTED;
     TcPack *P = new (std::nothrow) TcPack();
     if (!P) return NQS_ENOMEM;
     const int n = M->n, H = M->h, NC = H / CH;
-    const int KI = ((n + 15) / 16) * 16, KO = KI;
-    P->KI = KI; P->KO = KO; P->NC = NC;
-    const uint32_t in_bytes = (uint32_t)CH * KI * 2, w2_bytes = CH * 128, w3_bytes = (uint32_t)KO * 128, p2_bytes = 16 * 128;
-    uint32_t slot = in_bytes;
-    if (w2_bytes > slot) slot = w2_bytes;
-    if (w3_bytes > slot) slot = w3_bytes;
-    slot = (slot + 1023) & ~1023u;
-    P->slot_bytes = slot;
-    std::vector<uint8_t> img;
-    std::vector<uint2> prog;
-    auto put = [&](uint32_t off, float v) { __half hv = __float2half_rn(v); memcpy(&img[off], &hv, 2); };
-    auto new_tile = [&](uint32_t bytes) -> uint32_t {
-        const uint32_t off = (uint32_t)img.size();
-        img.resize(img.size() + ((bytes + 127) & ~127u), 0);
-        prog.push_back(make_uint2(off, bytes));
-        return off;
+    P->KI = KI; P->KO = KO; P->NC = NC; P->slot_bytes = slot; P->nslots = ns;
+    P->tm_d = (uint32_t)H / 2; P->tm_d3 = (uint32_t)H / 2 + 2 * CH;
+    P->L = smem_layout(KI, H, KO, NC, slot, ns);
+    const uint32_t in_bytes = (uint32_t)CH * KI * 2, w2_bytes = CH * 128, w3_bytes = (uint32_t)KO * 128;
+
+    std::vector<uint8_t> img, res((size_t)NC * 2048, 0);
+    std::vector<uint2> fills;
+    std::vector<MmaOp> prog;
+    std::vector<ChunkOp> chunks;
+    auto put = [](std::vector<uint8_t> &buf, uint32_t off, float v) { __half hv = __float2half_rn(v); memcpy(&buf[off], &hv, 2); };
+
+    // ---- streamed sub-tiles are appended to the open fill (<= slot bytes, in consumption order) ----
+    uint32_t fill_start = 0, fill_bytes = 0;
+    int open_first_op = -1, last_stream_op = -1;
+    auto close_fill = [&]() {
+        if (fill_bytes == 0) return;
+        fills.push_back(make_uint2(fill_start, fill_bytes));
+        prog[last_stream_op].w |= (uint32_t)F_END_SLOT << 8;
+        fill_bytes = 0; open_first_op = -1;
     };
-    auto input_tile = [&](int c, bool phase) {
-        const uint32_t off = new_tile(in_bytes);
+    // reserve `bytes` of streamed image for the op about to be pushed; returns the offset inside its slot
+    auto stream_alloc = [&](uint32_t bytes, uint32_t *flags) -> uint32_t {
+        if (fill_bytes + bytes > slot) close_fill();
+        if (fill_bytes == 0) { fill_start = (uint32_t)img.size(); *flags |= F_NEW_SLOT; open_first_op = (int)prog.size(); }
+        const uint32_t off_in_slot = fill_bytes;
+        img.resize(img.size() + bytes, 0);
+        fill_bytes += bytes;
+        last_stream_op = (int)prog.size();
+        return off_in_slot;
+    };
+    auto make_op = [](uint32_t a, uint32_t b, uint32_t d, uint32_t idesc, uint32_t kmask, uint32_t flags, uint32_t w0, uint32_t w1,
+                      uint32_t c0, uint32_t c1) {
+        MmaOp o{};
+        o.a = a; o.b = b; o.d = d; o.idesc = idesc;
+        o.w = (kmask & 0xFF) | ((flags & 0xFF) << 8) | ((w0 & 0xFF) << 16) | ((w1 & 0xFF) << 24);
+        o.c = (c0 & 0xFF) | ((c1 & 0xFF) << 8);
+        return o;
+    };
+
+    const uint32_t id64 = idesc_f16(128, 64), id16 = idesc_f16(128, 16);
+    int nchunk = 0;                          // running accumulator-chunk index inside the tile
+    std::vector<int> chunk_kind;             // 0 = -> A1 (epilogue frees the accumulator), 1 = in place
+    auto dcol = [&](int ci) { return P->tm_d + (uint32_t)(ci & 1) * CH; };
+    // wait needed before overwriting accumulator (ci & 1): only when its previous user was a kind-0 chunk of THIS tile
+    // (in-place chunks are released by tensor-pipe order: their consumer MMAs are issued before the overwrite)
+    auto free_wait = [&](int ci) -> uint32_t {
+        return (ci >= 2 && chunk_kind[ci - 2] == 0) ? (uint32_t)(BAR_DFREE + (ci & 1)) : W_NONE;
+    };
+
+    // input-layer chunk c (layer 1 or phase hidden): D[b] = A0 . Wc^T
+    auto input_chunk = [&](int c, bool phase, bool first_of_tile) {
+        const int ci = nchunk++;
+        chunk_kind.push_back(phase ? 1 : 0);
+        uint32_t flags = F_B_NOSWZ | F_ACC0;
+        const uint32_t boff = stream_alloc(in_bytes, &flags);
+        const uint32_t base = fill_start + boff;
+        uint32_t kmask = 0;
         for (int r = 0; r < CH; ++r) {
             const int j = c * CH + r;
             for (int k = 0; k < KI; ++k) {
                 float v = 0.f;
                 if (phase) { if (k < n - 2) v = M->p1[(size_t)j * (n - 2) + k]; }
                 else if (k < n) v = M->wm[0][(size_t)j * n + k];
-                put(off + noswz_offset(r, k, KI), v);
+                put(img, base + noswz_offset(r, k, KI), v);
+                if (v != 0.0f) kmask |= 1u << (k / 16);
             }
         }
+        if (!kmask) kmask = 1;                                  // the accumulator must still be overwritten
+        P->mma_issued += __builtin_popcount(kmask); P->mma_dense += KI / 16;
+        prog.push_back(make_op(0, boff, dcol(ci), id64, kmask, flags, first_of_tile ? W_A0 : W_NONE, free_wait(ci),
+                               BAR_DFULL + (ci & 1), W_NONE));
+        // K-steps are addressed from the start of the tile; skipped ones are simply not issued
+        ChunkOp co{};
+        co.bias_off = (uint16_t)((phase ? 0 : H) + c * CH);
+        co.kind = phase ? 1 : 0;
+        co.dst_col = (uint16_t)(c * (CH / 2));
+        chunks.push_back(co);
+        return ci;
     };
-    auto p2_tile = [&](int c) {
-        const uint32_t off = new_tile(p2_bytes);
-        for (int o = 0; o < 4; ++o)
-            for (int k = 0; k < CH; ++k) put(off + sw128_offset(o, k), M->p2[(size_t)o * H + c * CH + k]);
-    };
-    auto w3_tile = [&](int c) {
-        const uint32_t off = new_tile(w3_bytes);
-        for (int d = 0; d < n; ++d)
-            for (int k = 0; k < CH; ++k) put(off + sw128_offset(d, k), M->wm[2][(size_t)d * H + c * CH + k]);
-    };
-    // layer-2 tile occupancy (exact: a tile is skipped only if every masked weight in it is 0)
-    for (int c2 = 0; c2 < NC; ++c2) {
-        uint8_t m = 0;
-        for (int kb = 0; kb < NC; ++kb) {
-            bool any = false;
-            for (int r = 0; r < CH && !any; ++r)
-                for (int k = 0; k < CH; ++k)
-                    if (M->wm[1][(size_t)(c2 * CH + r) * H + kb * CH + k] != 0.0f) { any = true; break; }
-            if (any) m |= (uint8_t)(1u << kb);
+    // consumer of an in-place chunk: D3 (+)= D[ci] . Wc^T  (P2 resident tile or streamed layer-3 tile)
+    auto consumer = [&](int ci, int c, bool phase, bool last_of_tile, bool first_d3) {
+        uint32_t flags = F_A_TMEM, boff, kmask = 0, dst = P->tm_d3, idesc = 0;
+        if (phase) {
+            flags |= F_B_RES;
+            boff = P->L.res + (uint32_t)c * 2048;
+            for (int o = 0; o < 4; ++o)
+                for (int k = 0; k < CH; ++k) {
+                    const float v = M->p2[(size_t)o * H + c * CH + k];
+                    put(res, (uint32_t)c * 2048 + sw128_offset(12 + o, k), v);
+                    if (v != 0.0f) kmask |= 1u << (k / 16);
+                }
+            dst += (uint32_t)KO - 16; idesc = id16;
+            P->mma_dense += 4;
+        } else {
+            boff = stream_alloc(w3_bytes, &flags);
+            const uint32_t base = fill_start + boff;
+            int row_lo = KO;
+            for (int d = 0; d < n; ++d)
+                for (int k = 0; k < CH; ++k) {
+                    const float v = M->wm[2][(size_t)d * H + c * CH + k];
+                    put(img, base + sw128_offset(d, k), v);
+                    if (v != 0.0f) { kmask |= 1u << (k / 16); if (d < row_lo) row_lo = d; }
+                }
+            // output rows below the first nonzero one receive exactly 0 from this chunk: start the MMA at a 16-row boundary
+            const int n_lo = kmask ? (row_lo / 16) * 16 : 0;
+            boff += (uint32_t)(n_lo / 8) * 1024; dst += (uint32_t)n_lo;
+            idesc = idesc_f16(128, KO - n_lo);
+            P->mma_dense += 4;
         }
-        if (!m) m = 1;
-        P->nzmask[c2] = m;
+        P->mma_issued += __builtin_popcount(kmask);
+        prog.push_back(make_op(dcol(ci), boff, dst, idesc, kmask, flags, BAR_INPL + (ci & 1), first_d3 ? BAR_D3EMPTY : W_NONE,
+                               last_of_tile ? BAR_D3FULL : W_NONE, W_NONE));
+    };
+
+    // ---- the per-tile program ----
+    for (int c = 0; c < NC; ++c) input_chunk(c, false, c == 0);                  // layer 1 -> A1
+    int prev = -1, prev_c = -1;
+    bool first_d3 = true;
+    for (int c = 0; c < NC; ++c) {                                                // phase hidden, P2 one chunk behind
+        const int ci = input_chunk(c, true, false);
+        if (prev >= 0) { consumer(prev, prev_c, true, false, first_d3); first_d3 = false; }
+        prev = ci; prev_c = c;
     }
-    // consumption order (must mirror the MMA warp's program)
-    for (int c = 0; c < NC; ++c) { input_tile(c, true); if (c >= 1) p2_tile(c - 1); }
-    p2_tile(NC - 1);
-    for (int c = 0; c < NC; ++c) input_tile(c, false);
-    for (int c2 = 0; c2 < NC; ++c2) {
+    for (int c2 = 0; c2 < NC; ++c2) {                                             // layer 2 (TS), consumers one chunk behind
+        const int ci = nchunk++;
+        chunk_kind.push_back(1);
+        bool first = true;
+        int last_op = -1;
         for (int kb = 0; kb < NC; ++kb) {
-            if (!((P->nzmask[c2] >> kb) & 1)) continue;
-            const uint32_t off = new_tile(w2_bytes);
+            uint32_t kmask = 0;
             for (int r = 0; r < CH; ++r)
                 for (int k = 0; k < CH; ++k)
-                    put(off + sw128_offset(r, k), M->wm[1][(size_t)(c2 * CH + r) * H + kb * CH + k]);
+                    if (M->wm[1][(size_t)(c2 * CH + r) * H + kb * CH + k] != 0.0f) kmask |= 1u << (k / 16);
+            P->mma_dense += 4;
+            if (!kmask && !(first && kb == NC - 1)) continue;                     // exact: an all-zero tile adds 0
+            if (!kmask) kmask = 1;                                                // (never with a valid MADE mask)
+            uint32_t flags = F_A_TMEM | (first ? F_ACC0 : 0);
+            const uint32_t boff = stream_alloc(w2_bytes, &flags);
+            const uint32_t base = fill_start + boff;
+            for (int r = 0; r < CH; ++r)
+                for (int k = 0; k < CH; ++k)
+                    put(img, base + sw128_offset(r, k), M->wm[1][(size_t)(c2 * CH + r) * H + kb * CH + k]);
+            P->mma_issued += __builtin_popcount(kmask);
+            prog.push_back(make_op((uint32_t)kb * (CH / 2), boff, dcol(ci), id64, kmask, flags,
+                                   first ? free_wait(ci) : W_NONE, W_NONE, W_NONE, W_NONE));
+            last_op = (int)prog.size() - 1;
+            first = false;
         }
-        if (c2 >= 1) w3_tile(c2 - 1);
+        prog[last_op].c = (uint32_t)(BAR_DFULL + (ci & 1)) | (W_NONE << 8);
+        ChunkOp co{};
+        co.bias_off = (uint16_t)(2 * H + c2 * CH); co.kind = 1; co.dst_col = 0;
+        chunks.push_back(co);
+        // consumer of the previous in-place chunk (the last phase chunk, then layer-2 chunks)
+        const bool prev_phase = (c2 == 0);
+        consumer(prev, prev_c, prev_phase, false, first_d3); first_d3 = false;
+        prev = ci; prev_c = c2;
     }
-    w3_tile(NC - 1);
-    P->nprog = (int)prog.size();
+    consumer(prev, prev_c, false, true, false);
+    close_fill();
+    P->nprog = (int)prog.size(); P->nchunks = (int)chunks.size(); P->nfills = (int)fills.size();
+    P->res_bytes = (uint32_t)res.size();
+    if (P->nprog > MAX_OPS || (P->nchunks & 1)) { delete P; return NQS_EUNSUPPORTED; }
+
     // biases: [c1 | b1 | b2 | b3 (KO) | c2]
     std::vector<float> bias((size_t)3 * H + KO + 4, 0.f);
     for (int j = 0; j < H; ++j) { bias[j] = M->c1[j]; bias[H + j] = M->bias[0][j]; bias[2 * H + j] = M->bias[1][j]; }
     for (int d = 0; d < n; ++d) bias[3 * H + d] = M->bias[2][d];
     for (int o = 0; o < 4; ++o) bias[3 * H + KO + o] = M->c2[o];
-    // slots: as many as fit in 227 KB (max 22 barriers reserved)
-    int ns = 22;
-    while (ns > 2 && smem_layout(KI, H, KO, slot, ns).total > 227 * 1024 - 2048) --ns;
-    P->nslots = ns;
-    P->L = smem_layout(KI, H, KO, slot, ns);
+
     int dev = 0; cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&P->sms, cudaDevAttrMultiProcessorCount, dev);
-    bool ok = cudaMalloc(&P->d_wimg, img.size()) == cudaSuccess && cudaMalloc(&P->d_prog, prog.size() * sizeof(uint2)) == cudaSuccess &&
-              cudaMalloc(&P->d_bias, bias.size() * 4) == cudaSuccess;
-    ok = ok && cudaMemcpy(P->d_wimg, img.data(), img.size(), cudaMemcpyHostToDevice) == cudaSuccess &&
-         cudaMemcpy(P->d_prog, prog.data(), prog.size() * sizeof(uint2), cudaMemcpyHostToDevice) == cudaSuccess &&
-         cudaMemcpy(P->d_bias, bias.data(), bias.size() * 4, cudaMemcpyHostToDevice) == cudaSuccess;
+    auto up = [](void **dst, const void *src, size_t bytes) {
+        return cudaMalloc(dst, bytes ? bytes : 16) == cudaSuccess && (bytes == 0 || cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice) == cudaSuccess);
+    };
+    bool ok = up(&P->d_wimg, img.data(), img.size()) && up(&P->d_fills, fills.data(), fills.size() * sizeof(uint2)) &&
+              up(&P->d_prog, prog.data(), prog.size() * sizeof(MmaOp)) && up(&P->d_chunks, chunks.data(), chunks.size() * sizeof(ChunkOp)) &&
+              up(&P->d_res, res.data(), res.size()) && up(&P->d_bias, bias.data(), bias.size() * 4);
     ok = ok && cudaFuncSetAttribute(eloc_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->L.total) == cudaSuccess;
-    if (!ok) { cudaGetLastError(); cudaFree(P->d_wimg); cudaFree(P->d_prog); cudaFree(P->d_bias); delete P; return NQS_ECUDA; }
+    if (!ok) {
+        cudaGetLastError();
+        cudaFree(P->d_wimg); cudaFree(P->d_fills); cudaFree(P->d_prog); cudaFree(P->d_chunks); cudaFree(P->d_res); cudaFree(P->d_bias);
+        delete P;
+        return NQS_ECUDA;
+    }
     M->tc = P;
     return NQS_OK;
 }
 
 void tc_pack_free(const nqs_made *M) {
     if (!M->tc) return;
-    cudaFree(M->tc->d_wimg); cudaFree(M->tc->d_prog); cudaFree(M->tc->d_bias);
-    if (M->tc->d_fpos) cudaFree(M->tc->d_fpos);
-    if (M->tc->d_xpos) cudaFree(M->tc->d_xpos);
-    delete M->tc;
+    TcPack *P = M->tc;
+    cudaFree(P->d_wimg); cudaFree(P->d_fills); cudaFree(P->d_prog); cudaFree(P->d_chunks); cudaFree(P->d_res); cudaFree(P->d_bias);
+    if (P->d_fpos) cudaFree(P->d_fpos);
+    if (P->d_xpos) cudaFree(P->d_xpos);
+    delete P;
     M->tc = nullptr;
+}
+
+void tc_mma_counts(const nqs_made *M, long long *issued, long long *dense) {
+    *issued = M->tc ? M->tc->mma_issued : 0;
+    *dense = M->tc ? M->tc->mma_dense : 0;
 }
 
 static void fill_common(const nqs_made *M, TcParams &p) {
     const TcPack *P = M->tc;
     p.n = M->n; p.H = M->h; p.NC = P->NC; p.KI = P->KI; p.KO = P->KO;
-    p.wimg = (const uint8_t *)P->d_wimg; p.prog = (const uint2 *)P->d_prog; p.nprog = P->nprog;
+    p.tm_d = P->tm_d; p.tm_d3 = P->tm_d3;
+    p.wimg = (const uint8_t *)P->d_wimg; p.fills = (const uint2 *)P->d_fills; p.nfills = P->nfills;
+    p.prog = (const MmaOp *)P->d_prog; p.nprog = P->nprog;
+    p.chunks = (const ChunkOp *)P->d_chunks; p.nchunks = P->nchunks;
+    p.resimg = (const uint8_t *)P->d_res; p.res_bytes = P->res_bytes;
     p.slot_bytes = P->slot_bytes; p.nslots = P->nslots;
     p.bias = (const float *)P->d_bias;
-    memcpy(p.nzmask, P->nzmask, MAX_NC);
 }
 
 static int ensure(void **buf, size_t *cap, size_t bytes) {

@@ -97,3 +97,4 @@ int  launch_logpsi_tc(const nqs_made *made, const ulonglong2 *cfg, long long B, 
 int  launch_eloc_tc(const HamDev &hm, const nqs_made *made, const ulonglong2 *x, const float2 *base, long long B,
                     float2 *eloc, unsigned *max_ratio_bits, cudaStream_t st);
 size_t eloc_tc_ws_bytes(long long B, const HamDev &hm);
+void tc_mma_counts(const nqs_made *made, long long *issued, long long *dense);   // K-steps per tile: issued / dense chain
