@@ -29,25 +29,19 @@ constexpr int TILE_M = 128;
 constexpr int CH = 64;                   // hidden-unit chunk = accumulator columns
 constexpr int NTHREADS = 448;
 constexpr int MAX_NC = 8;                // hidden <= 512
-constexpr int MAX_OPS = 4 * MAX_NC + MAX_NC * MAX_NC;
 constexpr int MAX_SLOTS = 16;
 
 // barrier ids
 enum { BAR_A0FULL = 0, BAR_DFULL = 2, BAR_DFREE = 4, BAR_INPL = 6, BAR_D3FULL = 8, BAR_D3EMPTY = 9,
        BAR_WFULL = 10, BAR_WEMPTY = 10 + MAX_SLOTS, BAR_COUNT = 10 + 2 * MAX_SLOTS };
-constexpr uint32_t W_NONE = 0xFF, W_A0 = 0xFE;
 
-// One MMA group = one weight sub-tile: up to 8 K-steps (K = 16 each) into one accumulator.
-struct __align__(16) MmaOp {
-    uint32_t a;        // A operand: TS -> TMEM column offset; SS -> byte offset inside the A0 buffer
-    uint32_t b;        // B operand: byte offset inside the current ring slot (or from the smem base if F_B_RES)
-    uint32_t d;        // accumulator TMEM column offset
-    uint32_t idesc;
-    uint32_t w;        // kmask[0:8] | flags[8:16] | wait0[16:24] | wait1[24:32]
-    uint32_t c;        // commit0[0:8] | commit1[8:16]
-    uint32_t pad0, pad1;
-};
-enum { F_A_TMEM = 1, F_B_RES = 2, F_NEW_SLOT = 4, F_END_SLOT = 8, F_ACC0 = 16, F_B_NOSWZ = 32 };
+// Streamed weight sub-tiles are described by one 32-bit word each, in consumption order (kernel parameter
+// space -> uniform loads): offset inside the ring slot, ring hand-over flags and one small per-tile number.
+constexpr int MAX_SUB = 4 * MAX_NC + MAX_NC * MAX_NC;        // W1 + P1 + W2 blocks + W3
+constexpr uint32_t SUB_OFF_MASK = 0x7FFu;                    // [0:11)  byte offset inside the slot / 16
+constexpr uint32_t SUB_NEW = 1u << 11;                       // first sub-tile of a ring fill: wait for the fill
+constexpr uint32_t SUB_END = 1u << 12;                       // last sub-tile of a ring fill: release the slot
+constexpr int SUB_AUX_SHIFT = 16;                            // [16:24) input chunks: K-steps to issue; W2: k-block; W3: n_lo / 16
 
 struct ChunkOp { uint16_t bias_off; uint16_t dst_col; uint32_t kind; };   // kind 0: -> A1 at dst_col; 1: in place
 
@@ -62,7 +56,7 @@ __host__ __device__ inline SmemLayout smem_layout(int KI, int H, int KO, int NC,
     L.res = off; off += (uint32_t)NC * 2048;                     // resident P2 tiles (16 rows x 64 K, 128B swizzle)
     L.bias = off; off += (uint32_t)(3 * H + KO + 4) * 4;
     off = (off + 15) & ~15u;
-    L.prog = off; off += MAX_OPS * (uint32_t)sizeof(MmaOp);
+    L.prog = off;
     L.chunks = off; off += 3 * MAX_NC * (uint32_t)sizeof(ChunkOp);
     L.bars = off; off += BAR_COUNT * 8;
     off = (off + 1023) & ~1023u;
@@ -77,7 +71,8 @@ struct TcParams {
     const uint8_t *wimg;                 // packed streamed weight tiles
     const uint2 *fills;                  // per-tile ring fills: (byte offset, bytes), consumption order
     int nfills;
-    const MmaOp *prog; int nprog;        // per-tile MMA program
+    uint32_t sub[MAX_SUB];               // per-tile streamed sub-tiles (see SUB_*)
+    uint8_t nblk[MAX_NC];                // layer-2 k-blocks issued per output chunk
     const ChunkOp *chunks; int nchunks;  // per-tile accumulator chunks, in MMA order
     const uint8_t *resimg; uint32_t res_bytes;   // resident P2 tiles
     uint32_t slot_bytes; int nslots;
@@ -99,10 +94,6 @@ __device__ __forceinline__ unsigned long long shr128(ulonglong2 a, int s) {     
     if (s == 0) return a.x;
     if (s < 64) return (a.x >> s) | (a.y << (64 - s));
     return a.y >> (s - 64);
-}
-
-__device__ __forceinline__ float log_sigmoid_fast(float t) {
-    return fminf(t, 0.0f) - __logf(1.0f + __expf(-fabsf(t)));
 }
 
 __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_constant__ TcParams p) {
@@ -129,8 +120,6 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_const
     }
     if (warp == 1) tmem_alloc(&s_tmem_base, 512);
     for (int i = threadIdx.x; i < 3 * H + KO + 4; i += NTHREADS) s_bias[i] = p.bias[i];
-    for (int i = threadIdx.x; i < p.nprog * (int)(sizeof(MmaOp) / 16); i += NTHREADS)
-        reinterpret_cast<uint4 *>(smem + L.prog)[i] = reinterpret_cast<const uint4 *>(p.prog)[i];
     for (int i = threadIdx.x; i < p.nchunks * (int)(sizeof(ChunkOp) / 8); i += NTHREADS)
         reinterpret_cast<uint2 *>(smem + L.chunks)[i] = reinterpret_cast<const uint2 *>(p.chunks)[i];
     for (int i = threadIdx.x; i < (int)(p.res_bytes / 16); i += NTHREADS)
@@ -162,61 +151,126 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_const
             }
         }
     } else if (warp == 1) {
-        // =========================== MMA issuer: convergent warp, lane 0 issues ===========================
+        // =========================== MMA issuer: convergent warp, one elected lane issues ===========================
+        // The per-tile schedule is fixed code (stage A: layer 1 -> A1; stage P: phase hidden, in place, P2 one chunk
+        // behind; stage C: layer 2 from A1, in place, W3 one chunk behind); only the ring hand-over bits, the K-step
+        // counts and the k-block lists come from the parameter table.  Accumulator index b = chunk & 1 is a compile-
+        // time constant (loops unrolled by two), barrier parities live in the bits of `ph`.
         const uint32_t smem_base = smem_u32(smem);
-        const uint32_t a0_addr = smem_base + L.a0, slots_addr = smem_base + L.slots;
-        // descriptor high words: version 1 (bit 46); no-swizzle: lbo = 128 B, sbo = KI/8 * 128 B; 128B swizzle: sbo = 1024 B
+        const uint32_t a0_addr = smem_base + L.a0, slots_addr = smem_base + L.slots, res_addr = smem_base + L.res;
+        const uint32_t bars_addr = smem_base + L.bars;
         const uint64_t hi_noswz = ((uint64_t)(128 >> 4) << 16) | ((uint64_t)(((uint32_t)(KI / 8) * 128) >> 4) << 32) | (1ull << 46);
         const uint64_t hi_sw128 = ((uint64_t)(16 >> 4) << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
-        const MmaOp *prog = reinterpret_cast<const MmaOp *>(smem + L.prog);
-        unsigned long long ph = 0;                             // expected parity per barrier id (bit id)
-        uint32_t slot = 0, wpar = 0, tcount = 0;
-        for (long long t = t_lo; t < t_hi; ++t, ++tcount) {
-            const uint32_t a0_cur = a0_addr + (tcount & 1u) * L.a0_bytes;
-            for (int e = 0; e < p.nprog; ++e) {
-                const uint4 o0 = *reinterpret_cast<const uint4 *>(&prog[e]);
-                const uint2 o1 = *reinterpret_cast<const uint2 *>(&prog[e].w);
-                const uint32_t flags = (o1.x >> 8) & 0xFFu;
-                uint32_t kmask = o1.x & 0xFFu;
-#pragma unroll
-                for (int k = 0; k < 2; ++k) {
-                    uint32_t id = (o1.x >> (16 + 8 * k)) & 0xFFu;
-                    if (id != W_NONE) {
-                        if (id == W_A0) id = BAR_A0FULL + (tcount & 1u);
-                        mbar_wait(&bars[id], (uint32_t)(ph >> id) & 1u);
-                        ph ^= 1ull << id;
-                    }
-                }
-                if (flags & F_NEW_SLOT) mbar_wait(&bars[BAR_WFULL + slot], wpar);
-                tc_fence_after();
-                const uint32_t b_addr = (flags & F_B_RES) ? (smem_base + o0.y) : (slots_addr + slot * p.slot_bytes + o0.y);
-                const uint32_t d_addr = tmem + o0.z;
-                uint32_t acc = (flags & F_ACC0) ? 0u : 1u;
-                const uint64_t b_hi = (flags & F_B_NOSWZ) ? hi_noswz : hi_sw128;
-                const uint32_t b_step = (flags & F_B_NOSWZ) ? 16u : 2u;      // 256 B / 32 B per K-step, in 16 B units
-                uint32_t b_lo = (b_addr >> 4) & 0x3FFFu;
-                if (elect_one()) {
-                    if (flags & F_A_TMEM) {
-                        uint32_t a_t = tmem + o0.x;
-#pragma unroll
-                        for (int ks = 0; ks < 4; ++ks) {
-                            if (kmask & 1u) { mma_ts(d_addr, a_t, b_hi | b_lo, o0.w, acc != 0); acc = 1u; }
-                            kmask >>= 1; a_t += 8; b_lo += b_step;
-                        }
-                    } else {
-                        uint32_t a_lo = ((a0_cur + o0.x) >> 4) & 0x3FFFu;
+        const uint32_t id64 = idesc_f16(128, 64), id16 = idesc_f16(128, 16);
+        const uint32_t NC = (uint32_t)p.NC;
+        const uint32_t tm_d = tmem + p.tm_d, tm_d3 = tmem + p.tm_d3, tm_ph = tm_d3 + (uint32_t)KO - 16;
+        uint32_t ph = 0, slot = 0, wpar = 0, tcount = 0, slot_lo = (slots_addr >> 4) & 0x3FFFu;
+        auto bar_wait = [&](uint32_t id) {
+            mbar_wait_addr(bars_addr + id * 8, (ph >> id) & 1u);
+            ph ^= 1u << id;
+        };
+        auto slot_acquire = [&](uint32_t w) {
+            if (w & SUB_NEW) mbar_wait_addr(bars_addr + (BAR_WFULL + slot) * 8, wpar);
+        };
+        auto slot_release = [&](uint32_t w) {               // after the (elected) commit to WEMPTY[slot]
+            if (w & SUB_END) {
+                if (++slot == (uint32_t)p.nslots) { slot = 0; wpar ^= 1u; }
+                slot_lo = ((slots_addr + slot * p.slot_bytes) >> 4) & 0x3FFFu;
+            }
+        };
+        // input-layer chunk (SS): D[b] = A0 . Wc^T over the first nk K-steps (a prefix: masked columns are the high ones)
+        auto input_chunk = [&](uint32_t w, uint32_t a0_lo, uint32_t b) {
+            slot_acquire(w);
+            tc_fence_after();
+            const uint32_t nk = (w >> SUB_AUX_SHIFT) & 0xFFu;
+            uint32_t b_lo = slot_lo + (w & SUB_OFF_MASK);
+            if (elect_one()) {
+                uint32_t a_lo = a0_lo;
 #pragma unroll 1
-                        for (; kmask; kmask >>= 1, a_lo += 16, b_lo += b_step)
-                            if (kmask & 1u) { mma_ss(d_addr, hi_noswz | a_lo, b_hi | b_lo, o0.w, acc != 0); acc = 1u; }
-                    }
-                    if (flags & F_END_SLOT) mma_commit(&bars[BAR_WEMPTY + slot]);
-                    const uint32_t c0 = o1.y & 0xFFu, c1 = (o1.y >> 8) & 0xFFu;
-                    if (c0 != W_NONE) mma_commit(&bars[c0]);
-                    if (c1 != W_NONE) mma_commit(&bars[c1]);
+                for (uint32_t ks = 0; ks < nk; ++ks, a_lo += 16, b_lo += 16)
+                    mma_ss(tm_d + b * CH, hi_noswz | a_lo, hi_noswz | b_lo, id64, ks != 0);
+                if (w & SUB_END) mma_commit_addr(bars_addr + (BAR_WEMPTY + slot) * 8);
+                mma_commit_addr(bars_addr + (BAR_DFULL + b) * 8);
+            }
+            __syncwarp();
+            slot_release(w);
+        };
+        // consumer of the in-place fp16 chunk in D[b]: dst (+)= D[b] . B^T, 4 K-steps of 16
+        auto consume = [&](uint32_t b, uint32_t b_lo, uint32_t dst, uint32_t idesc, uint32_t end_bar, uint32_t rel_slot) {
+            if (elect_one()) {
+                const uint32_t a_t = tm_d + b * CH;
+#pragma unroll
+                for (uint32_t ks = 0; ks < 4; ++ks) mma_ts(dst, a_t + 8 * ks, hi_sw128 | (b_lo + 2 * ks), idesc, true);
+                if (rel_slot) mma_commit_addr(bars_addr + (BAR_WEMPTY + slot) * 8);
+                if (end_bar) mma_commit_addr(bars_addr + end_bar * 8);
+            }
+            __syncwarp();
+        };
+        auto consume_phase = [&](uint32_t c, uint32_t b) {                  // P2 tile c is resident
+            bar_wait(BAR_INPL + b);
+            if (c == 0) bar_wait(BAR_D3EMPTY);                               // first write into D3 of this tile
+            tc_fence_after();
+            consume(b, ((res_addr + c * 2048) >> 4) & 0x3FFFu, tm_ph, id16, 0, 0);
+        };
+        auto consume_w3 = [&](uint32_t w, uint32_t b, uint32_t end_bar) {   // streamed layer-3 tile
+            bar_wait(BAR_INPL + b);
+            slot_acquire(w);
+            tc_fence_after();
+            const uint32_t nlo = ((w >> SUB_AUX_SHIFT) & 0xFFu) * 16;       // output rows below n_lo receive exactly 0
+            consume(b, slot_lo + (w & SUB_OFF_MASK) + (nlo / 8) * 64, tm_d3 + nlo, idesc_f16(128, KO - (int)nlo), end_bar,
+                    w & SUB_END);
+            slot_release(w);
+        };
+        auto l2_chunk = [&](uint32_t c2, uint32_t b, uint32_t &si) {        // D[b] = A1 . W2[c2]^T over the listed k-blocks
+            const uint32_t nb = p.nblk[c2];
+#pragma unroll 1
+            for (uint32_t j = 0; j < nb; ++j) {
+                const uint32_t w = p.sub[si++];
+                slot_acquire(w);
+                tc_fence_after();
+                const uint32_t kb = (w >> SUB_AUX_SHIFT) & 0xFFu;
+                const uint32_t b_lo = slot_lo + (w & SUB_OFF_MASK);
+                if (elect_one()) {
+                    const uint32_t a_t = tmem + kb * (CH / 2);
+#pragma unroll
+                    for (uint32_t ks = 0; ks < 4; ++ks)
+                        mma_ts(tm_d + b * CH, a_t + 8 * ks, hi_sw128 | (b_lo + 2 * ks), id64, (j | ks) != 0);
+                    if (w & SUB_END) mma_commit_addr(bars_addr + (BAR_WEMPTY + slot) * 8);
+                    if (j + 1 == nb) mma_commit_addr(bars_addr + (BAR_DFULL + b) * 8);
                 }
                 __syncwarp();
-                if (flags & F_END_SLOT) { if (++slot == (uint32_t)p.nslots) { slot = 0; wpar ^= 1u; } }
+                slot_release(w);
             }
+        };
+        for (long long t = t_lo; t < t_hi; ++t, ++tcount) {
+            const uint32_t a0_lo = ((a0_addr + (tcount & 1u) * L.a0_bytes) >> 4) & 0x3FFFu;
+            uint32_t si = 0;
+            // ---- stage A: layer 1, epilogue -> A1 (frees the accumulator) ----
+            bar_wait(BAR_A0FULL + (tcount & 1u));
+            for (uint32_t c = 0; c < NC; c += 2) {
+                if (c >= 2) bar_wait(BAR_DFREE + 0);
+                input_chunk(p.sub[si++], a0_lo, 0);
+                if (c >= 2) bar_wait(BAR_DFREE + 1);
+                input_chunk(p.sub[si++], a0_lo, 1);
+            }
+            // ---- stage P: phase hidden layer, in place; its consumer runs one chunk behind ----
+            for (uint32_t c = 0; c < NC; c += 2) {
+                if (c == 0) bar_wait(BAR_DFREE + 0);          // last stage-A chunk of group 0 (=> all of its A1 is written)
+                input_chunk(p.sub[si++], a0_lo, 0);
+                if (c >= 2) consume_phase(c - 1, 1);
+                if (c == 0) bar_wait(BAR_DFREE + 1);
+                input_chunk(p.sub[si++], a0_lo, 1);
+                consume_phase(c, 0);
+            }
+            // ---- stage C: layer 2 from A1 (TS), in place; consumers (P2 of the last phase chunk, then W3) one behind ----
+            for (uint32_t c2 = 0; c2 < NC; c2 += 2) {
+                l2_chunk(c2, 0, si);
+                if (c2 == 0) consume_phase(NC - 1, 1);
+                else consume_w3(p.sub[si++], 1, 0);
+                l2_chunk(c2 + 1, 1, si);
+                consume_w3(p.sub[si++], 0, 0);
+            }
+            consume_w3(p.sub[si++], 1, BAR_D3FULL);
         }
     } else if (warp < 10) {
         // =========================== chunk epilogue groups: group g owns accumulator D[g] ===========================
@@ -334,7 +388,9 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_const
             // ---- final epilogue: log|psi| = 1/2 sum_d log sigmoid(+-a_d), phi = o[2 z_{n-2} + z_{n-1}] ----
             mbar_wait(&bars[BAR_D3FULL], tcount & 1u);
             tc_fence_after();
-            float part = 0.0f, phi = 0.0f;
+            // sum_d log sigmoid(t_d) = sum_d min(t_d, 0) - ln prod_d (1 + exp(-|t_d|)): every factor is in (1, 2], so a
+            // 16-term product cannot overflow and costs one LG2 per 16 conditionals; the 16 chains are independent (ILP).
+            float msum = 0.0f, lg = 0.0f, phi = 0.0f;
             for (int c0 = 0; c0 < KO; c0 += 16) {
                 uint32_t v[16];
                 tmem_ld16p(d3_addr + c0, v);
@@ -346,16 +402,29 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_const
                     const float o2 = __uint_as_float(v[14]) + s_c2[2], o3 = __uint_as_float(v[15]) + s_c2[3];
                     phi = sel == 0 ? o0 : (sel == 1 ? o1 : (sel == 2 ? o2 : o3));
                 }
-                const unsigned long long zb = shr128(zp, c0);
+                const uint32_t zb = (uint32_t)shr128(zp, c0);
+                const int nv = p.n - c0;                       // valid conditionals in this block (may be <= 0 or >= 16)
+                const float4 *bp = reinterpret_cast<const float4 *>(s_b3 + c0);
+                float prod0 = 1.0f, prod1 = 1.0f, m0 = 0.0f, m1 = 0.0f;
 #pragma unroll
-                for (int k = 0; k < 16; ++k) {
-                    const int d = c0 + k;
-                    if (d < p.n) {
-                        const float a = __uint_as_float(v[k]) + s_b3[d];
-                        part += log_sigmoid_fast(((zb >> k) & 1ull) ? a : -a);
+                for (int k4 = 0; k4 < 4; ++k4) {
+                    const float4 bb = bp[k4];
+                    const float bk[4] = {bb.x, bb.y, bb.z, bb.w};
+#pragma unroll
+                    for (int kk = 0; kk < 4; ++kk) {
+                        const int k = 4 * k4 + kk;
+                        const float a = __uint_as_float(v[k]) + bk[kk];
+                        float t = ((zb >> k) & 1u) ? a : -a;
+                        t = (k < nv) ? t : 1e30f;              // padding column: factor 1, min 0
+                        const float e = ex2_ftz(fabsf(t) * -1.4426950408889634f);
+                        if (k & 1) { prod1 *= 1.0f + e; m1 += fminf(t, 0.0f); }
+                        else       { prod0 *= 1.0f + e; m0 += fminf(t, 0.0f); }
                     }
                 }
+                msum += m0 + m1;
+                lg += lg2_ftz(prod0 * prod1);
             }
+            const float part = msum - 0.6931471805599453f * lg;
             tmem_wait_st();
             tc_fence_before();
             __syncwarp();
@@ -427,12 +496,14 @@ __global__ void diag_init_kernel(HamDev hm, const ulonglong2 *__restrict__ x, lo
 
 // ------------------------------------------------------------------------------------------------------------
 struct TcPack {
-    int KI = 0, KO = 0, NC = 0, nprog = 0, nchunks = 0, nfills = 0, nslots = 0;
+    int KI = 0, KO = 0, NC = 0, nsub = 0, nchunks = 0, nfills = 0, nslots = 0;
     uint32_t slot_bytes = 0, res_bytes = 0, tm_d = 0, tm_d3 = 0;
-    void *d_wimg = nullptr, *d_fills = nullptr, *d_prog = nullptr, *d_chunks = nullptr, *d_res = nullptr, *d_bias = nullptr;
+    void *d_wimg = nullptr, *d_fills = nullptr, *d_chunks = nullptr, *d_res = nullptr, *d_bias = nullptr;
     void *d_fpos = nullptr; size_t fpos_cap = 0; const void *fpos_for = nullptr; long long fpos_G = -1;
     void *d_xpos = nullptr; size_t xpos_cap = 0;
     SmemLayout L{};
+    uint32_t sub[MAX_SUB] = {0};
+    uint8_t nblk[MAX_NC] = {0};
     int sms = 148;
     long long mma_issued = 0, mma_dense = 0;                   // K-steps issued / K-steps of the dense chain, per tile
 };
@@ -477,56 +548,36 @@ int tc_pack_upload(const nqs_made *M) {
 
     std::vector<uint8_t> img, res((size_t)NC * 2048, 0);
     std::vector<uint2> fills;
-    std::vector<MmaOp> prog;
+    std::vector<uint32_t> sub;
     std::vector<ChunkOp> chunks;
     auto put = [](std::vector<uint8_t> &buf, uint32_t off, float v) { __half hv = __float2half_rn(v); memcpy(&buf[off], &hv, 2); };
 
-    // ---- streamed sub-tiles are appended to the open fill (<= slot bytes, in consumption order) ----
+    // ---- streamed sub-tiles are appended to the open ring fill (<= slot bytes, in consumption order) ----
     uint32_t fill_start = 0, fill_bytes = 0;
-    int open_first_op = -1, last_stream_op = -1;
     auto close_fill = [&]() {
         if (fill_bytes == 0) return;
         fills.push_back(make_uint2(fill_start, fill_bytes));
-        prog[last_stream_op].w |= (uint32_t)F_END_SLOT << 8;
-        fill_bytes = 0; open_first_op = -1;
+        sub.back() |= SUB_END;
+        fill_bytes = 0;
     };
-    // reserve `bytes` of streamed image for the op about to be pushed; returns the offset inside its slot
-    auto stream_alloc = [&](uint32_t bytes, uint32_t *flags) -> uint32_t {
+    // reserve `bytes` of streamed image for the next sub-tile; pushes its table word, returns its image offset
+    auto stream_alloc = [&](uint32_t bytes, uint32_t aux) -> uint32_t {
         if (fill_bytes + bytes > slot) close_fill();
-        if (fill_bytes == 0) { fill_start = (uint32_t)img.size(); *flags |= F_NEW_SLOT; open_first_op = (int)prog.size(); }
-        const uint32_t off_in_slot = fill_bytes;
+        uint32_t w = (aux & 0xFFu) << SUB_AUX_SHIFT;
+        if (fill_bytes == 0) { fill_start = (uint32_t)img.size(); w |= SUB_NEW; }
+        w |= (fill_bytes >> 4) & SUB_OFF_MASK;
+        const uint32_t base = fill_start + fill_bytes;
         img.resize(img.size() + bytes, 0);
         fill_bytes += bytes;
-        last_stream_op = (int)prog.size();
-        return off_in_slot;
-    };
-    auto make_op = [](uint32_t a, uint32_t b, uint32_t d, uint32_t idesc, uint32_t kmask, uint32_t flags, uint32_t w0, uint32_t w1,
-                      uint32_t c0, uint32_t c1) {
-        MmaOp o{};
-        o.a = a; o.b = b; o.d = d; o.idesc = idesc;
-        o.w = (kmask & 0xFF) | ((flags & 0xFF) << 8) | ((w0 & 0xFF) << 16) | ((w1 & 0xFF) << 24);
-        o.c = (c0 & 0xFF) | ((c1 & 0xFF) << 8);
-        return o;
+        sub.push_back(w);
+        return base;
     };
 
-    const uint32_t id64 = idesc_f16(128, 64), id16 = idesc_f16(128, 16);
-    int nchunk = 0;                          // running accumulator-chunk index inside the tile
-    std::vector<int> chunk_kind;             // 0 = -> A1 (epilogue frees the accumulator), 1 = in place
-    auto dcol = [&](int ci) { return P->tm_d + (uint32_t)(ci & 1) * CH; };
-    // wait needed before overwriting accumulator (ci & 1): only when its previous user was a kind-0 chunk of THIS tile
-    // (in-place chunks are released by tensor-pipe order: their consumer MMAs are issued before the overwrite)
-    auto free_wait = [&](int ci) -> uint32_t {
-        return (ci >= 2 && chunk_kind[ci - 2] == 0) ? (uint32_t)(BAR_DFREE + (ci & 1)) : W_NONE;
-    };
-
-    // input-layer chunk c (layer 1 or phase hidden): D[b] = A0 . Wc^T
-    auto input_chunk = [&](int c, bool phase, bool first_of_tile) {
-        const int ci = nchunk++;
-        chunk_kind.push_back(phase ? 1 : 0);
-        uint32_t flags = F_B_NOSWZ | F_ACC0;
-        const uint32_t boff = stream_alloc(in_bytes, &flags);
-        const uint32_t base = fill_start + boff;
-        uint32_t kmask = 0;
+    // input-layer chunk c (layer 1 or phase hidden): D = A0 . Wc^T.  Masked layer-1 columns are the high ones
+    // (M1[j][d] = deg[j] >= d+1), so the K-steps to issue are a prefix.
+    auto input_chunk = [&](int c, bool phase) {
+        const uint32_t base = stream_alloc(in_bytes, 0);
+        int nk = 1;                                             // the accumulator must be overwritten even if all zero
         for (int r = 0; r < CH; ++r) {
             const int j = c * CH + r;
             for (int k = 0; k < KI; ++k) {
@@ -534,104 +585,72 @@ int tc_pack_upload(const nqs_made *M) {
                 if (phase) { if (k < n - 2) v = M->p1[(size_t)j * (n - 2) + k]; }
                 else if (k < n) v = M->wm[0][(size_t)j * n + k];
                 put(img, base + noswz_offset(r, k, KI), v);
-                if (v != 0.0f) kmask |= 1u << (k / 16);
+                if (v != 0.0f && k / 16 + 1 > nk) nk = k / 16 + 1;
             }
         }
-        if (!kmask) kmask = 1;                                  // the accumulator must still be overwritten
-        P->mma_issued += __builtin_popcount(kmask); P->mma_dense += KI / 16;
-        prog.push_back(make_op(0, boff, dcol(ci), id64, kmask, flags, first_of_tile ? W_A0 : W_NONE, free_wait(ci),
-                               BAR_DFULL + (ci & 1), W_NONE));
-        // K-steps are addressed from the start of the tile; skipped ones are simply not issued
+        sub.back() |= (uint32_t)nk << SUB_AUX_SHIFT;
+        P->mma_issued += nk; P->mma_dense += KI / 16;
         ChunkOp co{};
         co.bias_off = (uint16_t)((phase ? 0 : H) + c * CH);
         co.kind = phase ? 1 : 0;
         co.dst_col = (uint16_t)(c * (CH / 2));
         chunks.push_back(co);
-        return ci;
     };
-    // consumer of an in-place chunk: D3 (+)= D[ci] . Wc^T  (P2 resident tile or streamed layer-3 tile)
-    auto consumer = [&](int ci, int c, bool phase, bool last_of_tile, bool first_d3) {
-        uint32_t flags = F_A_TMEM, boff, kmask = 0, dst = P->tm_d3, idesc = 0;
-        if (phase) {
-            flags |= F_B_RES;
-            boff = P->L.res + (uint32_t)c * 2048;
-            for (int o = 0; o < 4; ++o)
-                for (int k = 0; k < CH; ++k) {
-                    const float v = M->p2[(size_t)o * H + c * CH + k];
-                    put(res, (uint32_t)c * 2048 + sw128_offset(12 + o, k), v);
-                    if (v != 0.0f) kmask |= 1u << (k / 16);
-                }
-            dst += (uint32_t)KO - 16; idesc = id16;
-            P->mma_dense += 4;
-        } else {
-            boff = stream_alloc(w3_bytes, &flags);
-            const uint32_t base = fill_start + boff;
-            int row_lo = KO;
-            for (int d = 0; d < n; ++d)
-                for (int k = 0; k < CH; ++k) {
-                    const float v = M->wm[2][(size_t)d * H + c * CH + k];
-                    put(img, base + sw128_offset(d, k), v);
-                    if (v != 0.0f) { kmask |= 1u << (k / 16); if (d < row_lo) row_lo = d; }
-                }
-            // output rows below the first nonzero one receive exactly 0 from this chunk: start the MMA at a 16-row boundary
-            const int n_lo = kmask ? (row_lo / 16) * 16 : 0;
-            boff += (uint32_t)(n_lo / 8) * 1024; dst += (uint32_t)n_lo;
-            idesc = idesc_f16(128, KO - n_lo);
-            P->mma_dense += 4;
-        }
-        P->mma_issued += __builtin_popcount(kmask);
-        prog.push_back(make_op(dcol(ci), boff, dst, idesc, kmask, flags, BAR_INPL + (ci & 1), first_d3 ? BAR_D3EMPTY : W_NONE,
-                               last_of_tile ? BAR_D3FULL : W_NONE, W_NONE));
+    // resident P2 tile of phase chunk c: rows 12..15 of a 16-row tile hold the 4 phase outputs
+    auto phase_out_tile = [&](int c) {
+        for (int o = 0; o < 4; ++o)
+            for (int k = 0; k < CH; ++k) put(res, (uint32_t)c * 2048 + sw128_offset(12 + o, k), M->p2[(size_t)o * H + c * CH + k]);
+        P->mma_issued += 4; P->mma_dense += 4;
+    };
+    // streamed layer-3 tile of hidden chunk c; output rows below the first nonzero one receive exactly 0 from this
+    // chunk, so the MMA starts at a 16-row boundary n_lo (Mout[d][j] = d+1 > deg[j])
+    auto w3_tile = [&](int c) {
+        const uint32_t base = stream_alloc(w3_bytes, 0);
+        int row_lo = KO;
+        for (int d = 0; d < n; ++d)
+            for (int k = 0; k < CH; ++k) {
+                const float v = M->wm[2][(size_t)d * H + c * CH + k];
+                put(img, base + sw128_offset(d, k), v);
+                if (v != 0.0f && d < row_lo) row_lo = d;
+            }
+        const int n_lo = row_lo >= KO ? 0 : (row_lo / 16) * 16;
+        sub.back() |= (uint32_t)(n_lo / 16) << SUB_AUX_SHIFT;
+        P->mma_issued += 4; P->mma_dense += 4;
     };
 
-    // ---- the per-tile program ----
-    for (int c = 0; c < NC; ++c) input_chunk(c, false, c == 0);                  // layer 1 -> A1
-    int prev = -1, prev_c = -1;
-    bool first_d3 = true;
-    for (int c = 0; c < NC; ++c) {                                                // phase hidden, P2 one chunk behind
-        const int ci = input_chunk(c, true, false);
-        if (prev >= 0) { consumer(prev, prev_c, true, false, first_d3); first_d3 = false; }
-        prev = ci; prev_c = c;
-    }
-    for (int c2 = 0; c2 < NC; ++c2) {                                             // layer 2 (TS), consumers one chunk behind
-        const int ci = nchunk++;
-        chunk_kind.push_back(1);
-        bool first = true;
-        int last_op = -1;
+    // ---- the per-tile schedule (must match the MMA issuer in eloc_tc_kernel) ----
+    for (int c = 0; c < NC; ++c) input_chunk(c, false);                          // stage A: layer 1 -> A1
+    for (int c = 0; c < NC; ++c) { input_chunk(c, true); phase_out_tile(c); }     // stage P: phase hidden, in place
+    uint8_t nblk[MAX_NC] = {0};
+    for (int c2 = 0; c2 < NC; ++c2) {                                             // stage C: layer 2 (TS), in place
+        int nb = 0;
         for (int kb = 0; kb < NC; ++kb) {
-            uint32_t kmask = 0;
-            for (int r = 0; r < CH; ++r)
+            bool any = false;
+            for (int r = 0; r < CH && !any; ++r)
                 for (int k = 0; k < CH; ++k)
-                    if (M->wm[1][(size_t)(c2 * CH + r) * H + kb * CH + k] != 0.0f) kmask |= 1u << (k / 16);
+                    if (M->wm[1][(size_t)(c2 * CH + r) * H + kb * CH + k] != 0.0f) { any = true; break; }
             P->mma_dense += 4;
-            if (!kmask && !(first && kb == NC - 1)) continue;                     // exact: an all-zero tile adds 0
-            if (!kmask) kmask = 1;                                                // (never with a valid MADE mask)
-            uint32_t flags = F_A_TMEM | (first ? F_ACC0 : 0);
-            const uint32_t boff = stream_alloc(w2_bytes, &flags);
-            const uint32_t base = fill_start + boff;
+            if (!any && !(nb == 0 && kb == NC - 1)) continue;                     // exact: an all-zero block adds 0
+            const uint32_t base = stream_alloc(w2_bytes, (uint32_t)kb);
             for (int r = 0; r < CH; ++r)
                 for (int k = 0; k < CH; ++k)
                     put(img, base + sw128_offset(r, k), M->wm[1][(size_t)(c2 * CH + r) * H + kb * CH + k]);
-            P->mma_issued += __builtin_popcount(kmask);
-            prog.push_back(make_op((uint32_t)kb * (CH / 2), boff, dcol(ci), id64, kmask, flags,
-                                   first ? free_wait(ci) : W_NONE, W_NONE, W_NONE, W_NONE));
-            last_op = (int)prog.size() - 1;
-            first = false;
+            P->mma_issued += 4;
+            ++nb;
         }
-        prog[last_op].c = (uint32_t)(BAR_DFULL + (ci & 1)) | (W_NONE << 8);
+        nblk[c2] = (uint8_t)nb;
         ChunkOp co{};
         co.bias_off = (uint16_t)(2 * H + c2 * CH); co.kind = 1; co.dst_col = 0;
         chunks.push_back(co);
-        // consumer of the previous in-place chunk (the last phase chunk, then layer-2 chunks)
-        const bool prev_phase = (c2 == 0);
-        consumer(prev, prev_c, prev_phase, false, first_d3); first_d3 = false;
-        prev = ci; prev_c = c2;
+        if (c2 >= 1) w3_tile(c2 - 1);                                             // consumer of the previous layer-2 chunk
     }
-    consumer(prev, prev_c, false, true, false);
+    w3_tile(NC - 1);
     close_fill();
-    P->nprog = (int)prog.size(); P->nchunks = (int)chunks.size(); P->nfills = (int)fills.size();
+    P->nsub = (int)sub.size(); P->nchunks = (int)chunks.size(); P->nfills = (int)fills.size();
     P->res_bytes = (uint32_t)res.size();
-    if (P->nprog > MAX_OPS || (P->nchunks & 1)) { delete P; return NQS_EUNSUPPORTED; }
+    if (P->nsub > MAX_SUB || (P->nchunks & 1)) { delete P; return NQS_EUNSUPPORTED; }
+    memcpy(P->sub, sub.data(), sub.size() * 4);
+    memcpy(P->nblk, nblk, sizeof(nblk));
 
     // biases: [c1 | b1 | b2 | b3 (KO) | c2]
     std::vector<float> bias((size_t)3 * H + KO + 4, 0.f);
@@ -645,12 +664,12 @@ int tc_pack_upload(const nqs_made *M) {
         return cudaMalloc(dst, bytes ? bytes : 16) == cudaSuccess && (bytes == 0 || cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice) == cudaSuccess);
     };
     bool ok = up(&P->d_wimg, img.data(), img.size()) && up(&P->d_fills, fills.data(), fills.size() * sizeof(uint2)) &&
-              up(&P->d_prog, prog.data(), prog.size() * sizeof(MmaOp)) && up(&P->d_chunks, chunks.data(), chunks.size() * sizeof(ChunkOp)) &&
+              up(&P->d_chunks, chunks.data(), chunks.size() * sizeof(ChunkOp)) &&
               up(&P->d_res, res.data(), res.size()) && up(&P->d_bias, bias.data(), bias.size() * 4);
     ok = ok && cudaFuncSetAttribute(eloc_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->L.total) == cudaSuccess;
     if (!ok) {
         cudaGetLastError();
-        cudaFree(P->d_wimg); cudaFree(P->d_fills); cudaFree(P->d_prog); cudaFree(P->d_chunks); cudaFree(P->d_res); cudaFree(P->d_bias);
+        cudaFree(P->d_wimg); cudaFree(P->d_fills); cudaFree(P->d_chunks); cudaFree(P->d_res); cudaFree(P->d_bias);
         delete P;
         return NQS_ECUDA;
     }
@@ -661,7 +680,7 @@ int tc_pack_upload(const nqs_made *M) {
 void tc_pack_free(const nqs_made *M) {
     if (!M->tc) return;
     TcPack *P = M->tc;
-    cudaFree(P->d_wimg); cudaFree(P->d_fills); cudaFree(P->d_prog); cudaFree(P->d_chunks); cudaFree(P->d_res); cudaFree(P->d_bias);
+    cudaFree(P->d_wimg); cudaFree(P->d_fills); cudaFree(P->d_chunks); cudaFree(P->d_res); cudaFree(P->d_bias);
     if (P->d_fpos) cudaFree(P->d_fpos);
     if (P->d_xpos) cudaFree(P->d_xpos);
     delete P;
@@ -678,7 +697,7 @@ static void fill_common(const nqs_made *M, TcParams &p) {
     p.n = M->n; p.H = M->h; p.NC = P->NC; p.KI = P->KI; p.KO = P->KO;
     p.tm_d = P->tm_d; p.tm_d3 = P->tm_d3;
     p.wimg = (const uint8_t *)P->d_wimg; p.fills = (const uint2 *)P->d_fills; p.nfills = P->nfills;
-    p.prog = (const MmaOp *)P->d_prog; p.nprog = P->nprog;
+    memcpy(p.sub, P->sub, sizeof(p.sub)); memcpy(p.nblk, P->nblk, sizeof(p.nblk));
     p.chunks = (const ChunkOp *)P->d_chunks; p.nchunks = P->nchunks;
     p.resimg = (const uint8_t *)P->d_res; p.res_bytes = P->res_bytes;
     p.slot_bytes = P->slot_bytes; p.nslots = P->nslots;
