@@ -30,6 +30,7 @@ constexpr int CH = 64;                   // hidden-unit chunk = accumulator colu
 constexpr int NTHREADS = 448;
 constexpr int MAX_NC = 8;                // hidden <= 512
 constexpr int MAX_SLOTS = 16;
+constexpr int NPROD = 4;                 // producer lanes (bulk-copy issuers)
 
 // barrier ids
 enum { BAR_A0FULL = 0, BAR_DFULL = 2, BAR_DFREE = 4, BAR_INPL = 6, BAR_D3FULL = 8, BAR_D3EMPTY = 9,
@@ -137,141 +138,134 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_const
     const long long t_lo = ntiles * blockIdx.x / gridDim.x, t_hi = ntiles * (blockIdx.x + 1) / gridDim.x;
 
     if (warp == 0) {
-        // =========================== weight producer (TMA engine, 1-D bulk copies) ===========================
-        if (lane == 0) {
-            uint32_t slot = 0, par = 1;                         // a fresh barrier passes a parity-1 wait
-            for (long long t = t_lo; t < t_hi; ++t) {
-                for (int e = 0; e < p.nfills; ++e) {
-                    const uint2 pe = __ldg(&p.fills[e]);
-                    mbar_wait(&bars[BAR_WEMPTY + slot], par);
-                    mbar_arrive_expect_tx(&bars[BAR_WFULL + slot], pe.y);
-                    bulk_g2s(smem + L.slots + slot * p.slot_bytes, p.wimg + pe.x, pe.y, &bars[BAR_WFULL + slot]);
-                    if (++slot == (uint32_t)p.nslots) { slot = 0; par ^= 1; }
-                }
+        // =========================== weight producers (TMA engine, 1-D bulk copies) ===========================
+        // One thread sustains about one ring fill per ~700 cycles (measured: the rate does not depend on the fill
+        // size), so NPROD lanes share the fills round-robin; fill q always lands in slot q % nslots.
+        if (lane < NPROD) {
+            const long long total = (t_hi - t_lo) * (long long)p.nfills;
+            uint32_t e = (uint32_t)lane % (uint32_t)p.nfills, slot = (uint32_t)lane % (uint32_t)p.nslots;
+            uint32_t par = 1u ^ (((uint32_t)lane / (uint32_t)p.nslots) & 1u);   // a fresh barrier passes a parity-1 wait
+            for (long long q = lane; q < total; q += NPROD) {
+                const uint2 pe = __ldg(&p.fills[e]);
+                mbar_wait(&bars[BAR_WEMPTY + slot], par);
+                mbar_arrive_expect_tx(&bars[BAR_WFULL + slot], pe.y);
+                bulk_g2s(smem + L.slots + slot * p.slot_bytes, p.wimg + pe.x, pe.y, &bars[BAR_WFULL + slot]);
+                e += NPROD; while (e >= (uint32_t)p.nfills) e -= (uint32_t)p.nfills;
+                slot += NPROD; while (slot >= (uint32_t)p.nslots) { slot -= (uint32_t)p.nslots; par ^= 1u; }
             }
         }
     } else if (warp == 1) {
-        // =========================== MMA issuer: convergent warp, one elected lane issues ===========================
+        // =========================== MMA issuer: convergent warp, lane 0 issues (predicated) ===========================
+        // Every lane runs the same warp-uniform control flow so descriptors live in uniform registers; only the
+        // tcgen05.mma / tcgen05.commit instructions are predicated on `issue` (lane 0).
         // The per-tile schedule is fixed code (stage A: layer 1 -> A1; stage P: phase hidden, in place, P2 one chunk
         // behind; stage C: layer 2 from A1, in place, W3 one chunk behind); only the ring hand-over bits, the K-step
-        // counts and the k-block lists come from the parameter table.  Accumulator index b = chunk & 1 is a compile-
-        // time constant (loops unrolled by two), barrier parities live in the bits of `ph`.
-        const uint32_t smem_base = smem_u32(smem);
-        const uint32_t a0_addr = smem_base + L.a0, slots_addr = smem_base + L.slots, res_addr = smem_base + L.res;
-        const uint32_t bars_addr = smem_base + L.bars;
-        const uint64_t hi_noswz = ((uint64_t)(128 >> 4) << 16) | ((uint64_t)(((uint32_t)(KI / 8) * 128) >> 4) << 32) | (1ull << 46);
-        const uint64_t hi_sw128 = ((uint64_t)(16 >> 4) << 16) | ((uint64_t)(1024 >> 4) << 32) | (1ull << 46) | (2ull << 61);
-        const uint32_t id64 = idesc_f16(128, 64), id16 = idesc_f16(128, 16);
-        const uint32_t NC = (uint32_t)p.NC;
-        const uint32_t tm_d = tmem + p.tm_d, tm_d3 = tmem + p.tm_d3, tm_ph = tm_d3 + (uint32_t)KO - 16;
-        uint32_t ph = 0, slot = 0, wpar = 0, tcount = 0, slot_lo = (slots_addr >> 4) & 0x3FFFu;
-        auto bar_wait = [&](uint32_t id) {
-            mbar_wait_addr(bars_addr + id * 8, (ph >> id) & 1u);
-            ph ^= 1u << id;
-        };
-        auto slot_acquire = [&](uint32_t w) {
-            if (w & SUB_NEW) mbar_wait_addr(bars_addr + (BAR_WFULL + slot) * 8, wpar);
-        };
-        auto slot_release = [&](uint32_t w) {               // after the (elected) commit to WEMPTY[slot]
-            if (w & SUB_END) {
-                if (++slot == (uint32_t)p.nslots) { slot = 0; wpar ^= 1u; }
-                slot_lo = ((slots_addr + slot * p.slot_bytes) >> 4) & 0x3FFFu;
-            }
-        };
-        // input-layer chunk (SS): D[b] = A0 . Wc^T over the first nk K-steps (a prefix: masked columns are the high ones)
-        auto input_chunk = [&](uint32_t w, uint32_t a0_lo, uint32_t b) {
-            slot_acquire(w);
-            tc_fence_after();
-            const uint32_t nk = (w >> SUB_AUX_SHIFT) & 0xFFu;
-            uint32_t b_lo = slot_lo + (w & SUB_OFF_MASK);
-            if (elect_one()) {
-                uint32_t a_lo = a0_lo;
-#pragma unroll 1
-                for (uint32_t ks = 0; ks < nk; ++ks, a_lo += 16, b_lo += 16)
-                    mma_ss(tm_d + b * CH, hi_noswz | a_lo, hi_noswz | b_lo, id64, ks != 0);
-                if (w & SUB_END) mma_commit_addr(bars_addr + (BAR_WEMPTY + slot) * 8);
-                mma_commit_addr(bars_addr + (BAR_DFULL + b) * 8);
-            }
-            __syncwarp();
-            slot_release(w);
-        };
-        // consumer of the in-place fp16 chunk in D[b]: dst (+)= D[b] . B^T, 4 K-steps of 16
-        auto consume = [&](uint32_t b, uint32_t b_lo, uint32_t dst, uint32_t idesc, uint32_t end_bar, uint32_t rel_slot) {
-            if (elect_one()) {
-                const uint32_t a_t = tm_d + b * CH;
-#pragma unroll
-                for (uint32_t ks = 0; ks < 4; ++ks) mma_ts(dst, a_t + 8 * ks, hi_sw128 | (b_lo + 2 * ks), idesc, true);
-                if (rel_slot) mma_commit_addr(bars_addr + (BAR_WEMPTY + slot) * 8);
-                if (end_bar) mma_commit_addr(bars_addr + end_bar * 8);
-            }
-            __syncwarp();
-        };
-        auto consume_phase = [&](uint32_t c, uint32_t b) {                  // P2 tile c is resident
-            bar_wait(BAR_INPL + b);
-            if (c == 0) bar_wait(BAR_D3EMPTY);                               // first write into D3 of this tile
-            tc_fence_after();
-            consume(b, ((res_addr + c * 2048) >> 4) & 0x3FFFu, tm_ph, id16, 0, 0);
-        };
-        auto consume_w3 = [&](uint32_t w, uint32_t b, uint32_t end_bar) {   // streamed layer-3 tile
-            bar_wait(BAR_INPL + b);
-            slot_acquire(w);
-            tc_fence_after();
-            const uint32_t nlo = ((w >> SUB_AUX_SHIFT) & 0xFFu) * 16;       // output rows below n_lo receive exactly 0
-            consume(b, slot_lo + (w & SUB_OFF_MASK) + (nlo / 8) * 64, tm_d3 + nlo, idesc_f16(128, KO - (int)nlo), end_bar,
-                    w & SUB_END);
-            slot_release(w);
-        };
-        auto l2_chunk = [&](uint32_t c2, uint32_t b, uint32_t &si) {        // D[b] = A1 . W2[c2]^T over the listed k-blocks
-            const uint32_t nb = p.nblk[c2];
-#pragma unroll 1
-            for (uint32_t j = 0; j < nb; ++j) {
-                const uint32_t w = p.sub[si++];
-                slot_acquire(w);
+        // counts and the k-block lists come from the parameter table.  Barrier parities live in the bits of `ph`.
+        if (elect_one()) {
+            const uint32_t issue = 1u;
+            const uint32_t smem_base = smem_u32(smem);
+            const uint32_t bars_addr = smem_base + L.bars;
+            const uint32_t a0_lo0 = (smem_base + L.a0) >> 4, a0_step = L.a0_bytes >> 4;
+            const uint32_t slots_lo = (smem_base + L.slots) >> 4, slot_step = p.slot_bytes >> 4, res_lo = (smem_base + L.res) >> 4;
+            // descriptor words: lo = addr/16 | (lbo/16) << 16, hi = sbo/16 | version 1 << 14 | layout << 29
+            const uint32_t lo_noswz = (128u >> 4) << 16, hi_noswz = (((uint32_t)(KI / 8) * 128u) >> 4) | (1u << 14);
+            const uint32_t lo_sw128 = (16u >> 4) << 16, hi_sw128 = (1024u >> 4) | (1u << 14) | (2u << 29);
+            const uint32_t id64 = idesc_f16(128, 64), id16 = idesc_f16(128, 16), id0 = idesc_f16(128, 0);
+            const uint32_t NC = (uint32_t)p.NC, nslots = (uint32_t)p.nslots;
+            const uint32_t tm_d = tmem + p.tm_d, tm_d3 = tmem + p.tm_d3, tm_ph = tm_d3 + (uint32_t)KO - 16;
+            uint32_t ph = 0, slot = 0, wpar = 0, slot_lo = slots_lo, tcount = 0;
+#define BAR_ADDR(id) (bars_addr + (uint32_t)(id) * 8u)
+#define WAIT_BAR(id) do { mbar_spin(BAR_ADDR(id), (ph >> (id)) & 1u); ph ^= 1u << (id); } while (0)
+#define SLOT_ACQUIRE(w) do { if ((w) & SUB_NEW) mbar_spin(BAR_ADDR(BAR_WFULL + slot), wpar); } while (0)
+#define SLOT_RELEASE(w) do { if ((w) & SUB_END) { mma_commit_addr_if(issue, BAR_ADDR(BAR_WEMPTY + slot)); slot_lo += slot_step; \
+                             if (++slot == nslots) { slot = 0; wpar ^= 1u; slot_lo = slots_lo; } } } while (0)
+            // input-layer chunk (SS): D[b] = A0 . Wc^T over the first nk K-steps (a prefix: masked columns are the high ones)
+            auto input_chunk = [&](uint32_t w, uint32_t a0_lo, uint32_t b) {
+                SLOT_ACQUIRE(w);
                 tc_fence_after();
-                const uint32_t kb = (w >> SUB_AUX_SHIFT) & 0xFFu;
-                const uint32_t b_lo = slot_lo + (w & SUB_OFF_MASK);
-                if (elect_one()) {
-                    const uint32_t a_t = tmem + kb * (CH / 2);
+                const uint32_t nk = (w >> SUB_AUX_SHIFT) & 0xFFu, d = tm_d + b * CH;
+                uint32_t a_lo = a0_lo | lo_noswz, b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_noswz;
+                mma_ss2(issue, d, a_lo, hi_noswz, b_lo, hi_noswz, id64, 0u);
+#pragma unroll 1
+                for (uint32_t ks = 1; ks < nk; ++ks) { a_lo += 16; b_lo += 16; mma_ss2(issue, d, a_lo, hi_noswz, b_lo, hi_noswz, id64, 1u); }
+                SLOT_RELEASE(w);
+                mma_commit_addr_if(issue, BAR_ADDR(BAR_DFULL + b));
+            };
+            // consumer of the in-place fp16 chunk in D[b]: dst += D[b] . B^T, 4 K-steps of 16
+            auto consume = [&](uint32_t b, uint32_t b_lo, uint32_t dst, uint32_t idesc) {
+                const uint32_t a_t = tm_d + b * CH;
+                b_lo |= lo_sw128;
 #pragma unroll
-                    for (uint32_t ks = 0; ks < 4; ++ks)
-                        mma_ts(tm_d + b * CH, a_t + 8 * ks, hi_sw128 | (b_lo + 2 * ks), id64, (j | ks) != 0);
-                    if (w & SUB_END) mma_commit_addr(bars_addr + (BAR_WEMPTY + slot) * 8);
-                    if (j + 1 == nb) mma_commit_addr(bars_addr + (BAR_DFULL + b) * 8);
+                for (uint32_t ks = 0; ks < 4; ++ks) mma_ts2(issue, dst, a_t + 8 * ks, b_lo + 2 * ks, hi_sw128, idesc, 1u);
+            };
+            auto consume_phase = [&](uint32_t c, uint32_t b) {                  // P2 tile c is resident
+                WAIT_BAR(BAR_INPL + b);
+                if (c == 0) WAIT_BAR(BAR_D3EMPTY);                               // first write into D3 of this tile
+                tc_fence_after();
+                consume(b, res_lo + c * (2048u >> 4), tm_ph, id16);
+            };
+            auto consume_w3 = [&](uint32_t w, uint32_t b, bool last) {          // streamed layer-3 tile
+                WAIT_BAR(BAR_INPL + b);
+                SLOT_ACQUIRE(w);
+                tc_fence_after();
+                const uint32_t nlo = ((w >> SUB_AUX_SHIFT) & 0xFFu) * 16;       // output rows below n_lo receive exactly 0
+                consume(b, slot_lo + (w & SUB_OFF_MASK) + (nlo / 8) * 64, tm_d3 + nlo, id0 | ((((uint32_t)KO - nlo) >> 3) << 17));
+                SLOT_RELEASE(w);
+                if (last) mma_commit_addr_if(issue, BAR_ADDR(BAR_D3FULL));
+            };
+            auto l2_chunk = [&](uint32_t c2, uint32_t b, uint32_t &si) {        // D[b] = A1 . W2[c2]^T over the listed k-blocks
+                const uint32_t nb = p.nblk[c2], d = tm_d + b * CH;
+#pragma unroll 1
+                for (uint32_t j = 0; j < nb; ++j) {
+                    const uint32_t w = p.sub[si++];
+                    SLOT_ACQUIRE(w);
+                    tc_fence_after();
+                    const uint32_t a_t = tmem + ((w >> SUB_AUX_SHIFT) & 0xFFu) * (CH / 2);
+                    const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_sw128;
+                    mma_ts2(issue, d, a_t, b_lo, hi_sw128, id64, j);
+                    mma_ts2(issue, d, a_t + 8, b_lo + 2, hi_sw128, id64, 1u);
+                    mma_ts2(issue, d, a_t + 16, b_lo + 4, hi_sw128, id64, 1u);
+                    mma_ts2(issue, d, a_t + 24, b_lo + 6, hi_sw128, id64, 1u);
+                    SLOT_RELEASE(w);
                 }
-                __syncwarp();
-                slot_release(w);
+                mma_commit_addr_if(issue, BAR_ADDR(BAR_DFULL + b));
+            };
+            for (long long t = t_lo; t < t_hi; ++t, ++tcount) {
+                const uint32_t a0_lo = a0_lo0 + (tcount & 1u) * a0_step;
+                uint32_t si = 0;
+                // ---- stage A: layer 1, epilogue -> A1 (frees the accumulator) ----
+                WAIT_BAR(BAR_A0FULL + (tcount & 1u));
+                for (uint32_t c = 0; c < NC; c += 2) {
+                    if (c >= 2) WAIT_BAR(BAR_DFREE + 0);
+                    input_chunk(p.sub[si++], a0_lo, 0);
+                    if (c >= 2) WAIT_BAR(BAR_DFREE + 1);
+                    input_chunk(p.sub[si++], a0_lo, 1);
+                }
+                // ---- stage P: phase hidden layer, in place; its consumer runs one chunk behind ----
+                for (uint32_t c = 0; c < NC; c += 2) {
+                    if (c == 0) WAIT_BAR(BAR_DFREE + 0);      // last stage-A chunk of group 0 (=> all of its A1 is written)
+                    input_chunk(p.sub[si++], a0_lo, 0);
+                    if (c >= 2) consume_phase(c - 1, 1);
+                    if (c == 0) WAIT_BAR(BAR_DFREE + 1);
+                    input_chunk(p.sub[si++], a0_lo, 1);
+                    consume_phase(c, 0);
+                }
+                // ---- stage C: layer 2 from A1 (TS), in place; consumers (P2 of the last phase chunk, then W3) one behind ----
+                for (uint32_t c2 = 0; c2 < NC; c2 += 2) {
+                    l2_chunk(c2, 0, si);
+                    if (c2 == 0) consume_phase(NC - 1, 1);
+                    else consume_w3(p.sub[si++], 1, false);
+                    l2_chunk(c2 + 1, 1, si);
+                    consume_w3(p.sub[si++], 0, false);
+                }
+                consume_w3(p.sub[si++], 1, true);
             }
-        };
-        for (long long t = t_lo; t < t_hi; ++t, ++tcount) {
-            const uint32_t a0_lo = ((a0_addr + (tcount & 1u) * L.a0_bytes) >> 4) & 0x3FFFu;
-            uint32_t si = 0;
-            // ---- stage A: layer 1, epilogue -> A1 (frees the accumulator) ----
-            bar_wait(BAR_A0FULL + (tcount & 1u));
-            for (uint32_t c = 0; c < NC; c += 2) {
-                if (c >= 2) bar_wait(BAR_DFREE + 0);
-                input_chunk(p.sub[si++], a0_lo, 0);
-                if (c >= 2) bar_wait(BAR_DFREE + 1);
-                input_chunk(p.sub[si++], a0_lo, 1);
-            }
-            // ---- stage P: phase hidden layer, in place; its consumer runs one chunk behind ----
-            for (uint32_t c = 0; c < NC; c += 2) {
-                if (c == 0) bar_wait(BAR_DFREE + 0);          // last stage-A chunk of group 0 (=> all of its A1 is written)
-                input_chunk(p.sub[si++], a0_lo, 0);
-                if (c >= 2) consume_phase(c - 1, 1);
-                if (c == 0) bar_wait(BAR_DFREE + 1);
-                input_chunk(p.sub[si++], a0_lo, 1);
-                consume_phase(c, 0);
-            }
-            // ---- stage C: layer 2 from A1 (TS), in place; consumers (P2 of the last phase chunk, then W3) one behind ----
-            for (uint32_t c2 = 0; c2 < NC; c2 += 2) {
-                l2_chunk(c2, 0, si);
-                if (c2 == 0) consume_phase(NC - 1, 1);
-                else consume_w3(p.sub[si++], 1, 0);
-                l2_chunk(c2 + 1, 1, si);
-                consume_w3(p.sub[si++], 0, 0);
-            }
-            consume_w3(p.sub[si++], 1, BAR_D3FULL);
+#undef BAR_ADDR
+#undef WAIT_BAR
+#undef SLOT_ACQUIRE
+#undef SLOT_RELEASE
         }
+        __syncwarp();
     } else if (warp < 10) {
         // =========================== chunk epilogue groups: group g owns accumulator D[g] ===========================
         const int grp = (warp - 2) >> 2;
