@@ -72,7 +72,7 @@ struct TcParams {
     const uint8_t *wimg;                 // packed streamed weight tiles
     const uint2 *fills;                  // per-tile ring fills: (byte offset, bytes), consumption order
     int nfills;
-    uint32_t sub[MAX_SUB];               // per-tile streamed sub-tiles (see SUB_*)
+    uint32_t sub[MAX_SUB + 1];           // per-tile streamed sub-tiles (see SUB_*); one pad word (read-ahead)
     uint8_t nblk[MAX_NC];                // layer-2 k-blocks issued per output chunk
     const ChunkOp *chunks; int nchunks;  // per-tile accumulator chunks, in MMA order
     const uint8_t *resimg; uint32_t res_bytes;   // resident P2 tiles
@@ -175,19 +175,21 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_const
             const uint32_t tm_d = tmem + p.tm_d, tm_d3 = tmem + p.tm_d3, tm_ph = tm_d3 + (uint32_t)KO - 16;
             uint32_t ph = 0, slot = 0, wpar = 0, slot_lo = slots_lo, tcount = 0;
 #define BAR_ADDR(id) (bars_addr + (uint32_t)(id) * 8u)
-#define WAIT_BAR(id) do { mbar_spin(BAR_ADDR(id), (ph >> (id)) & 1u); ph ^= 1u << (id); } while (0)
-#define SLOT_ACQUIRE(w) do { if ((w) & SUB_NEW) mbar_spin(BAR_ADDR(BAR_WFULL + slot), wpar); } while (0)
+#define WAIT_BAR(id) do { mbar_spin(BAR_ADDR(id), (ph >> (id)) & 1u); ph ^= 1u << (id); tc_fence_after(); } while (0)
+#define SLOT_ACQUIRE(w) do { if ((w) & SUB_NEW) { mbar_spin(BAR_ADDR(BAR_WFULL + slot), wpar); tc_fence_after(); } } while (0)
 #define SLOT_RELEASE(w) do { if ((w) & SUB_END) { mma_commit_addr_if(issue, BAR_ADDR(BAR_WEMPTY + slot)); slot_lo += slot_step; \
                              if (++slot == nslots) { slot = 0; wpar ^= 1u; slot_lo = slots_lo; } } } while (0)
             // input-layer chunk (SS): D[b] = A0 . Wc^T over the first nk K-steps (a prefix: masked columns are the high ones)
             auto input_chunk = [&](uint32_t w, uint32_t a0_lo, uint32_t b) {
                 SLOT_ACQUIRE(w);
-                tc_fence_after();
                 const uint32_t nk = (w >> SUB_AUX_SHIFT) & 0xFFu, d = tm_d + b * CH;
-                uint32_t a_lo = a0_lo | lo_noswz, b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_noswz;
+                const uint32_t a_lo = a0_lo | lo_noswz, b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_noswz;
                 mma_ss2(issue, d, a_lo, hi_noswz, b_lo, hi_noswz, id64, 0u);
-#pragma unroll 1
-                for (uint32_t ks = 1; ks < nk; ++ks) { a_lo += 16; b_lo += 16; mma_ss2(issue, d, a_lo, hi_noswz, b_lo, hi_noswz, id64, 1u); }
+                // nested so that the common exit is ONE taken branch (KI <= 128 -> at most 8 K-steps)
+#define KSTEP(k) mma_ss2(issue, d, a_lo + 16u * (k), hi_noswz, b_lo + 16u * (k), hi_noswz, id64, 1u)
+                if (nk > 1) { KSTEP(1); if (nk > 2) { KSTEP(2); if (nk > 3) { KSTEP(3); if (nk > 4) { KSTEP(4);
+                if (nk > 5) { KSTEP(5); if (nk > 6) { KSTEP(6); if (nk > 7) { KSTEP(7); } } } } } } }
+#undef KSTEP
                 SLOT_RELEASE(w);
                 mma_commit_addr_if(issue, BAR_ADDR(BAR_DFULL + b));
             };
@@ -201,13 +203,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_const
             auto consume_phase = [&](uint32_t c, uint32_t b) {                  // P2 tile c is resident
                 WAIT_BAR(BAR_INPL + b);
                 if (c == 0) WAIT_BAR(BAR_D3EMPTY);                               // first write into D3 of this tile
-                tc_fence_after();
                 consume(b, res_lo + c * (2048u >> 4), tm_ph, id16);
             };
             auto consume_w3 = [&](uint32_t w, uint32_t b, bool last) {          // streamed layer-3 tile
                 WAIT_BAR(BAR_INPL + b);
                 SLOT_ACQUIRE(w);
-                tc_fence_after();
                 const uint32_t nlo = ((w >> SUB_AUX_SHIFT) & 0xFFu) * 16;       // output rows below n_lo receive exactly 0
                 consume(b, slot_lo + (w & SUB_OFF_MASK) + (nlo / 8) * 64, tm_d3 + nlo, id0 | ((((uint32_t)KO - nlo) >> 3) << 17));
                 SLOT_RELEASE(w);
@@ -215,11 +215,12 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_const
             };
             auto l2_chunk = [&](uint32_t c2, uint32_t b, uint32_t &si) {        // D[b] = A1 . W2[c2]^T over the listed k-blocks
                 const uint32_t nb = p.nblk[c2], d = tm_d + b * CH;
+                uint32_t w = p.sub[si];
 #pragma unroll 1
                 for (uint32_t j = 0; j < nb; ++j) {
-                    const uint32_t w = p.sub[si++];
+                    const uint32_t wn = p.sub[si + 1];                           // next word early: hides the constant-load latency
+                    ++si;
                     SLOT_ACQUIRE(w);
-                    tc_fence_after();
                     const uint32_t a_t = tmem + ((w >> SUB_AUX_SHIFT) & 0xFFu) * (CH / 2);
                     const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_sw128;
                     mma_ts2(issue, d, a_t, b_lo, hi_sw128, id64, j);
@@ -227,6 +228,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_const
                     mma_ts2(issue, d, a_t + 16, b_lo + 4, hi_sw128, id64, 1u);
                     mma_ts2(issue, d, a_t + 24, b_lo + 6, hi_sw128, id64, 1u);
                     SLOT_RELEASE(w);
+                    w = wn;
                 }
                 mma_commit_addr_if(issue, BAR_ADDR(BAR_DFULL + b));
             };
@@ -496,7 +498,7 @@ struct TcPack {
     void *d_fpos = nullptr; size_t fpos_cap = 0; const void *fpos_for = nullptr; long long fpos_G = -1;
     void *d_xpos = nullptr; size_t xpos_cap = 0;
     SmemLayout L{};
-    uint32_t sub[MAX_SUB] = {0};
+    uint32_t sub[MAX_SUB + 1] = {0};
     uint8_t nblk[MAX_NC] = {0};
     int sms = 148;
     long long mma_issued = 0, mma_dense = 0;                   // K-steps issued / K-steps of the dense chain, per tile
@@ -511,7 +513,8 @@ static bool tc_shape(const nqs_made *M, int *KI_, int *KO_, uint32_t *slot_, int
     uint32_t slot = (uint32_t)CH * KI * 2;                                  // input sub-tile (64 rows x KI)
     if ((uint32_t)CH * 128 > slot) slot = CH * 128;                          // layer-2 sub-tile (64 x 64)
     if ((uint32_t)KO * 128 > slot) slot = (uint32_t)KO * 128;                // layer-3 sub-tile (KO x 64)
-    slot = ((2 * slot) + 1023) & ~1023u;                                     // two sub-tiles per fill
+    slot = ((2 * slot) + 1023) & ~1023u;                                     // at least two sub-tiles per fill
+    if (slot < 32768u) slot = 32768u;                                        // few, large bulk copies (a thread sustains ~1 copy / 700 cycles)
     int ns = MAX_SLOTS;
     while (ns > 0 && smem_layout(KI, M->h, KO, NC, slot, ns).total > 227 * 1024 - 1024) --ns;
     if (ns < 3) return false;
