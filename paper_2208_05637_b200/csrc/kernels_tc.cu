@@ -141,23 +141,27 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_const
         // =========================== weight producers (TMA engine, 1-D bulk copies) ===========================
         // One thread sustains about one ring fill per ~700 cycles (measured: the rate does not depend on the fill
         // size), so NPROD lanes share the fills round-robin; fill q always lands in slot q % nslots.
-        if (lane < NPROD) {
+        // Never more lanes than slots: a lane that runs two uses of a slot ahead of the consumer would see the
+        // parity of an older phase and overwrite live data (parity waits alias after two phases).
+        const uint32_t nprod = (uint32_t)(p.nslots < NPROD ? p.nslots : NPROD);
+        if ((uint32_t)lane < nprod) {
             const long long total = (t_hi - t_lo) * (long long)p.nfills;
             uint32_t e = (uint32_t)lane % (uint32_t)p.nfills, slot = (uint32_t)lane % (uint32_t)p.nslots;
             uint32_t par = 1u ^ (((uint32_t)lane / (uint32_t)p.nslots) & 1u);   // a fresh barrier passes a parity-1 wait
-            for (long long q = lane; q < total; q += NPROD) {
+            for (long long q = lane; q < total; q += nprod) {
                 const uint2 pe = __ldg(&p.fills[e]);
                 mbar_wait(&bars[BAR_WEMPTY + slot], par);
                 mbar_arrive_expect_tx(&bars[BAR_WFULL + slot], pe.y);
                 bulk_g2s(smem + L.slots + slot * p.slot_bytes, p.wimg + pe.x, pe.y, &bars[BAR_WFULL + slot]);
-                e += NPROD; while (e >= (uint32_t)p.nfills) e -= (uint32_t)p.nfills;
-                slot += NPROD; while (slot >= (uint32_t)p.nslots) { slot -= (uint32_t)p.nslots; par ^= 1u; }
+                e += nprod; while (e >= (uint32_t)p.nfills) e -= (uint32_t)p.nfills;
+                slot += nprod; while (slot >= (uint32_t)p.nslots) { slot -= (uint32_t)p.nslots; par ^= 1u; }
             }
         }
     } else if (warp == 1) {
-        // =========================== MMA issuer: convergent warp, lane 0 issues (predicated) ===========================
-        // Every lane runs the same warp-uniform control flow so descriptors live in uniform registers; only the
-        // tcgen05.mma / tcgen05.commit instructions are predicated on `issue` (lane 0).
+        // =========================== MMA issuer: ONE elected thread ===========================
+        // Inside an elect.sync region ptxas knows a single thread is active and moves operands to uniform registers
+        // with plain R2UR; under `lane == 0` (or lane-predicated issue in a convergent warp) it emits a waterfall loop
+        // (ELECT / R2UR.BROADCAST / BRA.U.ANY, ~12 instructions) around every tcgen05.mma.
         // The per-tile schedule is fixed code (stage A: layer 1 -> A1; stage P: phase hidden, in place, P2 one chunk
         // behind; stage C: layer 2 from A1, in place, W3 one chunk behind); only the ring hand-over bits, the K-step
         // counts and the k-block lists come from the parameter table.  Barrier parities live in the bits of `ph`.
@@ -663,7 +667,13 @@ int tc_pack_upload(const nqs_made *M) {
     bool ok = up(&P->d_wimg, img.data(), img.size()) && up(&P->d_fills, fills.data(), fills.size() * sizeof(uint2)) &&
               up(&P->d_chunks, chunks.data(), chunks.size() * sizeof(ChunkOp)) &&
               up(&P->d_res, res.data(), res.size()) && up(&P->d_bias, bias.data(), bias.size() * 4);
-    ok = ok && cudaFuncSetAttribute(eloc_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->L.total) == cudaSuccess;
+    {   // the attribute belongs to the kernel, not to the model: keep the largest request
+        static int max_smem = 0;
+        if ((int)P->L.total > max_smem) {
+            ok = ok && cudaFuncSetAttribute(eloc_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->L.total) == cudaSuccess;
+            if (ok) max_smem = (int)P->L.total;
+        }
+    }
     if (!ok) {
         cudaGetLastError();
         cudaFree(P->d_wimg); cudaFree(P->d_fills); cudaFree(P->d_chunks); cudaFree(P->d_res); cudaFree(P->d_bias);
