@@ -73,6 +73,29 @@ def test_logpsi_parity(n, h, L, order):
     assert nqs.made_logpsi(M, torch.zeros((0, 2), dtype=torch.int64, device=DEV)).shape == (0, 2)   # B = 0
 
 
+@pytest.mark.parametrize("n,h", [(20, 128), (76, 128), (40, 256), (76, 512)])
+def test_logpsi_tensor_core_many_tiles_per_cta(n, h):
+    """Persistent-kernel paths that a few-tile launch never reaches: every CTA walks several 128-row tiles, so
+    the weight ring wraps, the double-buffered operand tile and every barrier parity are re-used (a producer
+    lane running ahead of the ring aliased a barrier parity exactly here).  Sampled rows against the oracle."""
+    p = wl.make_made_params(n, h, 300 + n)
+    M = nqs.made_create(p)
+    try:
+        assert M.resolved_path(nqs.PATH_TC) == nqs.PATH_TC
+    except nqs.NqsError as e:
+        assert e.status == -6
+        pytest.skip("shape not supported by the tensor-core path")
+    B = 128 * 148 * 3 + 77                                       # 3+ tiles per CTA and a ragged tail
+    rng = np.random.default_rng(n + h)
+    cfgs = wl.pack_bits(rng.integers(0, 2, size=(B, n)).astype(np.uint8))
+    out = nqs.made_logpsi(M, _dev_u64(cfgs), path=nqs.PATH_TC).cpu().numpy().astype(np.float64)
+    idx = np.concatenate([np.arange(40), rng.choice(B, size=200, replace=False), np.arange(B - 40, B)])
+    ref = omade.logpsi(p, cfgs[idx])
+    assert np.isfinite(out).all()
+    assert np.abs(out[idx, 0] - ref.real).max() < 2e-2
+    assert np.abs(out[idx, 1] - ref.imag).max() < 2e-2
+
+
 @pytest.mark.parametrize("cfg,B", [(1, 256), (2, 300), (3, 130)])
 def test_contraction_parity(cfg, B):
     w, (x, z, c), params, H, M = workload(cfg)
