@@ -183,8 +183,10 @@ def main():
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)      # > 126 MB L2
     stream = torch.cuda.current_stream()
 
+    from paper_2208_05637_b200.distributed import minibatch_of_step, max_over_ranks
+
     def step(k):
-        b = (k * world + rank) % n_mb
+        b = minibatch_of_step(k, rank, world, n_mb)
         return nqs.local_energy(H, M, xs_all[b * mb:(b + 1) * mb], cnt_all[b * mb:(b + 1) * mb], minibatch=mb,
                                 path=path, want_stats=True, stream=stream, out=out)
 
@@ -213,10 +215,7 @@ def main():
     launches = nqs.kernel_launch_count() - launches0
     clocks = sampler.stop()
     total_ms = sum(a.elapsed_time(b) for a, b in ev)
-    if world > 1:
-        t = torch.tensor([total_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(total_ms, dev)
     ms_per_step = total_ms / args.steps
     K, G = H.K, H.G
     pairs_per_step = mb * K * world
@@ -231,15 +230,12 @@ def main():
     barrier()
     t0 = time.perf_counter()
     for k in range(e2e_steps):
-        b = (k * world + rank) % n_mb
+        b = minibatch_of_step(k, rank, world, n_mb)
         nqs.local_energy_host(H, M, hs[b * mb:(b + 1) * mb].numpy().view(np.uint64), hc[b * mb:(b + 1) * mb].numpy(),
                               minibatch=mb, path=path, want_stats=True, out=ho.numpy())
     torch.cuda.synchronize()
     e2e_ms = 1e3 * (time.perf_counter() - t0) / e2e_steps
-    if world > 1:
-        t = torch.tensor([e2e_ms], dtype=torch.float64, device=dev)
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        e2e_ms = float(t.item())
+    e2e_ms = max_over_ranks(e2e_ms, dev)
     e2e_val = pairs_per_step / (e2e_ms / 1e3)
 
     if rank != 0:
