@@ -39,9 +39,9 @@ enum { BAR_A0FULL = 0, BAR_DFULL = 2, BAR_DFREE = 4, BAR_INPL = 6, BAR_D3FULL = 
 // Streamed weight sub-tiles are described by one 32-bit word each, in consumption order (kernel parameter
 // space -> uniform loads): offset inside the ring slot, ring hand-over flags and one small per-tile number.
 constexpr int MAX_SUB = 4 * MAX_NC + MAX_NC * MAX_NC;        // W1 + P1 + W2 blocks + W3
-constexpr uint32_t SUB_OFF_MASK = 0xFFFu;                    // [0:12)  byte offset inside the slot / 16 (slots <= 64 KB)
-constexpr uint32_t SUB_NEW = 1u << 12;                       // first sub-tile of a ring fill: wait for the fill
-constexpr uint32_t SUB_END = 1u << 13;                       // last sub-tile of a ring fill: release the slot
+constexpr uint32_t SUB_OFF_MASK = 0x1FFFu;                   // [0:13)  byte offset inside the slot / 16 (slots <= 128 KB)
+constexpr uint32_t SUB_NEW = 1u << 13;                       // first sub-tile of a ring fill: wait for the fill
+constexpr uint32_t SUB_END = 1u << 14;                       // last sub-tile of a ring fill: release the slot
 constexpr int SUB_AUX_SHIFT = 16;                            // [16:24) input chunks: K-steps to issue; W2: k-block; W3: n_lo / 16
 
 struct ChunkOp { uint16_t bias_off; uint16_t dst_col; uint32_t kind; };   // kind 0: -> A1 at dst_col; 1: in place
@@ -518,10 +518,10 @@ static bool tc_shape(const nqs_made *M, int *KI_, int *KO_, uint32_t *slot_, int
     if ((uint32_t)CH * 128 > slot) slot = CH * 128;                          // layer-2 sub-tile (64 x 64)
     if ((uint32_t)KO * 128 > slot) slot = (uint32_t)KO * 128;                // layer-3 sub-tile (KO x 64)
     slot = ((2 * slot) + 1023) & ~1023u;                                     // at least two sub-tiles per fill
-    if (slot < 40960u) slot = 40960u;                                        // few, large bulk copies (a thread sustains ~1 copy / 700 cycles)
+    if (slot < 81920u) slot = 81920u;                                        // few, large bulk copies (a thread sustains ~1 copy / 700 cycles)
     int ns = MAX_SLOTS;
     while (ns > 0 && smem_layout(KI, M->h, KO, NC, slot, ns).total > 227 * 1024 - 1024) --ns;
-    if (ns < 3) return false;
+    if (ns < 2) return false;
     *KI_ = KI; *KO_ = KO; *slot_ = slot; *nslots_ = ns;
     return true;
 }
