@@ -9,11 +9,13 @@
 //        all-zero 64x16 blocks of the masked weights are never issued (exact: they contribute 0),
 //   (a3) the Pauli contraction S[i,g] over the group's terms (popcount parity, (-i)^r folded into c),
 //   (a5) ratio = exp(dlog|psi|) cis(dphi), E_i += S * ratio, kept in registers per sample.
-// Warp roles (14 warps): 0 = weight producer (TMA 1-D bulk copies into a ring of smem slots), 1 = MMA issuer
-// (table-driven: walks a host-built program of MMA groups), 2-5 / 6-9 = two chunk-epilogue groups (one per
-// accumulator), 10-13 = tile warps (build A0 of the NEXT tile, then the final epilogue of the current one).
-// The weight tiles are pre-packed on the host into the exact shared-memory images (128B-swizzled / core-matrix
-// K-major) in consumption order.
+// Warp roles (14 warps): 0 = weight producers (a few lanes issue TMA 1-D bulk copies into a ring of large smem slots;
+// never more lanes than slots), 1 = MMA issuer (ONE elect.sync thread runs the fixed per-tile schedule; ring hand-over
+// bits, K-step counts and k-block lists come from a host-built table in kernel-parameter space), 2-5 / 6-9 = two
+// chunk-epilogue groups (one per accumulator), 10-13 = tile warps (build A0 of the NEXT tile, contraction, then the final
+// epilogue of the current one).  The weight tiles are pre-packed on the host into the exact shared-memory images
+// (128B-swizzled / core-matrix K-major) in consumption order.  What was measured and why the design is what it is:
+// DESIGN.md sections 6-7.
 // PAPER.md:122-134 (Alg. 1), :84-96 (architecture, Eq. 8-10), :152-158 (Eq. 15-16).
 #include <cstring>
 #include <new>
