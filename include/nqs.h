@@ -129,7 +129,8 @@ int nqs_made_logpsi(const nqs_made_t *made, const uint64_t *configs_dev, int64_t
 
 /* ---- (a3) Pauli contraction alone: Eq. 16 summed inside each unique-flip group --------
  * S[i][g - g0] = sum_{t in group g} c_t (-i)^{r_t} (-1)^{popcount(x_i & s_t)},  g in [g0, g1).
- * samples_dev : device uint64 [B][2];  S_out_dev : device float [B][g1-g0][2] (Re, Im).
+ * samples_dev : device uint64 [B][2];  S_out_dev : device float [g1-g0][B][2] (Re, Im), group-major: the B sums of
+ * one group are contiguous.
  * Provided for tests and for the contraction-only throughput figure; nqs_local_energy fuses this step
  * and never materialises S. */
 int nqs_pauli_contract(const nqs_ham_t *ham, const uint64_t *samples_dev, int64_t B, int64_t g0,

@@ -501,7 +501,7 @@ struct TcPack {
     int KI = 0, KO = 0, NC = 0, nsub = 0, nchunks = 0, nfills = 0, nslots = 0;
     uint32_t slot_bytes = 0, res_bytes = 0, tm_d = 0, tm_d3 = 0;
     void *d_wimg = nullptr, *d_fills = nullptr, *d_chunks = nullptr, *d_res = nullptr, *d_bias = nullptr;
-    void *d_fpos = nullptr; size_t fpos_cap = 0; const void *fpos_for = nullptr; long long fpos_G = -1;
+    void *d_fpos = nullptr; size_t fpos_cap = 0;
     void *d_xpos = nullptr; size_t xpos_cap = 0;
     SmemLayout L{};
     uint32_t sub[MAX_SUB + 1] = {0};
@@ -753,12 +753,11 @@ int launch_eloc_tc(const HamDev &hm, const nqs_made *M, const ulonglong2 *x, con
     TcPack *P = M->tc;
     if (!P) return NQS_EUNSUPPORTED;
     int rc;
-    // position-ordered flips, cached per Hamiltonian
-    if (P->fpos_for != (const void *)hm.flips || P->fpos_G != hm.G) {
-        if ((rc = ensure(&P->d_fpos, &P->fpos_cap, sizeof(ulonglong2) * (size_t)(hm.G ? hm.G : 1)))) return rc;
-        if (hm.G > 0 && (rc = permuted(M, hm.flips, hm.G, (ulonglong2 *)P->d_fpos, st))) return rc;
-        P->fpos_for = (const void *)hm.flips; P->fpos_G = hm.G;
-    }
+    // position-ordered flips: rebuilt on the caller's stream for every launch (19 MB of traffic at cfg 5, microseconds
+    // next to the chain kernel).  No cache: a device address is not an identity (a freed Hamiltonian's buffers are
+    // handed to the next one of the same size), and a cache filled on one stream is unordered against another.
+    if ((rc = ensure(&P->d_fpos, &P->fpos_cap, sizeof(ulonglong2) * (size_t)(hm.G ? hm.G : 1)))) return rc;
+    if (hm.G > 0 && (rc = permuted(M, hm.flips, hm.G, (ulonglong2 *)P->d_fpos, st))) return rc;
     if ((rc = ensure(&P->d_xpos, &P->xpos_cap, sizeof(ulonglong2) * (size_t)B))) return rc;
     if ((rc = permuted(M, x, B, (ulonglong2 *)P->d_xpos, st))) return rc;
     diag_init_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(hm, x, B, eloc);

@@ -91,6 +91,16 @@ def test_against_torch_dense_mlp():
     logpi = (z * torch.log(prob) + (1 - z) * torch.log(1 - prob)).sum(dim=1)
     lp = omade.logpsi(p, pack_mask(bits))
     np.testing.assert_allclose(lp.real, 0.5 * logpi.numpy(), atol=1e-12)
+    # phase net (reading A11) through the same independent library: dense n-2 -> h -> 4 on the
+    # first n-2 POSITIONS, output picked by torch.gather with the last two positions' bits
+    u = 2 * z[:, : n - 2] - 1
+    hid = torch.relu(torch.nn.functional.linear(u, torch.tensor(p.phase_weights[0].astype(np.float64)),
+                                                torch.tensor(p.phase_biases[0].astype(np.float64))))
+    o = torch.nn.functional.linear(hid, torch.tensor(p.phase_weights[1].astype(np.float64)),
+                                   torch.tensor(p.phase_biases[1].astype(np.float64)))
+    sel = (2 * z[:, n - 2] + z[:, n - 1]).long()
+    phi = torch.gather(o, 1, sel[:, None])[:, 0]
+    np.testing.assert_allclose(lp.imag, phi.numpy(), atol=1e-12)
 
 
 def test_log_sigmoid_vs_long_double_and_symmetry():
@@ -117,3 +127,37 @@ def test_phase_selector_and_input_independence():
     np.testing.assert_allclose(phis, o, atol=1e-14)
     lp = omade.logpsi(p, pack_mask(z))
     np.testing.assert_allclose(lp.imag, o, atol=1e-14)
+
+
+def test_phase_reads_positions_not_qubits():
+    """The phase net's n-2 inputs and its 2-bit selector are taken in autoregressive POSITION order
+    (z_d = x[order[d]], reading A10/A11), not in qubit order: with a non-trivial order (i) flipping the QUBITS
+    order[n-2], order[n-1] moves phi only among the four outputs of the same hidden state, while flipping
+    qubits n-2, n-1 (which sit at other positions) changes the hidden state; (ii) phi equals a hand evaluation
+    that gathers inputs through `order`, and differs from the one that ignores `order`."""
+    n, h = 9, 16
+    p = _params(n, h, 2, 21, "reverse")                      # position d reads qubit n-1-d
+    rng = np.random.default_rng(4)
+    bits = rng.integers(0, 2, size=(16, n)).astype(np.uint8)  # by qubit
+    P1, P2 = p.phase_weights[0].astype(np.float64), p.phase_weights[1].astype(np.float64)
+    c1, c2 = p.phase_biases[0].astype(np.float64), p.phase_biases[1].astype(np.float64)
+
+    def by_hand(zrow):                                        # zrow: bits already in the order the net reads them
+        hid = np.maximum(P1 @ (2.0 * zrow[: n - 2] - 1.0) + c1, 0.0)
+        return (P2 @ hid + c2)[2 * int(zrow[n - 2]) + int(zrow[n - 1])]
+
+    lp = omade.logpsi(p, pack_mask(bits))
+    pos = np.array([by_hand(bits[b][p.order].astype(np.float64)) for b in range(16)])
+    qub = np.array([by_hand(bits[b].astype(np.float64)) for b in range(16)])
+    np.testing.assert_allclose(lp.imag, pos, atol=1e-13)
+    assert np.abs(lp.imag - qub).max() > 1e-3
+    # (i) selector qubits are order[n-2], order[n-1] = qubits 1, 0 under the reverse order
+    q_hi, q_lo = int(p.order[n - 2]), int(p.order[n - 1])
+    assert (q_hi, q_lo) == (1, 0)
+    b0 = bits[:1].copy()
+    outs = []
+    for k in range(4):
+        b = b0.copy(); b[0, q_hi], b[0, q_lo] = k >> 1, k & 1
+        outs.append(omade.logpsi(p, pack_mask(b)).imag[0])
+    hid = np.maximum(P1 @ (2.0 * b0[0][p.order][: n - 2] - 1.0) + c1, 0.0)
+    np.testing.assert_allclose(outs, P2 @ hid + c2, atol=1e-13)
