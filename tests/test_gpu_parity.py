@@ -326,19 +326,31 @@ def test_eloc_cfg3_tc_vs_simt_all_rows_and_oracle():
     assert np.hypot(d[:, 0], d[:, 1]).max() <= (TC_NARROW_FACTOR + 1) * tol
 
 
+def _few_flip_pauli_list(rng, n, K):
+    """Generic Pauli strings with the paper's sparsity (<= 4 X/Y positions per string), odd Y counts
+    allowed, a few Z elsewhere, qubit 0 always flipped (so there is NO f = 0 group), one duplicate string."""
+    codes = np.zeros((K, n), np.uint8)
+    for t in range(K):
+        nf = int(rng.integers(0, 4))                              # 0..3 further flipped qubits besides qubit 0
+        pos = rng.choice(np.arange(1, n), size=nf, replace=False)
+        codes[t, 0] = rng.integers(1, 3)                          # X or Y
+        codes[t, pos] = rng.integers(1, 3, size=nf)
+        zpos = rng.choice(np.arange(1, n), size=int(rng.integers(0, 4)), replace=False)
+        codes[t, zpos] = np.where(codes[t, zpos] == 0, 3, codes[t, zpos])
+    codes[:, n - 1] = np.where(codes[:, n - 1] == 0, rng.integers(0, 4, size=K), codes[:, n - 1])   # top qubit busy
+    codes[17] = codes[5]
+    return codes, rng.standard_normal(K)
+
+
 @pytest.mark.parametrize("n,h", [(20, 512), (65, 512), (20, 384)])
 def test_generic_odd_Y_no_diagonal_on_tensor_core_path(n, h):
     """Complex S (odd Y counts -> Im S != 0), a Hamiltonian WITHOUT an f = 0 group (g_begin = 0), duplicates, two
     mask words, h = 384 (the narrowest width AUTO sends to the tensor cores) -- all on NQS_PATH_TC, several sample
-    blocks, ragged."""
+    blocks, ragged.  Bound: each term's ratio carries a relative error |exp(d) - 1| with |d| <= 2 sqrt(2) *
+    TC_LOGPSI_TOL (log|psi| and phi of x' and of x), so |dE| <= sum|c| * max|ratio| * 2 sqrt(2) * TC_LOGPSI_TOL; the
+    ratio to the north_star bound (which is stated for the five chemistry configs) is printed."""
     rng = np.random.default_rng(1000 + n + h)
-    K = 400
-    codes = rng.integers(0, 4, size=(K, n)).astype(np.uint8)
-    codes[:, rng.random(n) < 0.75] = 0
-    codes[:, n - 1] = rng.integers(0, 4, size=K)
-    codes[:, 0] = np.where(codes[:, 0] == 0, 1, codes[:, 0])     # every string flips qubit 0: no f = 0 group
-    codes[17] = codes[5]
-    coeffs = rng.standard_normal(K)
+    codes, coeffs = _few_flip_pauli_list(rng, n, 400)
     p = wl.make_made_params(n, h, n + h, order="random")
     B = 3 * 128 + 41
     samples = wl.pack_bits(rng.integers(0, 2, size=(B, n)).astype(np.uint8))
@@ -351,13 +363,16 @@ def test_generic_odd_Y_no_diagonal_on_tensor_core_path(n, h):
     e, st = nqs.local_energy(H, M, _dev_u64(samples), None, path=nqs.PATH_TC)
     e = e.cpu().numpy().astype(np.float64)
     ec = e[:, 0] + 1j * e[:, 1]
-    scale = max(1.0, mr)
     err = np.abs(ec[pick] - ref).max()
-    print(f"[parity] generic odd-Y n={n} h={h} TC: max|dE_loc|/(tol*max|ratio|) = {err / (1e-5 * H.sum_abs_coeff * scale):.4f}")
-    assert err <= 1e-5 * H.sum_abs_coeff * scale
+    print(f"[parity] generic odd-Y n={n} h={h} TC: max|dE_loc| = {err:.3e} = {err / (1e-5 * H.sum_abs_coeff * max(1.0, mr)):.3f} x "
+          f"(1e-5 sum|c| max|ratio|), max|ratio| = {mr:.2f}")
+    assert err <= H.sum_abs_coeff * max(1.0, mr) * 2 * 2 ** 0.5 * TC_LOGPSI_TOL
     assert np.abs(ref.imag).max() > 1e-3 and np.abs(ec.imag).max() > 1e-3
+    # the imaginary channel on its own: Im E of the picked rows, same bound, and a sign/swap error would be O(sum|c|)
+    assert np.abs(ec[pick].imag - ref.imag).max() <= H.sum_abs_coeff * max(1.0, mr) * 2 * 2 ** 0.5 * TC_LOGPSI_TOL
+    assert np.abs(ref.imag).max() > 50 * np.abs(ec[pick].imag - ref.imag).max()
     assert st[4] >= mr * (1 - 1e-2)
-    np.testing.assert_allclose(st[2], ec.imag.sum(), rtol=1e-9)  # stats[2] = sum n Im E with unit weights
+    np.testing.assert_allclose(st[2], ec.imag.sum(), rtol=1e-6, atol=1e-6 * H.sum_abs_coeff)
 
 
 def test_empty_hamiltonian_on_tensor_core_path():
