@@ -1,0 +1,877 @@
+// Tensor-core path (NQS_PATH_TC): ONE persistent, warp-specialised sm_100a kernel run by CTA PAIRS (clusters of two
+// CTAs on one TPC, tcgen05 cta_group::2).  A pair works on two tiles at a time — CTA r on tile 2q + r, a tile being
+// 128 samples x 1 unique-flip group g — and every MMA covers both: M = 256 rows (128 per CTA), the weight operand B
+// split by rows between the two CTAs' shared memories, so each SM streams only HALF of the weight image.  Per tile:
+//   (a2) x' = x xor f_g expanded to a +-1 fp16 operand tile A0, written straight into TENSOR MEMORY (A operand of the
+//        input-layer MMAs; no shared-memory copy of the inputs exists),
+//   (a4) the MADE chain and the phase MLP as tcgen05 MMAs (fp16 operands, fp32 accumulation in TMEM), in 128-unit
+//        hidden CHUNKS that rotate through up to three 128-column TMEM accumulators:
+//          layer 1   D = A0 . W1c^T   TS  -> epilogue: +b1, ReLU, fp16 -> A1 in SHARED memory (128B-swizzled K-major)
+//          phase     D = A0 . P1c^T   TS  -> epilogue: +c1, ReLU, fp16 IN PLACE -> D3 += D . P2c^T   (TS, N = 16)
+//          layer 2   D = A1 . W2c^T   SS  -> epilogue: +b2, ReLU, fp16 IN PLACE -> D3 += D . W3c^T   (TS)
+//        (one hidden layer: layer 1 is rewritten in place and feeds W3 directly).  All-zero K-steps of the masked
+//        weights are never issued (exact: they contribute 0),
+//   (a3) the Pauli contraction S[i,g] over the group's terms (popcount parity, (-i)^r folded into c),
+//   (a5) ratio = exp(dlog|psi|) cis(dphi), E_i += S * ratio, kept in registers per sample.
+// Warp roles (14 warps per CTA): 0 = weight producers (TMA 1-D bulk copies of this CTA's half of the weight image into
+// a ring of large slots); 1 = in the leader CTA the MMA issuer (ONE elect.sync thread issues every tcgen05.mma /
+// commit of the pair; commits are multicast to the barriers of both CTAs), in the peer CTA a forwarder that tells the
+// leader when the peer's half of a ring slot has landed; 2-5 / 6-9 = two chunk-epilogue groups (ops alternate);
+// 10-13 = tile warps (A0 of the NEXT tile, contraction, final epilogue).  DESIGN.md sections 6-7.
+// PAPER.md:122-134 (Alg. 1), :84-96 (architecture, Eq. 8-10), :152-158 (Eq. 15-16).
+#include <cstring>
+#include <new>
+#include <vector>
+#include "nqs_internal.h"
+#include "tc_ptx.cuh"
+
+using namespace tc;
+
+namespace {
+
+constexpr int TILE_M = 128;
+constexpr int CN = 128;                  // hidden-unit chunk = accumulator columns = MMA N of the pair
+constexpr int HALF = CN / 2;             // weight rows per CTA and chunk
+constexpr int NTHREADS = 448;
+constexpr int MAX_NC = 4;                // hidden <= 512
+constexpr int MAX_SLOTS = 8;
+constexpr int NPROD = 4;                 // producer lanes (bulk-copy issuers), never more than slots
+constexpr int MAX_OPS = 3 * MAX_NC;
+
+enum : uint8_t { T_L1S = 0, T_L1I = 1, T_P = 2, T_L2 = 3 };   // layer 1 -> smem A1 | layer 1 in place | phase hidden | layer 2
+
+// barrier ids.  Waited by the leader's issuer (arrivals from both CTAs): A0FULL, D3EMPTY, EDONE[], WFULL[] (leader copy).
+// Committed by the issuer into BOTH CTAs: A0FREE, A1FREE, D3FULL, FULL[], WEMPTY[].
+enum { BAR_A0FULL = 0, BAR_A0FREE = 1, BAR_A1FREE = 2, BAR_D3FULL = 3, BAR_D3EMPTY = 4, BAR_FULL = 5, BAR_EDONE = 8,
+       BAR_WFULL = 11, BAR_WEMPTY = 11 + MAX_SLOTS, BAR_COUNT = 11 + 2 * MAX_SLOTS };
+
+// Streamed weight sub-tiles: one 32-bit word each, in consumption order (kernel parameter space -> uniform loads).
+constexpr int MAX_SUB = 2 * MAX_NC + MAX_NC * 2 * MAX_NC + MAX_NC;   // W1 + P1 + W2 blocks + W3
+constexpr uint32_t SUB_OFF_MASK = 0x1FFFu;                   // [0:13)  byte offset inside the slot / 16
+constexpr uint32_t SUB_NEW = 1u << 13;                       // first sub-tile of a ring fill: wait for the fill
+constexpr uint32_t SUB_END = 1u << 14;                       // last sub-tile of a ring fill: release the slot
+constexpr int SUB_AUX_SHIFT = 16;                            // [16:24) input: K-steps; W2: k-block | K-step mask << 4; W3: n_lo / 16
+
+struct SmemLayout { uint32_t a1, res, bias, bars, slots, total; };
+
+__host__ __device__ inline SmemLayout smem_layout(int H, int KO, int L, uint32_t slot_bytes, int nslots) {
+    SmemLayout S;
+    uint32_t off = 0;
+    S.a1 = off; if (L == 2) off += (uint32_t)(H / 64) * 16384u;      // fp16 layer-1 activations, [H/64] K-blocks of 128 rows x 128 B
+    S.res = off; off += (uint32_t)(H / 64) * 1024u;                  // resident P2 tiles: 8 rows x 64 K per K-block (this CTA's half)
+    S.bias = off; off += (uint32_t)(3 * H + KO + 4) * 4;
+    off = (off + 15) & ~15u;
+    S.bars = off; off += BAR_COUNT * 8;
+    off = (off + 1023) & ~1023u;
+    S.slots = off; off += slot_bytes * (uint32_t)nslots;
+    S.total = off;
+    return S;
+}
+
+struct Tc2Params {
+    int n, H, NC, KI, KO, L, nacc, nops;
+    int last_a0_op, last_l2_op;
+    uint32_t tm_d3, tm_a0;               // TMEM columns: accumulator a at a * CN, D3 at tm_d3, A0 at tm_a0
+    const uint8_t *wimg; uint32_t img_stride;     // streamed weight image of cluster rank r at wimg + r * img_stride
+    const uint2 *fills; int nfills;      // per-tile ring fills (byte offset, bytes), consumption order, same for both ranks
+    uint32_t sub[MAX_SUB + 1];
+    uint8_t nblk[MAX_NC];                // layer-2 k-blocks issued per output chunk
+    uint8_t l2need[MAX_NC];              // layer-2 chunk c needs A1 chunks 0 .. l2need[c]
+    uint8_t optype[MAX_OPS], opchunk[MAX_OPS];
+    const uint8_t *resimg; uint32_t res_bytes;    // resident P2 tiles of rank r at resimg + r * res_bytes
+    uint32_t slot_bytes; int nslots;
+    const float *bias;                   // [c1 H | b1 H | b2 H | b3 KO | c2 4] fp32
+    int mode;                            // 0 = logpsi, 1 = local energy
+    const ulonglong2 *xpos;              // [B] configurations, bits in autoregressive POSITION order
+    long long B;
+    float2 *out;                         // mode 0: (log|psi|, phi) per row
+    const ulonglong2 *fpos;              // [G] flips in position order
+    const ulonglong2 *x;                 // [B] samples in qubit order (contraction parity)
+    HamDev hm;
+    const float2 *base;                  // [B] (log|psi|, phi) of the samples
+    float *eloc;                         // [B][2], pre-initialised with the f = 0 group; atomically accumulated
+    unsigned *max_ratio_bits;
+    long long g_begin;                   // first group that needs a forward pass (1 if group 0 is f = 0)
+};
+
+__device__ __forceinline__ unsigned long long shr128(ulonglong2 a, int s) {      // low 64 bits of a >> s, 0 <= s < 128
+    if (s == 0) return a.x;
+    if (s < 64) return (a.x >> s) | (a.y << (64 - s));
+    return a.y >> (s - 64);
+}
+
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc2_kernel(const __grid_constant__ Tc2Params p) {
+    extern __shared__ __align__(1024) uint8_t smem[];
+    __shared__ uint32_t s_tmem_base;
+    const SmemLayout SL = smem_layout(p.H, p.KO, p.L, p.slot_bytes, p.nslots);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + SL.bars);
+    float *s_bias = reinterpret_cast<float *>(smem + SL.bias);
+    const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
+    const int KI = p.KI, KO = p.KO, H = p.H;
+    const uint32_t nacc = (uint32_t)p.nacc, nops = (uint32_t)p.nops;
+    const uint32_t smem_base = smem_u32(smem);
+    const uint32_t bars_addr = smem_base + SL.bars;
+#define BAR_ADDR(id) (bars_addr + (uint32_t)(id) * 8u)
+
+    // ---- one-time setup ----
+    if (threadIdx.x == 0) {
+        mbar_init(&bars[BAR_A0FULL], 8); mbar_init(&bars[BAR_A0FREE], 1); mbar_init(&bars[BAR_A1FREE], 1);
+        mbar_init(&bars[BAR_D3FULL], 1); mbar_init(&bars[BAR_D3EMPTY], 8);
+        for (int a = 0; a < 3; ++a) { mbar_init(&bars[BAR_FULL + a], 1); mbar_init(&bars[BAR_EDONE + a], 8); }
+        for (int s = 0; s < p.nslots; ++s) {
+            mbar_init(&bars[BAR_WFULL + s], rank == 0 ? 2 : 1);      // leader: own producer + the peer's forwarder
+            mbar_init(&bars[BAR_WEMPTY + s], 1);
+        }
+        fence_mbar_init();
+    }
+    if (warp == 1) tmem_alloc_cg2(&s_tmem_base, 512);
+    for (int i = threadIdx.x; i < 3 * H + KO + 4; i += NTHREADS) s_bias[i] = p.bias[i];
+    for (int i = threadIdx.x; i < (int)(p.res_bytes / 16); i += NTHREADS)
+        reinterpret_cast<uint4 *>(smem + SL.res)[i] = reinterpret_cast<const uint4 *>(p.resimg + (size_t)rank * p.res_bytes)[i];
+    fence_proxy_async();                                  // resident tiles are read by the tensor core (async proxy)
+    tc_fence_before();
+    cluster_sync_all();
+    tc_fence_after();
+    const uint32_t tmem = s_tmem_base;
+
+    // ---- static schedule: a contiguous range of tile PAIRS per cluster, sample-block major; CTA r takes tile 2q + r ----
+    const long long nsb = (p.B + TILE_M - 1) / TILE_M;
+    const long long Gnd = (p.mode == 1) ? (p.hm.G - p.g_begin) : 1;
+    const long long ntiles = nsb * Gnd;
+    const long long npairs = (ntiles + 1) / 2;
+    const long long ncl = gridDim.x >> 1, cl = blockIdx.x >> 1;
+    const long long q_lo = npairs * cl / ncl, q_hi = npairs * (cl + 1) / ncl;
+    const long long ntl = q_hi - q_lo;
+
+    if (warp == 0) {
+        // =========================== weight producers (TMA engine, 1-D bulk copies), both CTAs ===========================
+        // Fill q always lands in slot q % nslots.  Never more lanes than slots: a lane two uses of a slot ahead of the
+        // consumer would pass its parity wait on an older phase and overwrite live data.
+        const uint32_t nprod = (uint32_t)(p.nslots < NPROD ? p.nslots : NPROD);
+        if ((uint32_t)lane < nprod) {
+            const long long total = ntl * (long long)p.nfills;
+            const uint8_t *img = p.wimg + (size_t)rank * p.img_stride;
+            uint32_t e = (uint32_t)lane % (uint32_t)p.nfills, slot = (uint32_t)lane, par = 1u;   // a fresh barrier passes a parity-1 wait
+            for (long long q = lane; q < total; q += nprod) {
+                const uint2 pe = __ldg(&p.fills[e]);
+                mbar_wait(&bars[BAR_WEMPTY + slot], par);
+                mbar_arrive_expect_tx(&bars[BAR_WFULL + slot], pe.y);
+                bulk_g2s(smem + SL.slots + slot * p.slot_bytes, img + pe.x, pe.y, &bars[BAR_WFULL + slot]);
+                e += nprod; while (e >= (uint32_t)p.nfills) e -= (uint32_t)p.nfills;
+                slot += nprod; while (slot >= (uint32_t)p.nslots) { slot -= (uint32_t)p.nslots; par ^= 1u; }
+            }
+        }
+    } else if (warp == 1 && rank != 0) {
+        // =========================== peer CTA: ring forwarder ===========================
+        // The leader's MMAs read this CTA's half of every ring slot; a bulk copy can only signal a barrier of its own
+        // CTA, so one thread waits for each local fill and arrives on the leader's WFULL barrier of the same slot.
+        if (elect_one()) {
+            const long long total = ntl * (long long)p.nfills;
+            uint32_t slot = 0, par = 0;
+            for (long long q = 0; q < total; ++q) {
+                mbar_wait(&bars[BAR_WFULL + slot], par);
+                mbar_arrive_cluster(BAR_ADDR(BAR_WFULL + slot), 0);
+                if (++slot == (uint32_t)p.nslots) { slot = 0; par ^= 1u; }
+            }
+        }
+        __syncwarp();
+    } else if (warp == 1) {
+        // =========================== leader CTA: MMA issuer, ONE elected thread ===========================
+        // Ops of a tile (p.optype / p.opchunk) are issued in order, op k into accumulator k % nacc; the consumer of an
+        // in-place op (P2 / W3 MMAs reading the fp16 chunk the epilogue wrote over the accumulator) is issued nacc - 1
+        // ops later, i.e. just before the accumulator's next producer — the tensor pipe executes in issue order, so
+        // MMA-after-MMA hazards need no barrier; only epilogue <-> MMA hand-overs do (FULL / EDONE).
+        if (elect_one()) {
+            const uint32_t a1_lo = (smem_base + SL.a1) >> 4, res_lo = (smem_base + SL.res) >> 4;
+            const uint32_t slots_lo = (smem_base + SL.slots) >> 4, slot_step = p.slot_bytes >> 4;
+            // descriptor words: lo = addr/16 | (lbo/16) << 16, hi = sbo/16 | version 1 << 14 | layout << 29
+            const uint32_t lo_noswz = (128u >> 4) << 16, hi_noswz = (((uint32_t)(KI / 8) * 128u) >> 4) | (1u << 14);
+            const uint32_t lo_sw128 = (16u >> 4) << 16, hi_sw128 = (1024u >> 4) | (1u << 14) | (2u << 29);
+            const uint32_t id128 = idesc_f16(256, CN), id16 = idesc_f16(256, 16), id0 = idesc_f16(256, 0);
+            const uint32_t nslots = (uint32_t)p.nslots, lag = nacc - 1;
+            const uint32_t tm_d3 = tmem + p.tm_d3, tm_ph = tm_d3 + (uint32_t)KO - 16, tm_a0 = tmem + p.tm_a0;
+            uint32_t slot = 0, wpar = 0, slot_lo = slots_lo;
+            uint32_t acc = 0, use = 0;                   // accumulator / use count of the next op
+            uint32_t d0 = 0, d1 = 0, d2 = 0;             // EDONE phases consumed per accumulator
+#define SPIN_CL(id, par) do { mbar_spin_cl(BAR_ADDR(id), (par)); tc_fence_after(); } while (0)
+#define ENSURE1(dx, idx, u) do { while (dx <= (u)) { mbar_spin_cl(BAR_ADDR(BAR_EDONE + idx), dx & 1u); ++dx; } } while (0)
+            // op on accumulator a with use count u has been through its chunk epilogue
+#define ENSURE(a, u) do { if ((a) == 0) ENSURE1(d0, 0, u); else if ((a) == 1) ENSURE1(d1, 1, u); else ENSURE1(d2, 2, u); tc_fence_after(); } while (0)
+#define SLOT_ACQUIRE(w) do { if ((w) & SUB_NEW) { mbar_spin_cl(BAR_ADDR(BAR_WFULL + slot), wpar); tc_fence_after(); } } while (0)
+#define SLOT_RELEASE(w) do { if ((w) & SUB_END) { mma_commit_cg2(BAR_ADDR(BAR_WEMPTY + slot)); slot_lo += slot_step; \
+                             if (++slot == nslots) { slot = 0; wpar ^= 1u; slot_lo = slots_lo; } } } while (0)
+            for (long long ti = 0; ti < ntl; ++ti) {
+                uint32_t si = 0, a1_ready = 0;
+                bool d3_open = false;
+                const uint32_t acc0 = acc, use0 = use;
+                SPIN_CL(BAR_A0FULL, (uint32_t)ti & 1u);
+                // consumer of tile-local op jc whose accumulator / use count are (ca, cu)
+                auto consume = [&](uint32_t jc, uint32_t ca, uint32_t cu) {
+                    const uint32_t type = p.optype[jc];
+                    if (type == T_L1S) return;
+                    ENSURE(ca, cu);
+                    if (!d3_open) { SPIN_CL(BAR_D3EMPTY, (uint32_t)ti & 1u); d3_open = true; }     // first write into D3 of this tile
+                    const uint32_t a_t = tmem + ca * CN;
+                    if (type == T_P) {                                          // resident P2 tile of this chunk, N = 16
+                        const uint32_t b_lo = (res_lo + (uint32_t)p.opchunk[jc] * (2048u >> 4)) | lo_sw128;
+#pragma unroll
+                        for (uint32_t ks = 0; ks < 8; ++ks)
+                            mma_ts_cg2(tm_ph, a_t + 8 * ks, b_lo + (ks >> 2) * (1024u >> 4) + 2 * (ks & 3), hi_sw128, id16, 1u);
+                    } else {                                                    // streamed layer-3 tile
+                        const uint32_t w = p.sub[si++];
+                        SLOT_ACQUIRE(w);
+                        const uint32_t nlo = ((w >> SUB_AUX_SHIFT) & 0xFFu) * 16;      // output rows below n_lo receive exactly 0
+                        const uint32_t N = (uint32_t)KO - nlo, kb_step = (N >> 1) * (128u >> 4);
+                        const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_sw128, idesc = id0 | ((N >> 3) << 17);
+#pragma unroll
+                        for (uint32_t ks = 0; ks < 8; ++ks)
+                            mma_ts_cg2(tm_d3 + nlo, a_t + 8 * ks, b_lo + (ks >> 2) * kb_step + 2 * (ks & 3), hi_sw128, idesc, 1u);
+                        SLOT_RELEASE(w);
+                    }
+                };
+#pragma unroll 1
+                for (uint32_t j = 0; j < nops; ++j) {
+                    const uint32_t type = p.optype[j], c = p.opchunk[j];
+                    if (use > 0) ENSURE(acc, use - 1);                          // the accumulator's previous op is through its epilogue
+                    const uint32_t d = tmem + acc * CN;
+                    if (type == T_L2) {
+                        // A1 chunks 0 .. l2need[c] written (layer-1 ops are the first NC ops of the tile)
+                        const uint32_t need = p.l2need[c];
+                        while (a1_ready <= need) {
+                            uint32_t a = acc0 + a1_ready, u = use0;
+                            if (a >= nacc) { a -= nacc; ++u; }
+                            if (a >= nacc) { a -= nacc; ++u; }
+                            ENSURE(a, u);
+                            ++a1_ready;
+                        }
+                        const uint32_t nb = p.nblk[c];
+                        uint32_t accum = 0;
+#pragma unroll 1
+                        for (uint32_t b = 0; b < nb; ++b) {
+                            const uint32_t w = p.sub[si++];
+                            SLOT_ACQUIRE(w);
+                            const uint32_t aux = (w >> SUB_AUX_SHIFT) & 0xFFu, kmask = aux >> 4;
+                            const uint32_t a_lo = (a1_lo + (aux & 7u) * (16384u >> 4)) | lo_sw128;
+                            const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_sw128;
+                            if (kmask == 0xFu) {
+                                mma_ss_cg2(d, a_lo, hi_sw128, b_lo, hi_sw128, id128, accum);
+                                mma_ss_cg2(d, a_lo + 2, hi_sw128, b_lo + 2, hi_sw128, id128, 1u);
+                                mma_ss_cg2(d, a_lo + 4, hi_sw128, b_lo + 4, hi_sw128, id128, 1u);
+                                mma_ss_cg2(d, a_lo + 6, hi_sw128, b_lo + 6, hi_sw128, id128, 1u);
+                                accum = 1u;
+                            } else {
+#pragma unroll
+                                for (uint32_t ks = 0; ks < 4; ++ks)
+                                    if ((kmask >> ks) & 1u) { mma_ss_cg2(d, a_lo + 2 * ks, hi_sw128, b_lo + 2 * ks, hi_sw128, id128, accum); accum = 1u; }
+                            }
+                            SLOT_RELEASE(w);
+                        }
+                    } else {
+                        // input layers (layer 1 / phase hidden): A = A0 in TMEM, B = this chunk's rows, K-step prefix
+                        const uint32_t w = p.sub[si++];
+                        SLOT_ACQUIRE(w);
+                        const uint32_t nk = (w >> SUB_AUX_SHIFT) & 0xFFu;
+                        const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_noswz;
+                        mma_ts_cg2(d, tm_a0, b_lo, hi_noswz, id128, 0u);
+#pragma unroll 1
+                        for (uint32_t ks = 1; ks < nk; ++ks) mma_ts_cg2(d, tm_a0 + 8 * ks, b_lo + 16 * ks, hi_noswz, id128, 1u);
+                        SLOT_RELEASE(w);
+                    }
+                    mma_commit_cg2(BAR_ADDR(BAR_FULL + acc));
+                    if ((int)j == p.last_a0_op) mma_commit_cg2(BAR_ADDR(BAR_A0FREE));     // A0 may be rebuilt for the next tile
+                    if ((int)j == p.last_l2_op) mma_commit_cg2(BAR_ADDR(BAR_A1FREE));     // A1 may be rewritten by the next tile
+                    if (j >= lag) {                                                       // consumer of op j - lag
+                        const uint32_t ca = acc >= lag ? acc - lag : acc + nacc - lag, cu = acc >= lag ? use : use - 1;
+                        consume(j - lag, ca, cu);
+                    }
+                    if (++acc == nacc) { acc = 0; ++use; }
+                }
+                for (uint32_t m = lag; m >= 1; --m) {                                     // consumers of the last ops
+                    if (nops < m) continue;
+                    const uint32_t ca = acc >= m ? acc - m : acc + nacc - m, cu = acc >= m ? use : use - 1;
+                    consume(nops - m, ca, cu);
+                }
+                mma_commit_cg2(BAR_ADDR(BAR_D3FULL));
+            }
+#undef SPIN_CL
+#undef ENSURE1
+#undef ENSURE
+#undef SLOT_ACQUIRE
+#undef SLOT_RELEASE
+        }
+        __syncwarp();
+    } else if (warp < 10) {
+        // =========================== chunk epilogue groups: ops alternate between the two groups ===========================
+        const uint32_t grp = (uint32_t)(warp - 2) >> 2;
+        const uint32_t row = (uint32_t)((warp & 3) * 32 + lane);
+        const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;     // TMEM lane quadrant of this warp
+        const uint32_t a1_row = smem_base + SL.a1 + (row >> 3) * 1024u + (row & 7u) * 128u, sw = row & 7u;
+        const long long total_ops = ntl * (long long)nops;
+        uint32_t acc = grp, use = 0, j = grp;
+        long long ti = 0, seen_ti = 0;
+        for (long long k = grp; k < total_ops; k += 2) {
+            const uint32_t type = p.optype[j], c = p.opchunk[j];
+            mbar_wait(&bars[BAR_FULL + acc], use & 1u);
+            tc_fence_after();
+            if (p.L == 2 && seen_ti != ti) {               // once per tile: the previous tile's layer-2 MMAs have read A1
+                mbar_wait(&bars[BAR_A1FREE], (uint32_t)(ti - 1) & 1u);
+                seen_ti = ti;
+            }
+            const uint32_t d_addr = tmem + lane_base + acc * CN;
+            const float *bias = s_bias + (type == T_P ? 0 : (type == T_L2 ? 2 * H : H)) + c * CN;
+            uint32_t va[32], vb[32];
+            tmem_ld32p(d_addr, va);
+#pragma unroll
+            for (int pc = 0; pc < 4; ++pc) {
+                uint32_t *v = (pc & 1) ? vb : va;
+                tmem_wait_ld();
+                if (pc < 3) tmem_ld32p(d_addr + 32 * (pc + 1), (pc & 1) ? va : vb);     // next piece in flight
+                const float4 *bp = reinterpret_cast<const float4 *>(bias + 32 * pc);
+                uint32_t w[16];
+#pragma unroll
+                for (int j4 = 0; j4 < 8; ++j4) {
+                    const float4 bb = bp[j4];
+                    w[2 * j4] = cvt_relu_f16x2(__uint_as_float(v[4 * j4]) + bb.x, __uint_as_float(v[4 * j4 + 1]) + bb.y);
+                    w[2 * j4 + 1] = cvt_relu_f16x2(__uint_as_float(v[4 * j4 + 2]) + bb.z, __uint_as_float(v[4 * j4 + 3]) + bb.w);
+                }
+                if (type == T_L1S) {
+                    // 32 hidden units = 64 B of this row: four 16-byte pieces of K-block 2c + pc/2, 128B swizzle
+                    const uint32_t kb_addr = a1_row + (2 * c + (uint32_t)(pc >> 1)) * 16384u;
+#pragma unroll
+                    for (uint32_t i = 0; i < 4; ++i) {
+                        const uint32_t jj = (uint32_t)(pc & 1) * 4 + i;
+                        st_shared_v4(kb_addr + ((jj ^ sw) << 4), w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
+                    }
+                } else {
+                    tmem_st16p(d_addr + 16 * pc, w);          // in place: columns [16 pc, 16 pc + 16) were read by piece pc / 2 <= pc
+                }
+            }
+            if (type == T_L1S) fence_proxy_async(); else tmem_wait_st();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(BAR_ADDR(BAR_EDONE + acc), 0);
+            acc += 2; while (acc >= nacc) { acc -= nacc; ++use; }
+            j += 2; if (j >= nops) { j -= nops; ++ti; }
+        }
+    } else {
+        // =========================== tile warps: A0 of the next tile, contraction, final epilogue ===========================
+        const int q = warp & 3;
+        const int row = q * 32 + lane;
+        const uint32_t lane_base = (uint32_t)(q * 32) << 16;
+        const uint32_t d3_addr = tmem + lane_base + p.tm_d3, a0_addr = tmem + lane_base + p.tm_a0;
+        const float *s_b3 = s_bias + 3 * H, *s_c2 = s_bias + 3 * H + KO;
+        const uint32_t zero16[16] = {0};
+
+        struct RowState { long long sb, i; ulonglong2 xp, xq; float2 b0; };
+        auto load_row = [&](long long sb, bool valid, RowState &r) {
+            r.sb = sb; r.i = valid ? sb * TILE_M + row : p.B;
+            if (r.i < p.B) {
+                r.xp = p.xpos[r.i];
+                if (p.mode == 1) { r.xq = p.x[r.i]; r.b0 = p.base[r.i]; }
+                else { r.xq = make_ulonglong2(0, 0); r.b0 = make_float2(0.f, 0.f); }
+            } else { r.i = p.B; r.xp = make_ulonglong2(0, 0); r.xq = r.xp; r.b0 = make_float2(0.f, 0.f); }
+        };
+        // (a2) A0: +-1 fp16, one row per thread = one TMEM lane, 16 inputs = 8 columns per K-step
+        auto build_a0 = [&](ulonglong2 zp) {
+            for (int kc = 0; kc < KI / 16; ++kc) {
+                const uint32_t bits = (uint32_t)(shr128(zp, kc * 16) & 0xFFFFull);
+                uint32_t w[8];
+#pragma unroll
+                for (int jj = 0; jj < 8; ++jj)
+                    w[jj] = 0xBC00BC00u ^ (((bits >> (2 * jj)) & 1u) << 15) ^ (((bits >> (2 * jj + 1)) & 1u) << 31);
+                tmem_st8p(a0_addr + 8 * kc, w);
+            }
+            tmem_wait_st();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(BAR_ADDR(BAR_A0FULL), 0);
+        };
+        auto flip_of = [&](long long t, bool valid) -> ulonglong2 {
+            if (p.mode != 1 || !valid) return make_ulonglong2(0, 0);
+            return __ldg(&p.fpos[p.g_begin + (t % Gnd)]);
+        };
+
+        // D3 accumulates from zero (every MMA into it has accumulate = 1)
+        for (int c = 0; c < KO; c += 16) tmem_st16(d3_addr + c, zero16);
+        tmem_wait_st();
+        tc_fence_before();
+        __syncwarp();
+        if (lane == 0) mbar_arrive_cluster(BAR_ADDR(BAR_D3EMPTY), 0);
+
+        RowState cur{}, nxt{};
+        ulonglong2 zp = make_ulonglong2(0, 0), zp_n = zp;
+        float2 E = make_float2(0.f, 0.f);
+        float mr = (p.mode == 1 && p.hm.has_diag) ? 1.0f : 0.0f;     // the f = 0 group has ratio exactly 1
+        if (ntl > 0) {
+            const long long t = 2 * q_lo + rank;
+            const bool valid = t < ntiles;
+            load_row(t / Gnd, valid, cur);
+            const ulonglong2 f = flip_of(t, valid);
+            zp = make_ulonglong2(cur.xp.x ^ f.x, cur.xp.y ^ f.y);
+            build_a0(zp);
+        }
+        for (long long ti = 0; ti < ntl; ++ti) {
+            const long long t = 2 * (q_lo + ti) + rank;
+            const bool valid = t < ntiles;
+            const long long g = p.g_begin + (t % Gnd);
+            const bool has_next = ti + 1 < ntl;
+            if (has_next) {
+                const long long tn = t + 2;
+                const bool validn = tn < ntiles;
+                const long long sbn = tn / Gnd;
+                if (sbn != cur.sb || !validn) load_row(sbn, validn, nxt); else nxt = cur;
+                const ulonglong2 f = flip_of(tn, validn);
+                zp_n = make_ulonglong2(nxt.xp.x ^ f.x, nxt.xp.y ^ f.y);
+            }
+            // ---- (a3) S = sum_{t in g} c_t (-i)^{r_t} (-1)^{popcount(x & s_t)}: independent of the MMAs, done while they run ----
+            float2 S = make_float2(0.f, 0.f);
+            if (p.mode == 1 && valid && cur.i < p.B) {
+                const uint32_t t1 = __ldg(&p.hm.offsets[g + 1]);
+                for (uint32_t tt = __ldg(&p.hm.offsets[g]); tt < t1; ++tt) {
+                    const ulonglong2 zy = __ldg(&p.hm.zy[tt]);
+                    const float2 c = __ldg(&p.hm.cph[tt]);
+                    const bool neg = ((__popcll(cur.xq.x & zy.x) + __popcll(cur.xq.y & zy.y)) & 1) != 0;
+                    S.x += neg ? -c.x : c.x;
+                    S.y += neg ? -c.y : c.y;
+                }
+            }
+            // ---- operand tile of the NEXT tile, once the last MMA that reads the current one has completed ----
+            if (has_next) {
+                mbar_wait(&bars[BAR_A0FREE], (uint32_t)ti & 1u);
+                tc_fence_after();
+                build_a0(zp_n);
+            }
+            // ---- final epilogue: log|psi| = 1/2 sum_d log sigmoid(+-a_d), phi = o[2 z_{n-2} + z_{n-1}] ----
+            mbar_wait(&bars[BAR_D3FULL], (uint32_t)ti & 1u);
+            tc_fence_after();
+            // sum_d log sigmoid(t_d) = sum_d min(t_d, 0) - ln prod_d (1 + exp(-|t_d|)): every factor is in (1, 2], so a
+            // 16-term product cannot overflow and costs one LG2 per 16 conditionals; the 16 chains are independent (ILP).
+            float msum = 0.0f, lg = 0.0f, phi = 0.0f;
+            for (int c0 = 0; c0 < KO; c0 += 16) {
+                uint32_t v[16];
+                tmem_ld16p(d3_addr + c0, v);
+                tmem_wait_ld();
+                tmem_st16(d3_addr + c0, zero16);              // D3 restarts from zero for the next tile
+                if (c0 + 16 >= KO) {
+                    const int sel = (int)((shr128(zp, p.n - 2) & 1ull) * 2 + (shr128(zp, p.n - 1) & 1ull));
+                    const float o0 = __uint_as_float(v[12]) + s_c2[0], o1 = __uint_as_float(v[13]) + s_c2[1];
+                    const float o2 = __uint_as_float(v[14]) + s_c2[2], o3 = __uint_as_float(v[15]) + s_c2[3];
+                    phi = sel == 0 ? o0 : (sel == 1 ? o1 : (sel == 2 ? o2 : o3));
+                }
+                const uint32_t zb = (uint32_t)shr128(zp, c0);
+                const int nv = p.n - c0;                       // valid conditionals in this block (may be <= 0 or >= 16)
+                const float4 *bp = reinterpret_cast<const float4 *>(s_b3 + c0);
+                float prod0 = 1.0f, prod1 = 1.0f, m0 = 0.0f, m1 = 0.0f;
+#pragma unroll
+                for (int k4 = 0; k4 < 4; ++k4) {
+                    const float4 bb = bp[k4];
+                    const float bk[4] = {bb.x, bb.y, bb.z, bb.w};
+#pragma unroll
+                    for (int kk = 0; kk < 4; ++kk) {
+                        const int k = 4 * k4 + kk;
+                        const float a = __uint_as_float(v[k]) + bk[kk];
+                        float tt = ((zb >> k) & 1u) ? a : -a;
+                        tt = (k < nv) ? tt : 1e30f;            // padding column: factor 1, min 0
+                        const float e = ex2_ftz(fabsf(tt) * -1.4426950408889634f);
+                        if (k & 1) { prod1 *= 1.0f + e; m1 += fminf(tt, 0.0f); }
+                        else       { prod0 *= 1.0f + e; m0 += fminf(tt, 0.0f); }
+                    }
+                }
+                msum += m0 + m1;
+                lg += lg2_ftz(prod0 * prod1);
+            }
+            const float part = msum - 0.6931471805599453f * lg;
+            tmem_wait_st();
+            tc_fence_before();
+            __syncwarp();
+            if (lane == 0) mbar_arrive_cluster(BAR_ADDR(BAR_D3EMPTY), 0);
+            const float lp = 0.5f * part;
+            if (p.mode == 0) {
+                if (cur.i < p.B) p.out[cur.i] = make_float2(lp, phi);
+            } else if (cur.i < p.B) {
+                // (a5)
+                const float mag = __expf(lp - cur.b0.x);
+                float sn, cs;
+                __sincosf(phi - cur.b0.y, &sn, &cs);
+                const float rr = mag * cs, ri = mag * sn;
+                mr = fmaxf(mr, mag);
+                E.x += S.x * rr - S.y * ri;
+                E.y += S.x * ri + S.y * rr;
+            }
+            if (!has_next || nxt.sb != cur.sb || nxt.i != cur.i) {
+                if (p.mode == 1 && cur.i < p.B) {
+                    atomicAdd(&p.eloc[2 * cur.i], E.x);
+                    atomicAdd(&p.eloc[2 * cur.i + 1], E.y);
+                }
+                E = make_float2(0.f, 0.f);
+            }
+            cur = nxt; zp = zp_n;
+        }
+        if (p.mode == 1) atomicMax(p.max_ratio_bits, __float_as_uint(mr));
+    }
+#undef BAR_ADDR
+    tc_fence_before();
+    cluster_sync_all();
+    if (warp == 1) tmem_dealloc_cg2(tmem, 512);
+}
+
+// position-ordered copy of 128-bit configurations: out bit d = in bit order[d]
+__global__ void permute_bits_kernel(const ulonglong2 *__restrict__ in, long long N, const int32_t *__restrict__ order, int n,
+                                    ulonglong2 *__restrict__ out) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= N) return;
+    const ulonglong2 a = in[i];
+    unsigned long long lo = 0, hi = 0;
+    for (int d = 0; d < n; ++d) {
+        const int qb = __ldg(order + d);
+        const unsigned long long bit = ((qb < 64 ? a.x : a.y) >> (qb & 63)) & 1ull;
+        if (d < 64) lo |= bit << d; else hi |= bit << (d - 64);
+    }
+    out[i] = make_ulonglong2(lo, hi);
+}
+
+// eloc[i] = S[i, group 0] when group 0 is the f = 0 group (psi ratio == 1), else 0.
+__global__ void diag_init_kernel(HamDev hm, const ulonglong2 *__restrict__ x, long long B, float2 *__restrict__ eloc) {
+    const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
+    if (i >= B) return;
+    float2 S = make_float2(0.f, 0.f);
+    if (hm.has_diag) {
+        const ulonglong2 xr = x[i];
+        const uint32_t t1 = hm.offsets[1];
+        for (uint32_t t = hm.offsets[0]; t < t1; ++t) {
+            const ulonglong2 zy = __ldg(&hm.zy[t]);
+            const float2 c = __ldg(&hm.cph[t]);
+            const bool neg = ((__popcll(xr.x & zy.x) + __popcll(xr.y & zy.y)) & 1) != 0;
+            S.x += neg ? -c.x : c.x;
+            S.y += neg ? -c.y : c.y;
+        }
+    }
+    eloc[i] = S;
+}
+
+}  // namespace
+
+// ------------------------------------------------------------------------------------------------------------
+struct Tc2Pack {
+    int KI = 0, KO = 0, NC = 0, nacc = 0, nops = 0, nsub = 0, nfills = 0, nslots = 0, last_a0_op = -1, last_l2_op = -1;
+    uint32_t slot_bytes = 0, res_bytes = 0, img_stride = 0, tm_d3 = 0, tm_a0 = 0;
+    void *d_wimg = nullptr, *d_fills = nullptr, *d_res = nullptr, *d_bias = nullptr;
+    void *d_fpos = nullptr; size_t fpos_cap = 0;
+    void *d_xpos = nullptr; size_t xpos_cap = 0;
+    SmemLayout L{};
+    uint32_t sub[MAX_SUB + 1] = {0};
+    uint8_t nblk[MAX_NC] = {0}, l2need[MAX_NC] = {0}, optype[MAX_OPS] = {0}, opchunk[MAX_OPS] = {0};
+    int sms = 148;
+    long long mma_issued = 0, mma_dense = 0;                   // 16-wide K-steps x N issued / of the dense chain, per tile (MACs / 2048)
+};
+
+static inline int round16(int v) { return (v + 15) / 16 * 16; }
+
+struct Tc2Shape { int KI, KO, NC, nacc, nslots; uint32_t slot; };
+
+static bool tc2_shape(const nqs_made *M, Tc2Shape *out) {
+    if ((M->L != 1 && M->L != 2) || M->h % CN != 0 || M->h < CN || M->h > CN * MAX_NC) return false;
+    Tc2Shape s;
+    s.KI = round16(M->n); s.KO = round16(M->n + 4); s.NC = M->h / CN;
+    if (s.KI > 128 || s.KO > 144) return false;
+    // TMEM: nacc accumulators of CN columns, D3 (KO), A0 (KI/2)
+    s.nacc = 3;
+    if (s.nacc * CN + s.KO + s.KI / 2 > 512) s.nacc = 2;
+    if (s.nacc * CN + s.KO + s.KI / 2 > 512) return false;
+    uint32_t need = (uint32_t)HALF * s.KI * 2;                                 // input sub-tile (64 rows x KI)
+    if ((uint32_t)HALF * 128 > need) need = HALF * 128;                        // layer-2 sub-tile (64 x 64)
+    if ((uint32_t)s.KO * 128 > need) need = (uint32_t)s.KO * 128;              // layer-3 tile (KO/2 rows x 128 K)
+    const uint32_t budget = 227 * 1024 - 1024;
+    const uint32_t fixed = smem_layout(M->h, s.KO, M->L, 0, 0).total;
+    if (fixed + 2 * need > budget) return false;
+    const uint32_t ring = budget - fixed;
+    int ns = 4;                                                                // few, large fills: every ring hand-over costs the issuer a poll
+    while (ns > 2 && (ring / ns) / 1024 * 1024 < 2 * need) --ns;
+    uint32_t slot = (ring / ns) / 1024 * 1024;
+    if (slot < need) return false;
+    if (slot > 0x1FFFu * 16u) slot = 0x1FFFu * 16u / 1024 * 1024;
+    s.slot = slot; s.nslots = ns;
+    *out = s;
+    return true;
+}
+
+bool tc2_supported(const nqs_made *M) {
+    Tc2Shape s;
+    return tc2_shape(M, &s);
+}
+
+static inline uint32_t noswz_offset(uint32_t r, uint32_t k, uint32_t KI) {
+    return (r >> 3) * (KI / 8) * 128u + (k >> 3) * 128u + (r & 7u) * 16u + (k & 7u) * 2u;
+}
+
+int tc2_pack_upload(const nqs_made *M) {
+    if (M->tc2) return NQS_OK;
+    Tc2Shape sh;
+    if (!tc2_shape(M, &sh)) return NQS_EUNSUPPORTED;
+    Tc2Pack *P = new (std::nothrow) Tc2Pack();
+    if (!P) return NQS_ENOMEM;
+    const int n = M->n, H = M->h, NC = sh.NC, KI = sh.KI, KO = sh.KO, L = M->L;
+    P->KI = KI; P->KO = KO; P->NC = NC; P->nacc = sh.nacc; P->slot_bytes = sh.slot; P->nslots = sh.nslots;
+    P->tm_d3 = (uint32_t)sh.nacc * CN; P->tm_a0 = P->tm_d3 + (uint32_t)KO;
+    P->L = smem_layout(H, KO, L, sh.slot, sh.nslots);
+    const uint32_t slot = sh.slot;
+    const uint32_t in_bytes = (uint32_t)HALF * KI * 2, w2_bytes = HALF * 128;
+    const std::vector<float> &W1 = M->wm[0], &W3 = M->wm[L];
+
+    // ---- the per-tile op list (must match the issuer / epilogue loops of eloc_tc2_kernel) ----
+    int nops = 0;
+    if (L == 2) {
+        for (int c = 0; c < NC; ++c) { P->optype[nops] = T_L1S; P->opchunk[nops++] = (uint8_t)c; }
+        for (int c = 0; c < NC; ++c) {
+            P->optype[nops] = T_P; P->opchunk[nops] = (uint8_t)c; P->last_a0_op = nops++;
+            P->optype[nops] = T_L2; P->opchunk[nops] = (uint8_t)c; P->last_l2_op = nops++;
+        }
+    } else {
+        for (int c = 0; c < NC; ++c) {
+            P->optype[nops] = T_L1I; P->opchunk[nops++] = (uint8_t)c;
+            P->optype[nops] = T_P; P->opchunk[nops] = (uint8_t)c; P->last_a0_op = nops++;
+        }
+    }
+    P->nops = nops;
+
+    std::vector<uint8_t> img[2], res[2];
+    res[0].assign((size_t)(H / 64) * 1024, 0); res[1] = res[0];
+    std::vector<uint2> fills;
+    std::vector<uint32_t> sub;
+    auto put = [](std::vector<uint8_t> &buf, size_t off, float v) { __half hv = __float2half_rn(v); memcpy(&buf[off], &hv, 2); };
+
+    // ---- streamed sub-tiles are appended to the open ring fill (<= slot bytes, in consumption order) ----
+    uint32_t fill_start = 0, fill_bytes = 0;
+    auto close_fill = [&]() {
+        if (fill_bytes == 0) return;
+        fills.push_back(make_uint2(fill_start, fill_bytes));
+        sub.back() |= SUB_END;
+        fill_bytes = 0;
+    };
+    auto stream_alloc = [&](uint32_t bytes, uint32_t aux) -> uint32_t {
+        if (fill_bytes + bytes > slot) close_fill();
+        uint32_t w = (aux & 0xFFu) << SUB_AUX_SHIFT;
+        if (fill_bytes == 0) { fill_start = (uint32_t)img[0].size(); w |= SUB_NEW; }
+        w |= (fill_bytes >> 4) & SUB_OFF_MASK;
+        const uint32_t base = fill_start + fill_bytes;
+        img[0].resize(img[0].size() + bytes, 0); img[1].resize(img[1].size() + bytes, 0);
+        fill_bytes += bytes;
+        sub.push_back(w);
+        return base;
+    };
+
+    // input-layer chunk c (layer 1 or phase hidden): rank r holds units 128 c + 64 r .. + 63.  Masked layer-1 columns
+    // are the high ones for sorted degrees; in general the issued K-steps are the prefix up to the last non-zero one.
+    auto input_chunk = [&](int c, bool phase) {
+        const uint32_t base = stream_alloc(in_bytes, 0);
+        int nk = 1;                                             // the accumulator must be overwritten even if all zero
+        for (int r = 0; r < 2; ++r)
+            for (int rr = 0; rr < HALF; ++rr) {
+                const int j = c * CN + r * HALF + rr;
+                for (int k = 0; k < KI; ++k) {
+                    float v = 0.f;
+                    if (phase) { if (k < n - 2) v = M->p1[(size_t)j * (n - 2) + k]; }
+                    else if (k < n) v = W1[(size_t)j * n + k];
+                    put(img[r], base + noswz_offset(rr, k, KI), v);
+                    if (v != 0.0f && k / 16 + 1 > nk) nk = k / 16 + 1;
+                }
+            }
+        sub.back() |= (uint32_t)nk << SUB_AUX_SHIFT;
+        P->mma_issued += (long long)nk * CN; P->mma_dense += (long long)(KI / 16) * CN;
+    };
+    // resident P2 tile of phase chunk c: rows 12..15 of the 16-row tile hold the 4 phase outputs -> rank 1, rows 4..7
+    auto phase_out_tile = [&](int c) {
+        for (int o = 0; o < 4; ++o)
+            for (int k = 0; k < CN; ++k)
+                put(res[1], (size_t)c * 2048 + (size_t)(k / 64) * 1024 + sw128_offset(4 + o, k % 64), M->p2[(size_t)o * H + c * CN + k]);
+        P->mma_issued += 8 * 16; P->mma_dense += 8 * 16;
+    };
+    // layer-2 chunk c2: k-blocks of 64 with any non-zero weight, and inside a block only the non-zero K-steps
+    auto l2_chunk = [&](int c2) {
+        const std::vector<float> &W2 = M->wm[1];
+        int nb = 0, need = 0;
+        for (int kb = 0; kb < H / 64; ++kb) {
+            uint32_t kmask = 0;
+            for (int r = 0; r < CN; ++r)
+                for (int k = 0; k < 64; ++k)
+                    if (W2[(size_t)(c2 * CN + r) * H + kb * 64 + k] != 0.0f) kmask |= 1u << (k / 16);
+            P->mma_dense += 4 * CN;
+            if (!kmask && !(nb == 0 && kb == H / 64 - 1)) continue;      // exact: an all-zero block adds 0
+            if (!kmask) kmask = 1;                                       // nothing at all: still overwrite the accumulator
+            const uint32_t base = stream_alloc(w2_bytes, (uint32_t)kb | (kmask << 4));
+            for (int r = 0; r < 2; ++r)
+                for (int rr = 0; rr < HALF; ++rr)
+                    for (int k = 0; k < 64; ++k)
+                        put(img[r], base + sw128_offset(rr, k), W2[(size_t)(c2 * CN + r * HALF + rr) * H + kb * 64 + k]);
+            P->mma_issued += (long long)__builtin_popcount(kmask) * CN;
+            need = kb / 2;
+            ++nb;
+        }
+        P->nblk[c2] = (uint8_t)nb; P->l2need[c2] = (uint8_t)need;
+    };
+    // streamed layer-3 tile of hidden chunk c: N = KO - n_lo output rows (rows below the first non-zero one receive
+    // exactly 0 from this chunk), rank r holds rows n_lo + r N/2 .. ; two K-blocks of N/2 rows x 128 B
+    auto w3_tile = [&](int c) {
+        int row_lo = KO;
+        for (int d = 0; d < n; ++d)
+            for (int k = 0; k < CN; ++k)
+                if (W3[(size_t)d * H + c * CN + k] != 0.0f && d < row_lo) row_lo = d;
+        const int n_lo = row_lo >= KO ? KO - 16 : (row_lo / 16) * 16;
+        const int N = KO - n_lo, Nh = N / 2;
+        const uint32_t base = stream_alloc((uint32_t)2 * Nh * 128, (uint32_t)(n_lo / 16));
+        for (int r = 0; r < 2; ++r)
+            for (int rr = 0; rr < Nh; ++rr) {
+                const int d = n_lo + r * Nh + rr;
+                if (d >= n) continue;
+                for (int k = 0; k < CN; ++k)
+                    put(img[r], base + (size_t)(k / 64) * Nh * 128 + sw128_offset(rr, k % 64), W3[(size_t)d * H + c * CN + k]);
+            }
+        P->mma_issued += (long long)8 * N; P->mma_dense += (long long)8 * KO;
+    };
+    auto emit_op = [&](int j) {
+        const int c = P->opchunk[j];
+        switch (P->optype[j]) {
+            case T_L1S: case T_L1I: input_chunk(c, false); break;
+            case T_P: input_chunk(c, true); phase_out_tile(c); break;
+            default: l2_chunk(c); break;
+        }
+    };
+    auto emit_consumer = [&](int j) {
+        if (P->optype[j] == T_L2 || P->optype[j] == T_L1I) w3_tile(P->opchunk[j]);
+    };
+    const int lag = sh.nacc - 1;
+    for (int j = 0; j < nops; ++j) { emit_op(j); if (j >= lag) emit_consumer(j - lag); }
+    for (int m = lag; m >= 1; --m) if (nops >= m) emit_consumer(nops - m);
+    close_fill();
+    P->nsub = (int)sub.size(); P->nfills = (int)fills.size();
+    P->res_bytes = (uint32_t)res[0].size();
+    if (P->nsub > MAX_SUB) { delete P; return NQS_EUNSUPPORTED; }
+    memcpy(P->sub, sub.data(), sub.size() * 4);
+    P->img_stride = (uint32_t)((img[0].size() + 255) & ~(size_t)255);
+
+    // biases: [c1 | b1 | b2 | b3 (KO) | c2]
+    std::vector<float> bias((size_t)3 * H + KO + 4, 0.f);
+    for (int j = 0; j < H; ++j) { bias[j] = M->c1[j]; bias[H + j] = M->bias[0][j]; if (L == 2) bias[2 * H + j] = M->bias[1][j]; }
+    for (int d = 0; d < n; ++d) bias[3 * H + d] = M->bias[L][d];
+    for (int o = 0; o < 4; ++o) bias[3 * H + KO + o] = M->c2[o];
+
+    std::vector<uint8_t> wboth((size_t)2 * P->img_stride, 0), rboth((size_t)2 * P->res_bytes, 0);
+    for (int r = 0; r < 2; ++r) {
+        memcpy(&wboth[(size_t)r * P->img_stride], img[r].data(), img[r].size());
+        memcpy(&rboth[(size_t)r * P->res_bytes], res[r].data(), res[r].size());
+    }
+    int dev = 0; cudaGetDevice(&dev);
+    cudaDeviceGetAttribute(&P->sms, cudaDevAttrMultiProcessorCount, dev);
+    auto up = [](void **dst, const void *src, size_t bytes) {
+        return cudaMalloc(dst, bytes ? bytes : 16) == cudaSuccess && (bytes == 0 || cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice) == cudaSuccess);
+    };
+    const bool ok = up(&P->d_wimg, wboth.data(), wboth.size()) && up(&P->d_fills, fills.data(), fills.size() * sizeof(uint2)) &&
+                    up(&P->d_res, rboth.data(), rboth.size()) && up(&P->d_bias, bias.data(), bias.size() * 4);
+    if (!ok) {
+        cudaGetLastError();
+        cudaFree(P->d_wimg); cudaFree(P->d_fills); cudaFree(P->d_res); cudaFree(P->d_bias);
+        delete P;
+        return NQS_ECUDA;
+    }
+    M->tc2 = P;
+    return NQS_OK;
+}
+
+void tc2_pack_free(const nqs_made *M) {
+    if (!M->tc2) return;
+    Tc2Pack *P = M->tc2;
+    cudaFree(P->d_wimg); cudaFree(P->d_fills); cudaFree(P->d_res); cudaFree(P->d_bias);
+    if (P->d_fpos) cudaFree(P->d_fpos);
+    if (P->d_xpos) cudaFree(P->d_xpos);
+    delete P;
+    M->tc2 = nullptr;
+}
+
+void tc2_mma_counts(const nqs_made *M, long long *issued, long long *dense) {
+    *issued = M->tc2 ? M->tc2->mma_issued : 0;
+    *dense = M->tc2 ? M->tc2->mma_dense : 0;
+}
+
+static void fill_common(const nqs_made *M, Tc2Params &p) {
+    const Tc2Pack *P = M->tc2;
+    p.n = M->n; p.H = M->h; p.NC = P->NC; p.KI = P->KI; p.KO = P->KO; p.L = M->L; p.nacc = P->nacc; p.nops = P->nops;
+    p.last_a0_op = P->last_a0_op; p.last_l2_op = P->last_l2_op;
+    p.tm_d3 = P->tm_d3; p.tm_a0 = P->tm_a0;
+    p.wimg = (const uint8_t *)P->d_wimg; p.img_stride = P->img_stride;
+    p.fills = (const uint2 *)P->d_fills; p.nfills = P->nfills;
+    memcpy(p.sub, P->sub, sizeof(p.sub)); memcpy(p.nblk, P->nblk, sizeof(p.nblk)); memcpy(p.l2need, P->l2need, sizeof(p.l2need));
+    memcpy(p.optype, P->optype, sizeof(p.optype)); memcpy(p.opchunk, P->opchunk, sizeof(p.opchunk));
+    p.resimg = (const uint8_t *)P->d_res; p.res_bytes = P->res_bytes;
+    p.slot_bytes = P->slot_bytes; p.nslots = P->nslots;
+    p.bias = (const float *)P->d_bias;
+}
+
+static int ensure(void **buf, size_t *cap, size_t bytes) {
+    if (*cap >= bytes) return NQS_OK;
+    if (*buf) cudaFree(*buf);
+    *buf = nullptr; *cap = 0;
+    if (cudaMalloc(buf, bytes) != cudaSuccess) { cudaGetLastError(); return NQS_ENOMEM; }
+    *cap = bytes;
+    return NQS_OK;
+}
+
+static int permuted(const nqs_made *M, const ulonglong2 *in, long long N, ulonglong2 *out, cudaStream_t st) {
+    permute_bits_kernel<<<(unsigned)((N + 255) / 256), 256, 0, st>>>(in, N, M->dev.order, M->n, out);
+    ++g_launch_count;
+    return cudaGetLastError() == cudaSuccess ? NQS_OK : NQS_ECUDA;
+}
+
+static int launch_chain(const Tc2Pack *P, const Tc2Params &p, long long ntiles, cudaStream_t st) {
+    // the attribute is per device and per kernel; setting it is a cheap host call, so no process-wide cache
+    if (cudaFuncSetAttribute(eloc_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->L.total) != cudaSuccess) {
+        cudaGetLastError();
+        return NQS_ECUDA;
+    }
+    const long long npairs = (ntiles + 1) / 2;
+    const long long ncl_max = P->sms / 2;
+    const int grid = 2 * (int)(npairs < ncl_max ? npairs : ncl_max);
+    eloc_tc2_kernel<<<grid, NTHREADS, P->L.total, st>>>(p);
+    ++g_launch_count;
+    return cudaGetLastError() == cudaSuccess ? NQS_OK : NQS_ECUDA;
+}
+
+int launch_logpsi_tc2(const nqs_made *M, const ulonglong2 *cfg, long long B, float2 *out, cudaStream_t st) {
+    if (B <= 0) return NQS_OK;
+    Tc2Pack *P = M->tc2;
+    if (!P) return NQS_EUNSUPPORTED;
+    int rc = ensure(&P->d_xpos, &P->xpos_cap, sizeof(ulonglong2) * (size_t)B);
+    if (rc) return rc;
+    if ((rc = permuted(M, cfg, B, (ulonglong2 *)P->d_xpos, st))) return rc;
+    Tc2Params p{};
+    fill_common(M, p);
+    p.mode = 0; p.xpos = (const ulonglong2 *)P->d_xpos; p.B = B; p.out = out;
+    return launch_chain(P, p, (B + TILE_M - 1) / TILE_M, st);
+}
+
+int launch_eloc_tc2(const HamDev &hm, const nqs_made *M, const ulonglong2 *x, const float2 *base, long long B,
+                    float2 *eloc, unsigned *max_ratio_bits, cudaStream_t st) {
+    if (B <= 0) return NQS_OK;
+    Tc2Pack *P = M->tc2;
+    if (!P) return NQS_EUNSUPPORTED;
+    int rc;
+    // position-ordered flips: rebuilt on the caller's stream for every launch (19 MB of traffic at cfg 5, microseconds
+    // next to the chain kernel).  No cache: a device address is not an identity (a freed Hamiltonian's buffers are
+    // handed to the next one of the same size), and a cache filled on one stream is unordered against another.
+    if ((rc = ensure(&P->d_fpos, &P->fpos_cap, sizeof(ulonglong2) * (size_t)(hm.G ? hm.G : 1)))) return rc;
+    if (hm.G > 0 && (rc = permuted(M, hm.flips, hm.G, (ulonglong2 *)P->d_fpos, st))) return rc;
+    if ((rc = ensure(&P->d_xpos, &P->xpos_cap, sizeof(ulonglong2) * (size_t)B))) return rc;
+    if ((rc = permuted(M, x, B, (ulonglong2 *)P->d_xpos, st))) return rc;
+    diag_init_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(hm, x, B, eloc);
+    ++g_launch_count;
+    if (cudaGetLastError() != cudaSuccess) return NQS_ECUDA;
+    Tc2Params p{};
+    fill_common(M, p);
+    p.mode = 1; p.xpos = (const ulonglong2 *)P->d_xpos; p.B = B; p.fpos = (const ulonglong2 *)P->d_fpos; p.x = x;
+    p.hm = hm; p.base = base; p.eloc = (float *)eloc; p.max_ratio_bits = max_ratio_bits;
+    p.g_begin = hm.has_diag ? 1 : 0;
+    const long long nsb = (B + TILE_M - 1) / TILE_M;
+    const long long ntiles = nsb * (hm.G - p.g_begin);
+    if (ntiles > 0) return launch_chain(P, p, ntiles, st);
+    return NQS_OK;
+}
