@@ -13,12 +13,13 @@
 //        weights are never issued (exact: they contribute 0),
 //   (a3) the Pauli contraction S[i,g] over the group's terms (popcount parity, (-i)^r folded into c),
 //   (a5) ratio = exp(dlog|psi|) cis(dphi), E_i += S * ratio, kept in registers per sample.
-// Warp roles (14 warps per CTA): 0 = weight producers (TMA 1-D bulk copies of this CTA's half of the weight image into
-// a ring of large slots); 1 = in the leader CTA the MMA issuer (ONE elect.sync thread issues every tcgen05.mma /
+// Warp roles (14 warps per CTA): 12 = weight producers (TMA 1-D bulk copies of this CTA's half of the weight image into
+// a ring of large slots); 13 = in the leader CTA the MMA issuer (ONE elect.sync thread issues every tcgen05.mma /
 // commit of the pair; commits are multicast to the barriers of both CTAs), in the peer CTA a forwarder that tells the
-// leader when the peer's half of a ring slot has landed; 2-5 / 6-9 = two chunk-epilogue groups (ops alternate);
-// 10-13 = tile warps (A0 of the NEXT tile, contraction, final epilogue).  DESIGN.md sections 6-7.
+// leader when the peer's half of a ring slot has landed; 4-7 / 8-11 = two chunk-epilogue groups (ops alternate);
+// 0-3 = tile warps (A0 of the NEXT tile, contraction, final epilogue).  DESIGN.md sections 6-7.
 // PAPER.md:122-134 (Alg. 1), :84-96 (architecture, Eq. 8-10), :152-158 (Eq. 15-16).
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -37,6 +38,11 @@ constexpr int MAX_NC = 4;                // hidden <= 512
 constexpr int MAX_SLOTS = 8;
 constexpr int NPROD = 4;                 // producer lanes (bulk-copy issuers), never more than slots
 constexpr int MAX_OPS = 3 * MAX_NC;
+// warp roles.  The warp scheduler of an SM sub-partition (warp id % 4) prefers the HIGHEST warp id among its eligible
+// warps, and every sub-partition hosts epilogue warps (a warp reaches only TMEM lane quadrant id % 4): the one thread
+// that issues all MMAs therefore lives in the highest warp id of its sub-partition, or it only gets the issue slots
+// the epilogue warps leave over.
+constexpr int W_TILE = 0, W_EPI = 4, W_PROD = 12, W_ISSUE = 13;
 
 enum : uint8_t { T_L1S = 0, T_L1I = 1, T_P = 2, T_L2 = 3 };   // layer 1 -> smem A1 | layer 1 in place | phase hidden | layer 2
 
@@ -78,6 +84,8 @@ struct Tc2Params {
     uint8_t nblk[MAX_NC];                // layer-2 k-blocks issued per output chunk
     uint8_t l2need[MAX_NC];              // layer-2 chunk c needs A1 chunks 0 .. l2need[c]
     uint8_t optype[MAX_OPS], opchunk[MAX_OPS];
+    uint8_t prewait[MAX_OPS];            // bit a: wait for the chunk epilogue pending on accumulator a before issuing op j
+    uint32_t cntmask;                    // bit a: accumulator a is used an odd number of times per tile
     const uint8_t *resimg; uint32_t res_bytes;    // resident P2 tiles of rank r at resimg + r * res_bytes
     uint32_t slot_bytes; int nslots;
     const float *bias;                   // [c1 H | b1 H | b2 H | b3 KO | c2 4] fp32
@@ -92,7 +100,20 @@ struct Tc2Params {
     float *eloc;                         // [B][2], pre-initialised with the f = 0 group; atomically accumulated
     unsigned *max_ratio_bits;
     long long g_begin;                   // first group that needs a forward pass (1 if group 0 is f = 0)
+#ifdef TC2_PROF
+    long long *prof;                     // [grid][16] cycle counters (instrumented build only)
+#endif
 };
+
+#ifdef TC2_PROF
+#define PROF_T0() const long long _t0 = clock64()
+#define PROF_ADD(v) (v) += clock64() - _t0
+#define PROF_STALL(sp) do { if (sp) { pw_stall += clock64() - _t0; ++pw_nstall; } ++pw_npoll; } while (0)
+#else
+#define PROF_T0() do {} while (0)
+#define PROF_ADD(v) do {} while (0)
+#define PROF_STALL(sp) do { (void)(sp); } while (0)
+#endif
 
 __device__ __forceinline__ unsigned long long shr128(ulonglong2 a, int s) {      // low 64 bits of a >> s, 0 <= s < 128
     if (s == 0) return a.x;
@@ -100,7 +121,26 @@ __device__ __forceinline__ unsigned long long shr128(ulonglong2 a, int s) {     
     return a.y >> (s - 64);
 }
 
+// The per-tile op schedule, fixed at compile time so that the issuing thread runs straight-line code (it is
+// instruction-bound: the tensor pipe queues only ~100 cycles of MMAs ahead of the issuer, measured).  Two hidden
+// layers: layer-1 chunks 0..NC-1 (-> A1), then phase chunk c / layer-2 chunk c alternating; one hidden layer: layer-1
+// chunk c (in place) / phase chunk c alternating.  Op j runs in accumulator j % NACC and is handed to epilogue group
+// j & 1; the consumer of an in-place op is issued LAG = NACC - 1 ops later, just before the accumulator's next producer.
+template <int NC, int L, int NACC>
+struct Sched {
+    static constexpr int NOPS = (L == 2) ? 3 * NC : 2 * NC;
+    static constexpr int LAG = NACC - 1;
+    static constexpr int FIRST_INPLACE = (L == 2) ? NC : 0;
+    static constexpr int LAST_A0 = (L == 2) ? NOPS - 2 : NOPS - 1;
+    __host__ __device__ static constexpr int type(int j) {
+        return L == 2 ? (j < NC ? (int)T_L1S : (((j - NC) & 1) ? (int)T_L2 : (int)T_P)) : ((j & 1) ? (int)T_P : (int)T_L1I);
+    }
+    __host__ __device__ static constexpr int chunk(int j) { return L == 2 ? (j < NC ? j : (j - NC) / 2) : j / 2; }
+};
+
+template <int NC, int L, int NACC>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc2_kernel(const __grid_constant__ Tc2Params p) {
+    using S = Sched<NC, L, NACC>;
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t s_tmem_base;
     const SmemLayout SL = smem_layout(p.H, p.KO, p.L, p.slot_bytes, p.nslots);
@@ -109,7 +149,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();
     const int KI = p.KI, KO = p.KO, H = p.H;
-    const uint32_t nacc = (uint32_t)p.nacc, nops = (uint32_t)p.nops;
+    constexpr uint32_t nacc = NACC, nops = S::NOPS;
     const uint32_t smem_base = smem_u32(smem);
     const uint32_t bars_addr = smem_base + SL.bars;
 #define BAR_ADDR(id) (bars_addr + (uint32_t)(id) * 8u)
@@ -125,7 +165,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
         }
         fence_mbar_init();
     }
-    if (warp == 1) tmem_alloc_cg2(&s_tmem_base, 512);
+    if (warp == W_ISSUE) tmem_alloc_cg2(&s_tmem_base, 512);
     for (int i = threadIdx.x; i < 3 * H + KO + 4; i += NTHREADS) s_bias[i] = p.bias[i];
     for (int i = threadIdx.x; i < (int)(p.res_bytes / 16); i += NTHREADS)
         reinterpret_cast<uint4 *>(smem + SL.res)[i] = reinterpret_cast<const uint4 *>(p.resimg + (size_t)rank * p.res_bytes)[i];
@@ -144,7 +184,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
     const long long q_lo = npairs * cl / ncl, q_hi = npairs * (cl + 1) / ncl;
     const long long ntl = q_hi - q_lo;
 
-    if (warp == 0) {
+    if (warp == W_PROD) {
         // =========================== weight producers (TMA engine, 1-D bulk copies), both CTAs ===========================
         // Fill q always lands in slot q % nslots.  Never more lanes than slots: a lane two uses of a slot ahead of the
         // consumer would pass its parity wait on an older phase and overwrite live data.
@@ -162,7 +202,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                 slot += nprod; while (slot >= (uint32_t)p.nslots) { slot -= (uint32_t)p.nslots; par ^= 1u; }
             }
         }
-    } else if (warp == 1 && rank != 0) {
+    } else if (warp == W_ISSUE && rank != 0) {
         // =========================== peer CTA: ring forwarder ===========================
         // The leader's MMAs read this CTA's half of every ring slot; a bulk copy can only signal a barrier of its own
         // CTA, so one thread waits for each local fill and arrives on the leader's WFULL barrier of the same slot.
@@ -176,12 +216,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             }
         }
         __syncwarp();
-    } else if (warp == 1) {
+    } else if (warp == W_ISSUE) {
         // =========================== leader CTA: MMA issuer, ONE elected thread ===========================
-        // Ops of a tile (p.optype / p.opchunk) are issued in order, op k into accumulator k % nacc; the consumer of an
-        // in-place op (P2 / W3 MMAs reading the fp16 chunk the epilogue wrote over the accumulator) is issued nacc - 1
-        // ops later, i.e. just before the accumulator's next producer — the tensor pipe executes in issue order, so
-        // MMA-after-MMA hazards need no barrier; only epilogue <-> MMA hand-overs do (FULL / EDONE).
+        // Ops of a tile are issued in the fixed order of Sched; the consumer of an in-place op (P2 / W3 MMAs reading the
+        // fp16 chunk the epilogue wrote over the accumulator) is issued LAG ops later — the tensor pipe executes in
+        // issue order, so MMA-after-MMA hazards need no barrier; only epilogue <-> MMA hand-overs do (FULL / EDONE).
+        // Every EDONE phase is waited exactly once, at a position fixed on the host (p.prewait) or at the consumer, so
+        // barrier parities are plain bits of `ph`.
         if (elect_one()) {
             const uint32_t a1_lo = (smem_base + SL.a1) >> 4, res_lo = (smem_base + SL.res) >> 4;
             const uint32_t slots_lo = (smem_base + SL.slots) >> 4, slot_step = p.slot_bytes >> 4;
@@ -189,37 +230,38 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             const uint32_t lo_noswz = (128u >> 4) << 16, hi_noswz = (((uint32_t)(KI / 8) * 128u) >> 4) | (1u << 14);
             const uint32_t lo_sw128 = (16u >> 4) << 16, hi_sw128 = (1024u >> 4) | (1u << 14) | (2u << 29);
             const uint32_t id128 = idesc_f16(256, CN), id16 = idesc_f16(256, 16), id0 = idesc_f16(256, 0);
-            const uint32_t nslots = (uint32_t)p.nslots, lag = nacc - 1;
+            const uint32_t nslots = (uint32_t)p.nslots;
             const uint32_t tm_d3 = tmem + p.tm_d3, tm_ph = tm_d3 + (uint32_t)KO - 16, tm_a0 = tmem + p.tm_a0;
             uint32_t slot = 0, wpar = 0, slot_lo = slots_lo;
-            uint32_t acc = 0, use = 0;                   // accumulator / use count of the next op
-            uint32_t d0 = 0, d1 = 0, d2 = 0;             // EDONE phases consumed per accumulator
-#define SPIN_CL(id, par) do { mbar_spin_cl(BAR_ADDR(id), (par)); tc_fence_after(); } while (0)
-#define ENSURE1(dx, idx, u) do { while (dx <= (u)) { mbar_spin_cl(BAR_ADDR(BAR_EDONE + idx), dx & 1u); ++dx; } } while (0)
-            // op on accumulator a with use count u has been through its chunk epilogue
-#define ENSURE(a, u) do { if ((a) == 0) ENSURE1(d0, 0, u); else if ((a) == 1) ENSURE1(d1, 1, u); else ENSURE1(d2, 2, u); tc_fence_after(); } while (0)
-#define SLOT_ACQUIRE(w) do { if ((w) & SUB_NEW) { mbar_spin_cl(BAR_ADDR(BAR_WFULL + slot), wpar); tc_fence_after(); } } while (0)
+            uint32_t ph = 0;                             // parity of the next phase to wait for, one bit per barrier id
+#ifdef TC2_PROF
+            long long pw_wait = 0, pw_wf = 0, pw_tot = clock64();
+#endif
+#define WAIT(id) do { PROF_T0(); mbar_spin_cl(BAR_ADDR(id), (ph >> (id)) & 1u); ph ^= 1u << (id); tc_fence_after(); PROF_ADD(pw_wait); } while (0)
+#define SLOT_ACQUIRE(w) do { if ((w) & SUB_NEW) { PROF_T0(); mbar_spin_cl(BAR_ADDR(BAR_WFULL + slot), wpar); tc_fence_after(); PROF_ADD(pw_wf); } } while (0)
 #define SLOT_RELEASE(w) do { if ((w) & SUB_END) { mma_commit_cg2(BAR_ADDR(BAR_WEMPTY + slot)); slot_lo += slot_step; \
                              if (++slot == nslots) { slot = 0; wpar ^= 1u; slot_lo = slots_lo; } } } while (0)
             for (long long ti = 0; ti < ntl; ++ti) {
-                uint32_t si = 0, a1_ready = 0;
-                bool d3_open = false;
-                const uint32_t acc0 = acc, use0 = use;
-                SPIN_CL(BAR_A0FULL, (uint32_t)ti & 1u);
-                // consumer of tile-local op jc whose accumulator / use count are (ca, cu)
-                auto consume = [&](uint32_t jc, uint32_t ca, uint32_t cu) {
-                    const uint32_t type = p.optype[jc];
+                // (the table index goes through an opaque asm so that the compiler cannot prove the table words loop-invariant
+                // and unswitch the tile loop on them: that multiplied the issuer's code size by ten)
+                uint32_t si = 0;
+                asm volatile("" : "+r"(si));
+                uint32_t w = p.sub[si];                      // current table word; the next one is always loaded one step ahead
+                WAIT(BAR_A0FULL);
+                // consumer of tile-local op jc (jc is a compile-time constant after unrolling)
+                auto consume = [&](const int jc) {
+                    const int type = S::type(jc);
                     if (type == T_L1S) return;
-                    ENSURE(ca, cu);
-                    if (!d3_open) { SPIN_CL(BAR_D3EMPTY, (uint32_t)ti & 1u); d3_open = true; }     // first write into D3 of this tile
-                    const uint32_t a_t = tmem + ca * CN;
+                    WAIT(BAR_EDONE + jc % NACC);
+                    if (jc == S::FIRST_INPLACE) WAIT(BAR_D3EMPTY);              // first write into D3 of this tile
+                    const uint32_t a_t = tmem + (uint32_t)(jc % NACC) * CN;
                     if (type == T_P) {                                          // resident P2 tile of this chunk, N = 16
-                        const uint32_t b_lo = (res_lo + (uint32_t)p.opchunk[jc] * (2048u >> 4)) | lo_sw128;
+                        const uint32_t b_lo = (res_lo + (uint32_t)S::chunk(jc) * (2048u >> 4)) | lo_sw128;
 #pragma unroll
                         for (uint32_t ks = 0; ks < 8; ++ks)
                             mma_ts_cg2(tm_ph, a_t + 8 * ks, b_lo + (ks >> 2) * (1024u >> 4) + 2 * (ks & 3), hi_sw128, id16, 1u);
                     } else {                                                    // streamed layer-3 tile
-                        const uint32_t w = p.sub[si++];
+                        const uint32_t wn = p.sub[++si];
                         SLOT_ACQUIRE(w);
                         const uint32_t nlo = ((w >> SUB_AUX_SHIFT) & 0xFFu) * 16;      // output rows below n_lo receive exactly 0
                         const uint32_t N = (uint32_t)KO - nlo, kb_step = (N >> 1) * (128u >> 4);
@@ -228,28 +270,25 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                         for (uint32_t ks = 0; ks < 8; ++ks)
                             mma_ts_cg2(tm_d3 + nlo, a_t + 8 * ks, b_lo + (ks >> 2) * kb_step + 2 * (ks & 3), hi_sw128, idesc, 1u);
                         SLOT_RELEASE(w);
+                        w = wn;
                     }
                 };
-#pragma unroll 1
-                for (uint32_t j = 0; j < nops; ++j) {
-                    const uint32_t type = p.optype[j], c = p.opchunk[j];
-                    if (use > 0) ENSURE(acc, use - 1);                          // the accumulator's previous op is through its epilogue
-                    const uint32_t d = tmem + acc * CN;
+#pragma unroll
+                for (int j = 0; j < S::NOPS; ++j) {
+                    const int type = S::type(j), c = S::chunk(j), acc = j % NACC;
+                    uint32_t jj = (uint32_t)j;
+                    asm volatile("" : "+r"(jj));
+                    const uint32_t pw = p.prewait[jj];      // pending chunk epilogues this op depends on (accumulator reuse, A1 chunks)
+                    if (pw & 1u) WAIT(BAR_EDONE + 0);
+                    if (NACC > 1 && (pw & 2u)) WAIT(BAR_EDONE + 1);
+                    if (NACC > 2 && (pw & 4u)) WAIT(BAR_EDONE + 2);
+                    const uint32_t d = tmem + (uint32_t)acc * CN;
                     if (type == T_L2) {
-                        // A1 chunks 0 .. l2need[c] written (layer-1 ops are the first NC ops of the tile)
-                        const uint32_t need = p.l2need[c];
-                        while (a1_ready <= need) {
-                            uint32_t a = acc0 + a1_ready, u = use0;
-                            if (a >= nacc) { a -= nacc; ++u; }
-                            if (a >= nacc) { a -= nacc; ++u; }
-                            ENSURE(a, u);
-                            ++a1_ready;
-                        }
-                        const uint32_t nb = p.nblk[c];
+                        const uint32_t nb = p.nblk[jj - (uint32_t)(j - c)];
                         uint32_t accum = 0;
 #pragma unroll 1
                         for (uint32_t b = 0; b < nb; ++b) {
-                            const uint32_t w = p.sub[si++];
+                            const uint32_t wn = p.sub[++si];
                             SLOT_ACQUIRE(w);
                             const uint32_t aux = (w >> SUB_AUX_SHIFT) & 0xFFu, kmask = aux >> 4;
                             const uint32_t a_lo = (a1_lo + (aux & 7u) * (16384u >> 4)) | lo_sw128;
@@ -266,57 +305,57 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                                     if ((kmask >> ks) & 1u) { mma_ss_cg2(d, a_lo + 2 * ks, hi_sw128, b_lo + 2 * ks, hi_sw128, id128, accum); accum = 1u; }
                             }
                             SLOT_RELEASE(w);
+                            w = wn;
                         }
                     } else {
                         // input layers (layer 1 / phase hidden): A = A0 in TMEM, B = this chunk's rows, K-step prefix
-                        const uint32_t w = p.sub[si++];
+                        const uint32_t wn = p.sub[++si];
                         SLOT_ACQUIRE(w);
                         const uint32_t nk = (w >> SUB_AUX_SHIFT) & 0xFFu;
                         const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_noswz;
                         mma_ts_cg2(d, tm_a0, b_lo, hi_noswz, id128, 0u);
-#pragma unroll 1
-                        for (uint32_t ks = 1; ks < nk; ++ks) mma_ts_cg2(d, tm_a0 + 8 * ks, b_lo + 16 * ks, hi_noswz, id128, 1u);
+                        // nested so that the common exit is one taken branch (KI <= 128 -> at most 8 K-steps)
+#define KSTEP(k) mma_ts_cg2(d, tm_a0 + 8u * (k), b_lo + 16u * (k), hi_noswz, id128, 1u)
+                        if (nk > 1) { KSTEP(1); if (nk > 2) { KSTEP(2); if (nk > 3) { KSTEP(3); if (nk > 4) { KSTEP(4);
+                        if (nk > 5) { KSTEP(5); if (nk > 6) { KSTEP(6); if (nk > 7) { KSTEP(7); } } } } } } }
+#undef KSTEP
                         SLOT_RELEASE(w);
+                        w = wn;
                     }
                     mma_commit_cg2(BAR_ADDR(BAR_FULL + acc));
-                    if ((int)j == p.last_a0_op) mma_commit_cg2(BAR_ADDR(BAR_A0FREE));     // A0 may be rebuilt for the next tile
-                    if ((int)j == p.last_l2_op) mma_commit_cg2(BAR_ADDR(BAR_A1FREE));     // A1 may be rewritten by the next tile
-                    if (j >= lag) {                                                       // consumer of op j - lag
-                        const uint32_t ca = acc >= lag ? acc - lag : acc + nacc - lag, cu = acc >= lag ? use : use - 1;
-                        consume(j - lag, ca, cu);
-                    }
-                    if (++acc == nacc) { acc = 0; ++use; }
+                    if (j == S::LAST_A0) mma_commit_cg2(BAR_ADDR(BAR_A0FREE));                 // A0 may be rebuilt for the next tile
+                    if (L == 2 && j == S::NOPS - 1) mma_commit_cg2(BAR_ADDR(BAR_A1FREE));      // A1 may be rewritten by the next tile
+                    if (j >= S::LAG) consume(j - S::LAG);
                 }
-                for (uint32_t m = lag; m >= 1; --m) {                                     // consumers of the last ops
-                    if (nops < m) continue;
-                    const uint32_t ca = acc >= m ? acc - m : acc + nacc - m, cu = acc >= m ? use : use - 1;
-                    consume(nops - m, ca, cu);
-                }
+#pragma unroll
+                for (int m = S::LAG; m >= 1; --m) consume(S::NOPS - m);                       // consumers of the last ops
                 mma_commit_cg2(BAR_ADDR(BAR_D3FULL));
             }
-#undef SPIN_CL
-#undef ENSURE1
-#undef ENSURE
+#ifdef TC2_PROF
+            if (p.prof) { long long *pr = p.prof + (size_t)blockIdx.x * 32; pr[0] = clock64() - pw_tot; pr[1] = pw_wait; pr[3] = pw_wf; pr[5] = ntl; }
+#endif
+#undef WAIT
 #undef SLOT_ACQUIRE
 #undef SLOT_RELEASE
         }
         __syncwarp();
-    } else if (warp < 10) {
+    } else if (warp >= W_EPI) {
         // =========================== chunk epilogue groups: ops alternate between the two groups ===========================
-        const uint32_t grp = (uint32_t)(warp - 2) >> 2;
+        const uint32_t grp = (uint32_t)(warp - W_EPI) >> 2;
         const uint32_t row = (uint32_t)((warp & 3) * 32 + lane);
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;     // TMEM lane quadrant of this warp
         const uint32_t a1_row = smem_base + SL.a1 + (row >> 3) * 1024u + (row & 7u) * 128u, sw = row & 7u;
-        const long long total_ops = ntl * (long long)nops;
-        uint32_t acc = grp, use = 0, j = grp;
-        long long ti = 0, seen_ti = 0;
-        for (long long k = grp; k < total_ops; k += 2) {
+        uint32_t fb = 0;                                   // bit a: parity of accumulator a's first FULL phase of this tile
+        long long pe_wait = 0, pe_a1 = 0, pe_tot = clock64(), pe_fence = 0, pe_arr = 0;
+        (void)pe_wait; (void)pe_a1; (void)pe_tot; (void)pe_fence; (void)pe_arr;
+        for (long long ti = 0; ti < ntl; ++ti, fb ^= p.cntmask)
+        for (uint32_t j = grp; j < nops; j += 2) {
             const uint32_t type = p.optype[j], c = p.opchunk[j];
-            mbar_wait(&bars[BAR_FULL + acc], use & 1u);
+            const uint32_t q = (NACC == 2) ? (j >> 1) : ((NACC == 3) ? ((j * 11u) >> 5) : j), acc = j - q * NACC;   // j / NACC, j % NACC (j < 32)
+            { PROF_T0(); mbar_wait(&bars[BAR_FULL + acc], ((fb >> acc) ^ q) & 1u); PROF_ADD(pe_wait); }
             tc_fence_after();
-            if (p.L == 2 && seen_ti != ti) {               // once per tile: the previous tile's layer-2 MMAs have read A1
-                mbar_wait(&bars[BAR_A1FREE], (uint32_t)(ti - 1) & 1u);
-                seen_ti = ti;
+            if (L == 2 && ti > 0 && j == grp) {            // once per tile: the previous tile's layer-2 MMAs have read A1
+                PROF_T0(); mbar_wait(&bars[BAR_A1FREE], (uint32_t)(ti - 1) & 1u); PROF_ADD(pe_a1);
             }
             const uint32_t d_addr = tmem + lane_base + acc * CN;
             const float *bias = s_bias + (type == T_P ? 0 : (type == T_L2 ? 2 * H : H)) + c * CN;
@@ -347,13 +386,17 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                     tmem_st16p(d_addr + 16 * pc, w);          // in place: columns [16 pc, 16 pc + 16) were read by piece pc / 2 <= pc
                 }
             }
+            { PROF_T0();
             if (type == T_L1S) fence_proxy_async(); else tmem_wait_st();
             tc_fence_before();
-            __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(BAR_ADDR(BAR_EDONE + acc), 0);
-            acc += 2; while (acc >= nacc) { acc -= nacc; ++use; }
-            j += 2; if (j >= nops) { j -= nops; ++ti; }
+            __syncwarp(); PROF_ADD(pe_fence); }
+            { PROF_T0();
+            if (lane == 0) mbar_arrive_leader(BAR_ADDR(BAR_EDONE + acc), rank);
+            __syncwarp(); PROF_ADD(pe_arr); }
         }
+#ifdef TC2_PROF
+        if (p.prof && lane == 0 && (warp == W_EPI || warp == W_EPI + 4)) { long long *pr = p.prof + (size_t)blockIdx.x * 32 + (warp == W_EPI ? 6 : 11); pr[0] = clock64() - pe_tot; pr[1] = pe_wait; pr[2] = pe_a1; pr[3] = pe_fence; pr[4] = pe_arr; }
+#endif
     } else {
         // =========================== tile warps: A0 of the next tile, contraction, final epilogue ===========================
         const int q = warp & 3;
@@ -385,7 +428,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             tmem_wait_st();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(BAR_ADDR(BAR_A0FULL), 0);
+            if (lane == 0) mbar_arrive_leader(BAR_ADDR(BAR_A0FULL), rank);
         };
         auto flip_of = [&](long long t, bool valid) -> ulonglong2 {
             if (p.mode != 1 || !valid) return make_ulonglong2(0, 0);
@@ -397,12 +440,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
         tmem_wait_st();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive_cluster(BAR_ADDR(BAR_D3EMPTY), 0);
+        if (lane == 0) mbar_arrive_leader(BAR_ADDR(BAR_D3EMPTY), rank);
 
         RowState cur{}, nxt{};
         ulonglong2 zp = make_ulonglong2(0, 0), zp_n = zp;
         float2 E = make_float2(0.f, 0.f);
         float mr = (p.mode == 1 && p.hm.has_diag) ? 1.0f : 0.0f;     // the f = 0 group has ratio exactly 1
+        long long pt_a0 = 0, pt_d3 = 0, pt_tot = clock64(), pt_s = 0, pt_fin = 0;
+        (void)pt_a0; (void)pt_d3; (void)pt_tot; (void)pt_s; (void)pt_fin;
         if (ntl > 0) {
             const long long t = 2 * q_lo + rank;
             const bool valid = t < ntiles;
@@ -426,6 +471,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             }
             // ---- (a3) S = sum_{t in g} c_t (-i)^{r_t} (-1)^{popcount(x & s_t)}: independent of the MMAs, done while they run ----
             float2 S = make_float2(0.f, 0.f);
+#ifdef TC2_PROF
+            const long long _ts = clock64();
+#endif
             if (p.mode == 1 && valid && cur.i < p.B) {
                 const uint32_t t1 = __ldg(&p.hm.offsets[g + 1]);
                 for (uint32_t tt = __ldg(&p.hm.offsets[g]); tt < t1; ++tt) {
@@ -436,15 +484,21 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                     S.y += neg ? -c.y : c.y;
                 }
             }
+#ifdef TC2_PROF
+            pt_s += (long long)__float_as_int(S.x) * 0 + clock64() - _ts;
+#endif
             // ---- operand tile of the NEXT tile, once the last MMA that reads the current one has completed ----
             if (has_next) {
-                mbar_wait(&bars[BAR_A0FREE], (uint32_t)ti & 1u);
+                { PROF_T0(); mbar_wait(&bars[BAR_A0FREE], (uint32_t)ti & 1u); PROF_ADD(pt_a0); }
                 tc_fence_after();
                 build_a0(zp_n);
             }
             // ---- final epilogue: log|psi| = 1/2 sum_d log sigmoid(+-a_d), phi = o[2 z_{n-2} + z_{n-1}] ----
-            mbar_wait(&bars[BAR_D3FULL], (uint32_t)ti & 1u);
+            { PROF_T0(); mbar_wait(&bars[BAR_D3FULL], (uint32_t)ti & 1u); PROF_ADD(pt_d3); }
             tc_fence_after();
+#ifdef TC2_PROF
+            const long long _tf = clock64();
+#endif
             // sum_d log sigmoid(t_d) = sum_d min(t_d, 0) - ln prod_d (1 + exp(-|t_d|)): every factor is in (1, 2], so a
             // 16-term product cannot overflow and costs one LG2 per 16 conditionals; the 16 chains are independent (ILP).
             float msum = 0.0f, lg = 0.0f, phi = 0.0f;
@@ -485,7 +539,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             tmem_wait_st();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive_cluster(BAR_ADDR(BAR_D3EMPTY), 0);
+            if (lane == 0) mbar_arrive_leader(BAR_ADDR(BAR_D3EMPTY), rank);
             const float lp = 0.5f * part;
             if (p.mode == 0) {
                 if (cur.i < p.B) p.out[cur.i] = make_float2(lp, phi);
@@ -506,14 +560,20 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                 }
                 E = make_float2(0.f, 0.f);
             }
+#ifdef TC2_PROF
+            pt_fin += clock64() - _tf;
+#endif
             cur = nxt; zp = zp_n;
         }
         if (p.mode == 1) atomicMax(p.max_ratio_bits, __float_as_uint(mr));
+#ifdef TC2_PROF
+        if (p.prof && lane == 0 && warp == W_TILE) { long long *pr = p.prof + (size_t)blockIdx.x * 32 + 16; pr[0] = clock64() - pt_tot; pr[1] = pt_a0; pr[2] = pt_d3; pr[3] = pt_s; pr[4] = pt_fin; }
+#endif
     }
 #undef BAR_ADDR
     tc_fence_before();
     cluster_sync_all();
-    if (warp == 1) tmem_dealloc_cg2(tmem, 512);
+    if (warp == W_ISSUE) tmem_dealloc_cg2(tmem, 512);
 }
 
 // position-ordered copy of 128-bit configurations: out bit d = in bit order[d]
@@ -561,7 +621,8 @@ struct Tc2Pack {
     void *d_xpos = nullptr; size_t xpos_cap = 0;
     SmemLayout L{};
     uint32_t sub[MAX_SUB + 1] = {0};
-    uint8_t nblk[MAX_NC] = {0}, l2need[MAX_NC] = {0}, optype[MAX_OPS] = {0}, opchunk[MAX_OPS] = {0};
+    uint8_t nblk[MAX_NC] = {0}, l2need[MAX_NC] = {0}, optype[MAX_OPS] = {0}, opchunk[MAX_OPS] = {0}, prewait[MAX_OPS] = {0};
+    uint32_t cntmask = 0;
     int sms = 148;
     long long mma_issued = 0, mma_dense = 0;                   // 16-wide K-steps x N issued / of the dense chain, per tile (MACs / 2048)
 };
@@ -591,6 +652,10 @@ static bool tc2_shape(const nqs_made *M, Tc2Shape *out) {
     uint32_t slot = (ring / ns) / 1024 * 1024;
     if (slot < need) return false;
     if (slot > 0x1FFFu * 16u) slot = 0x1FFFu * 16u / 1024 * 1024;
+#ifdef TC2_PROF
+    if (const char *e = getenv("NQS_TC2_SLOT_KB")) { slot = (uint32_t)atoi(e) * 1024; }
+    if (const char *e = getenv("NQS_TC2_NSLOTS")) { ns = atoi(e); }
+#endif
     s.slot = slot; s.nslots = ns;
     *out = s;
     return true;
@@ -744,6 +809,31 @@ int tc2_pack_upload(const nqs_made *M) {
     for (int j = 0; j < nops; ++j) { emit_op(j); if (j >= lag) emit_consumer(j - lag); }
     for (int m = lag; m >= 1; --m) if (nops >= m) emit_consumer(nops - m);
     close_fill();
+    // ---- where the issuer waits for chunk epilogues that have no consumer MMA (layer-1 chunks written to A1): before
+    // the accumulator's next producer or the first layer-2 op that reads the chunk, whichever is issued first ----
+    if (L == 2) P->l2need[NC - 1] = (uint8_t)(NC - 1);          // every layer-1 epilogue is waited for inside its own tile
+    {
+        int pending[3] = {-1, -1, -1};
+        auto consumed = [&](int j) { if (P->optype[j] != T_L1S && pending[j % sh.nacc] == j) pending[j % sh.nacc] = -1; };
+        for (int j = 0; j < nops; ++j) {
+            const int a = j % sh.nacc;
+            uint8_t pw = 0;
+            if (pending[a] >= 0) { pw |= (uint8_t)(1u << a); pending[a] = -1; }
+            if (P->optype[j] == T_L2)
+                for (int cn = 0; cn <= P->l2need[P->opchunk[j]]; ++cn)
+                    if (pending[cn % sh.nacc] == cn) { pw |= (uint8_t)(1u << (cn % sh.nacc)); pending[cn % sh.nacc] = -1; }
+            P->prewait[j] = pw;
+            pending[a] = j;
+            if (j >= lag) consumed(j - lag);
+        }
+        for (int m = lag; m >= 1; --m) if (nops >= m) consumed(nops - m);
+        if (pending[0] >= 0 || pending[1] >= 0 || pending[2] >= 0) { delete P; return NQS_EUNSUPPORTED; }
+        for (int a = 0; a < sh.nacc; ++a) {
+            int cnt = 0;
+            for (int j = a; j < nops; j += sh.nacc) ++cnt;
+            if (cnt & 1) P->cntmask |= 1u << a;
+        }
+    }
     P->nsub = (int)sub.size(); P->nfills = (int)fills.size();
     P->res_bytes = (uint32_t)res[0].size();
     if (P->nsub > MAX_SUB) { delete P; return NQS_EUNSUPPORTED; }
@@ -802,6 +892,7 @@ static void fill_common(const nqs_made *M, Tc2Params &p) {
     p.fills = (const uint2 *)P->d_fills; p.nfills = P->nfills;
     memcpy(p.sub, P->sub, sizeof(p.sub)); memcpy(p.nblk, P->nblk, sizeof(p.nblk)); memcpy(p.l2need, P->l2need, sizeof(p.l2need));
     memcpy(p.optype, P->optype, sizeof(p.optype)); memcpy(p.opchunk, P->opchunk, sizeof(p.opchunk));
+    memcpy(p.prewait, P->prewait, sizeof(p.prewait)); p.cntmask = P->cntmask;
     p.resimg = (const uint8_t *)P->d_res; p.res_bytes = P->res_bytes;
     p.slot_bytes = P->slot_bytes; p.nslots = P->nslots;
     p.bias = (const float *)P->d_bias;
@@ -822,16 +913,40 @@ static int permuted(const nqs_made *M, const ulonglong2 *in, long long N, ulongl
     return cudaGetLastError() == cudaSuccess ? NQS_OK : NQS_ECUDA;
 }
 
-static int launch_chain(const Tc2Pack *P, const Tc2Params &p, long long ntiles, cudaStream_t st) {
+#ifdef TC2_PROF
+long long *g_tc2_prof = nullptr;   // [148][16], set by the profiling harness through nqs_tc2_prof_buffer()
+extern "C" void nqs_tc2_prof_buffer(long long *dev_buf) { g_tc2_prof = dev_buf; }
+#endif
+
+template <int NC, int L, int NACC>
+static int launch_inst(const Tc2Params &p, int grid, uint32_t smem_bytes, cudaStream_t st) {
     // the attribute is per device and per kernel; setting it is a cheap host call, so no process-wide cache
-    if (cudaFuncSetAttribute(eloc_tc2_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->L.total) != cudaSuccess) {
+    if (cudaFuncSetAttribute(eloc_tc2_kernel<NC, L, NACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes) != cudaSuccess) {
         cudaGetLastError();
         return NQS_ECUDA;
     }
+    eloc_tc2_kernel<NC, L, NACC><<<grid, NTHREADS, smem_bytes, st>>>(p);
+    return NQS_OK;
+}
+
+static int launch_chain(const Tc2Pack *P, Tc2Params &p, long long ntiles, cudaStream_t st) {
+#ifdef TC2_PROF
+    p.prof = g_tc2_prof;
+#endif
     const long long npairs = (ntiles + 1) / 2;
     const long long ncl_max = P->sms / 2;
     const int grid = 2 * (int)(npairs < ncl_max ? npairs : ncl_max);
-    eloc_tc2_kernel<<<grid, NTHREADS, P->L.total, st>>>(p);
+    int rc = NQS_EUNSUPPORTED;
+#define TC2_CASE(NC_, L_, NA_) case (NC_ * 16 + L_ * 4 + NA_): rc = launch_inst<NC_, L_, NA_>(p, grid, P->L.total, st); break;
+    switch (p.NC * 16 + p.L * 4 + p.nacc) {
+        TC2_CASE(1, 1, 2) TC2_CASE(2, 1, 2) TC2_CASE(3, 1, 2) TC2_CASE(4, 1, 2)
+        TC2_CASE(1, 2, 2) TC2_CASE(2, 2, 2) TC2_CASE(3, 2, 2) TC2_CASE(4, 2, 2)
+        TC2_CASE(1, 1, 3) TC2_CASE(2, 1, 3) TC2_CASE(3, 1, 3) TC2_CASE(4, 1, 3)
+        TC2_CASE(1, 2, 3) TC2_CASE(2, 2, 3) TC2_CASE(3, 2, 3) TC2_CASE(4, 2, 3)
+        default: break;
+    }
+#undef TC2_CASE
+    if (rc) return rc;
     ++g_launch_count;
     return cudaGetLastError() == cudaSuccess ? NQS_OK : NQS_ECUDA;
 }

@@ -269,21 +269,40 @@ __device__ __forceinline__ void tmem_alloc_cg2(uint32_t *dst_smem, uint32_t ncol
 __device__ __forceinline__ void tmem_dealloc_cg2(uint32_t addr, uint32_t ncols) {
     asm volatile("tcgen05.dealloc.cta_group::2.sync.aligned.b32 %0, %1;\n" ::"r"(addr), "r"(ncols) : "memory");
 }
-// remote (or local) arrive on the barrier at the same offset in CTA `cta` of the cluster
+// arrive on the barrier at the same offset in CTA `cta` of the cluster.  Default (.release.cta) semantics on purpose: a
+// cluster-scope release costs ~800 cycles per arrive (measured), and what the waiter consumes is ordered by
+// tcgen05.fence / fence.proxy.async executed before the arrive, not by the arrive itself.
 __device__ __forceinline__ void mbar_arrive_cluster(uint32_t bar_addr, uint32_t cta) {
     asm volatile("{\n\t.reg .b32 ra;\n\tmapa.shared::cluster.u32 ra, %0, %1;\n\t"
-                 "mbarrier.arrive.release.cluster.shared::cluster.b64 _, [ra];\n\t}\n" ::"r"(bar_addr), "r"(cta) : "memory");
+                 "mbarrier.arrive.shared::cluster.b64 _, [ra];\n\t}\n" ::"r"(bar_addr), "r"(cta) : "memory");
 }
-// cluster-scope acquire poll (the barrier receives arrivals from the peer CTA)
+__device__ __forceinline__ void mbar_arrive_addr(uint32_t bar_addr) {
+    asm volatile("mbarrier.arrive.shared::cta.b64 _, [%0];\n" ::"r"(bar_addr) : "memory");
+}
+// arrive on the LEADER's copy of a barrier: local in the leader CTA, remote from the peer
+__device__ __forceinline__ void mbar_arrive_leader(uint32_t bar_addr, uint32_t my_rank) {
+    if (my_rank == 0) mbar_arrive_addr(bar_addr); else mbar_arrive_cluster(bar_addr, 0);
+}
+// poll of a barrier that also receives arrivals from the peer CTA (default acquire.cta, as for the arrives above)
 __device__ __forceinline__ bool mbar_try_wait_cl(uint32_t bar, uint32_t parity) {
     uint32_t ok;
-    asm volatile("{\n\t.reg .pred P;\n\tmbarrier.try_wait.parity.acquire.cluster.shared::cta.b64 P, [%1], %2;\n\tselp.u32 %0, 1, 0, P;\n\t}\n"
+    asm volatile("{\n\t.reg .pred P;\n\tmbarrier.try_wait.parity.shared::cta.b64 P, [%1], %2;\n\tselp.u32 %0, 1, 0, P;\n\t}\n"
                  : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
     return ok != 0;
 }
-__device__ __forceinline__ void mbar_spin_cl(uint32_t bar, uint32_t parity) {
+__device__ __forceinline__ uint32_t mbar_spin_cl(uint32_t bar, uint32_t parity) {    // returns the number of failed polls
     uint32_t spins = 0;
+#ifdef TC2_PROF
+    {   // non-blocking probe first, so that the instrumented build can tell a real stall from the cost of the poll
+        uint32_t ok;
+        asm volatile("{\n\t.reg .pred P;\n\tmbarrier.test_wait.parity.shared::cta.b64 P, [%1], %2;\n\tselp.u32 %0, 1, 0, P;\n\t}\n"
+                     : "=r"(ok) : "r"(bar), "r"(parity) : "memory");
+        if (ok) return 0;
+        spins = 1;
+    }
+#endif
     while (!mbar_try_wait_cl(bar, parity)) { if (++spins == (1u << 26)) __trap(); }
+    return spins;
 }
 __device__ __forceinline__ void mma_commit_cg2(uint32_t bar) {                       // arrives in BOTH CTAs
     asm volatile("tcgen05.commit.cta_group::2.mbarrier::arrive::one.shared::cluster.multicast::cluster.b64 [%0], %1;\n"
