@@ -45,16 +45,23 @@ enum nqs_status {
     NQS_ENOMEM       = -3,   /* host or device allocation failed                                                 */
     NQS_ECUDA        = -4,   /* a CUDA runtime call or kernel launch failed (no device, ...)                      */
     NQS_EARCH        = -5,   /* device is not compute capability 10.x (the kernels are sm_100a only)             */
-    NQS_EUNSUPPORTED = -6    /* the requested path cannot run this shape (e.g. NQS_PATH_TC on hidden % 64 != 0)   */
+    NQS_EUNSUPPORTED = -6    /* the requested path cannot run this shape (e.g. NQS_PATH_TC on hidden % 128 != 0)  */
 };
 
 /* Which kernels evaluate the MADE chain.  Both are CUDA; neither touches the CPU.
  *  NQS_PATH_SIMT : fp32 FFMA on CUDA cores, every layer (reference-quality, any shape).
- *  NQS_PATH_TC   : tcgen05 tensor cores, fp16 operands / fp32 accumulation in TMEM, fused gather of
- *                  x xor f into the operand tile and log|psi| / phase / ratio / E_loc in the epilogue.
- *                  Needs n_hidden_layers == 2, hidden a multiple of 64 in [64, 512], n_qubits <= 112.
+ *  NQS_PATH_TC   : tcgen05 tensor cores driven by CTA pairs (cta_group::2), fp16 operands / fp32 accumulation in
+ *                  TMEM, fused gather of x xor f into the operand tile and log|psi| / phase / ratio / E_loc in the
+ *                  epilogue.  Needs n_hidden_layers in {1, 2} and hidden a multiple of 128 in [128, 512]; every
+ *                  n_qubits in [3, 128] fits (two 128-column accumulators + round16(n+4) output columns +
+ *                  round16(n)/2 input columns <= 512 TMEM columns; three accumulators when n <= 76).  Other shapes
+ *                  return NQS_EUNSUPPORTED.
  *  NQS_PATH_AUTO : TC when the shape supports it and hidden >= 384 (where single-pass fp16 operands keep
- *                  |dE_loc| several times below 1e-5 sum|c|), else SIMT. */
+ *                  |dE_loc| several times below 1e-5 sum|c| on the chemistry workloads),
+ *                  else SIMT.
+ * A handle (nqs_made_t / nqs_ham_t) owns device scratch that its compute calls reuse: use one handle from one
+ * host thread and one CUDA stream at a time, on the device that was current when it was first used (other
+ * devices: NQS_EINVAL). */
 enum nqs_path { NQS_PATH_AUTO = 0, NQS_PATH_SIMT = 1, NQS_PATH_TC = 2 };
 
 /* ---- (a1) Hamiltonian compile: Fig. 1 (:101) -------------------------------------

@@ -10,7 +10,6 @@ _HERE = os.path.dirname(os.path.abspath(__file__))
 LIB_PATH = os.path.join(_HERE, "csrc", "libnqs.so")
 
 PATH_AUTO, PATH_SIMT, PATH_TC = 0, 1, 2
-PATH_TC2 = 3   # development hook: the CTA-pair kernel while it is being brought up
 _lib = None
 
 c_void_p, c_int, c_int64 = ctypes.c_void_p, ctypes.c_int, ctypes.c_int64

@@ -23,8 +23,14 @@ static int upload(const T *src, size_t count, void **dst) {
     return NQS_OK;
 }
 
+static int same_device(int recorded) {
+    int dev = -1;
+    if (cudaGetDevice(&dev) != cudaSuccess) { cudaGetLastError(); return NQS_ECUDA; }
+    return dev == recorded ? NQS_OK : NQS_EINVAL;
+}
+
 int nqs_ham_upload(const nqs_ham *H) {
-    if (H->on_device) return NQS_OK;
+    if (H->on_device) return same_device(H->device);
     int rc = nqs_check_device();
     if (rc) return rc;
     cudaGetDevice(&H->device);
@@ -63,7 +69,7 @@ extern "C" void nqs_ham_free(nqs_ham_t *H) {
 }
 
 int nqs_made_upload(const nqs_made *M) {
-    if (M->on_device) return NQS_OK;
+    if (M->on_device) return same_device(M->device);
     int rc = nqs_check_device();
     if (rc) return rc;
     cudaGetDevice(&M->device);
@@ -110,7 +116,6 @@ int nqs_made_upload(const nqs_made *M) {
     if ((rc = up(M->c1, &d.c1))) return rc;
     if ((rc = up(M->c2, &d.c2))) return rc;
     if (tc_supported(M) && (rc = tc_pack_upload(M))) return rc;
-    if (tc2_supported(M) && (rc = tc2_pack_upload(M))) return rc;
     M->on_device = true;
     return NQS_OK;
 }
@@ -129,15 +134,12 @@ extern "C" void nqs_made_free(nqs_made_t *M) {
     if (M->ws) cudaFree(M->ws);
     for (cudaEvent_t e : M->ev) cudaEventDestroy(e);
     tc_pack_free(M);
-    tc2_pack_free(M);
     delete M;
 }
 
-// use_tc: 0 = CUDA cores, 1 = single-CTA tensor-core kernel (round 1), 2 = CTA-pair tensor-core kernel
 static int resolve_path(const nqs_made *M, int path, int *use_tc) {
     if (path == NQS_PATH_SIMT) { *use_tc = 0; return NQS_OK; }
     if (path == NQS_PATH_TC) { if (!tc_supported(M)) return NQS_EUNSUPPORTED; *use_tc = 1; return NQS_OK; }
-    if (path == 3) { if (!tc2_supported(M)) return NQS_EUNSUPPORTED; *use_tc = 2; return NQS_OK; }
     if (path == NQS_PATH_AUTO) { *use_tc = (tc_supported(M) && M->h >= 384) ? 1 : 0; return NQS_OK; }
     return NQS_EINVAL;
 }
@@ -158,7 +160,6 @@ extern "C" int nqs_made_logpsi(const nqs_made_t *M, const uint64_t *configs_dev,
     if (B == 0) return NQS_OK;
     if ((rc = nqs_made_upload(M))) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
-    if (use_tc == 2) return launch_logpsi_tc2(M, (const ulonglong2 *)configs_dev, B, (float2 *)out_dev, st);
     if (use_tc) return launch_logpsi_tc(M, (const ulonglong2 *)configs_dev, B, (float2 *)out_dev, st);
     return launch_logpsi_simt(M->dev, (const ulonglong2 *)configs_dev, B, (float2 *)out_dev, st);
 }
@@ -221,13 +222,11 @@ extern "C" int nqs_local_energy(const nqs_ham_t *H, const nqs_made_t *M, const u
         const ulonglong2 *xs = (const ulonglong2 *)samples_dev + i0;
         float2 *eo = (float2 *)eloc_out_dev + i0;
         // base amplitudes f(x) (Alg. 1 line 2), same arithmetic path as the connected ones
-        if (use_tc == 2) rc = launch_logpsi_tc2(M, xs, nb, d_base, st);
-        else if (use_tc) rc = launch_logpsi_tc(M, xs, nb, d_base, st);
+        if (use_tc) rc = launch_logpsi_tc(M, xs, nb, d_base, st);
         else        rc = launch_logpsi_simt(M->dev, xs, nb, d_base, st);
         if (rc) return rc;
         CU(cudaEventRecord(M->ev[2 * b], st));
-        if (use_tc == 2) rc = launch_eloc_tc2(hm, M, xs, d_base, nb, eo, d_maxr, st);
-        else if (use_tc) rc = launch_eloc_tc(hm, M, xs, d_base, nb, eo, d_maxr, st);
+        if (use_tc) rc = launch_eloc_tc(hm, M, xs, d_base, nb, eo, d_maxr, st);
         else        rc = launch_eloc_simt(hm, M->dev, xs, d_base, nb, eo, (float2 *)d_scratch, nsplit, d_maxr, st);
         if (rc) return rc;
         CU(cudaEventRecord(M->ev[2 * b + 1], st));

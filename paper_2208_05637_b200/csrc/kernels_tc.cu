@@ -1,22 +1,25 @@
-// Tensor-core path (NQS_PATH_TC): ONE persistent, warp-specialised sm_100a kernel that runs, per tile of
-// 128 samples x 1 unique-flip group g,
-//   (a2) x' = x xor f_g expanded to a +-1 fp16 operand tile A0 in shared memory (double-buffered),
-//   (a4) the MADE chain and the phase MLP as tcgen05 MMAs (fp16 operands, fp32 accumulation in TMEM), in
-//        64-unit hidden CHUNKS that ping-pong between two TMEM accumulators D[0] / D[1]:
-//          layer 1   D = A0 . W1c^T        SS   -> epilogue: +b1, ReLU, fp16 -> A1 (TMEM, A operand of layer 2)
-//          phase     D = A0 . P1c^T        SS   -> epilogue: +c1, ReLU, fp16 IN PLACE -> D3 += D . P2c^T   (TS)
-//          layer 2   D = A1 . W2c^T        TS   -> epilogue: +b2, ReLU, fp16 IN PLACE -> D3 += D . W3c^T   (TS)
-//        all-zero 64x16 blocks of the masked weights are never issued (exact: they contribute 0),
+// Tensor-core path (NQS_PATH_TC): ONE persistent, warp-specialised sm_100a kernel run by CTA PAIRS (clusters of two
+// CTAs on one TPC, tcgen05 cta_group::2).  A pair works on two tiles at a time — CTA r on tile 2q + r, a tile being
+// 128 samples x 1 unique-flip group g — and every MMA covers both: M = 256 rows (128 per CTA), the weight operand B
+// split by rows between the two CTAs' shared memories, so each SM streams only HALF of the weight image.  Per tile:
+//   (a2) x' = x xor f_g expanded to a +-1 fp16 operand tile A0, written straight into TENSOR MEMORY (A operand of the
+//        input-layer MMAs; no shared-memory copy of the inputs exists),
+//   (a4) the MADE chain and the phase MLP as tcgen05 MMAs (fp16 operands, fp32 accumulation in TMEM), in 128-unit
+//        hidden CHUNKS that rotate through up to three 128-column TMEM accumulators:
+//          layer 1   D = A0 . W1c^T   TS  -> epilogue: +b1, ReLU, fp16 -> A1 in SHARED memory (128B-swizzled K-major)
+//          phase     D = A0 . P1c^T   TS  -> epilogue: +c1, ReLU, fp16 IN PLACE -> D3 += D . P2c^T   (TS, N = 16)
+//          layer 2   D = A1 . W2c^T   SS  -> epilogue: +b2, ReLU, fp16 IN PLACE -> D3 += D . W3c^T   (TS)
+//        (one hidden layer: layer 1 is rewritten in place and feeds W3 directly).  All-zero K-steps of the masked
+//        weights are never issued (exact: they contribute 0),
 //   (a3) the Pauli contraction S[i,g] over the group's terms (popcount parity, (-i)^r folded into c),
 //   (a5) ratio = exp(dlog|psi|) cis(dphi), E_i += S * ratio, kept in registers per sample.
-// Warp roles (14 warps): 0 = weight producers (a few lanes issue TMA 1-D bulk copies into a ring of large smem slots;
-// never more lanes than slots), 1 = MMA issuer (ONE elect.sync thread runs the fixed per-tile schedule; ring hand-over
-// bits, K-step counts and k-block lists come from a host-built table in kernel-parameter space), 2-5 / 6-9 = two
-// chunk-epilogue groups (one per accumulator), 10-13 = tile warps (build A0 of the NEXT tile, contraction, then the final
-// epilogue of the current one).  The weight tiles are pre-packed on the host into the exact shared-memory images
-// (128B-swizzled / core-matrix K-major) in consumption order.  What was measured and why the design is what it is:
-// DESIGN.md sections 6-7.
+// Warp roles (14 warps per CTA): 12 = weight producers (TMA 1-D bulk copies of this CTA's half of the weight image into
+// a ring of large slots); 13 = in the leader CTA the MMA issuer (ONE elect.sync thread issues every tcgen05.mma /
+// commit of the pair; commits are multicast to the barriers of both CTAs), in the peer CTA a forwarder that tells the
+// leader when the peer's half of a ring slot has landed; 4-7 / 8-11 = two chunk-epilogue groups (ops alternate);
+// 0-3 = tile warps (A0 of the NEXT tile, contraction, final epilogue).  DESIGN.md sections 6-7.
 // PAPER.md:122-134 (Alg. 1), :84-96 (architecture, Eq. 8-10), :152-158 (Eq. 15-16).
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <vector>
@@ -28,56 +31,62 @@ using namespace tc;
 namespace {
 
 constexpr int TILE_M = 128;
-constexpr int CH = 64;                   // hidden-unit chunk = accumulator columns
+constexpr int CN = 128;                  // hidden-unit chunk = accumulator columns = MMA N of the pair
+constexpr int HALF = CN / 2;             // weight rows per CTA and chunk
 constexpr int NTHREADS = 448;
-constexpr int MAX_NC = 8;                // hidden <= 512
-constexpr int MAX_SLOTS = 16;
-constexpr int NPROD = 4;                 // producer lanes (bulk-copy issuers)
+constexpr int MAX_NC = 4;                // hidden <= 512
+constexpr int MAX_SLOTS = 8;
+constexpr int NPROD = 4;                 // producer lanes (bulk-copy issuers), never more than slots
+constexpr int MAX_OPS = 3 * MAX_NC;
+// warp roles.  The warp scheduler of an SM sub-partition (warp id % 4) prefers the HIGHEST warp id among its eligible
+// warps, and every sub-partition hosts epilogue warps (a warp reaches only TMEM lane quadrant id % 4): the one thread
+// that issues all MMAs therefore lives in the highest warp id of its sub-partition, or it only gets the issue slots
+// the epilogue warps leave over.
+constexpr int W_EPI = 4, W_PROD = 12, W_ISSUE = 13;      // warps 0-3: tile warps
 
-// barrier ids
-enum { BAR_A0FULL = 0, BAR_DFULL = 2, BAR_DFREE = 4, BAR_INPL = 6, BAR_D3FULL = 8, BAR_D3EMPTY = 9,
-       BAR_WFULL = 10, BAR_WEMPTY = 10 + MAX_SLOTS, BAR_COUNT = 10 + 2 * MAX_SLOTS };
+enum : uint8_t { T_L1S = 0, T_L1I = 1, T_P = 2, T_L2 = 3 };   // layer 1 -> smem A1 | layer 1 in place | phase hidden | layer 2
 
-// Streamed weight sub-tiles are described by one 32-bit word each, in consumption order (kernel parameter
-// space -> uniform loads): offset inside the ring slot, ring hand-over flags and one small per-tile number.
-constexpr int MAX_SUB = 4 * MAX_NC + MAX_NC * MAX_NC;        // W1 + P1 + W2 blocks + W3
-constexpr uint32_t SUB_OFF_MASK = 0x1FFFu;                   // [0:13)  byte offset inside the slot / 16 (slots <= 128 KB)
+// barrier ids.  Waited by the leader's issuer (arrivals from both CTAs): A0FULL, D3EMPTY, EDONE[], WFULL[] (leader copy).
+// Committed by the issuer into BOTH CTAs: A0FREE, A1FREE, D3FULL, FULL[], WEMPTY[].
+enum { BAR_A0FULL = 0, BAR_A0FREE = 1, BAR_A1FREE = 2, BAR_D3FULL = 3, BAR_D3EMPTY = 4, BAR_FULL = 5, BAR_EDONE = 8,
+       BAR_WFULL = 11, BAR_WEMPTY = 11 + MAX_SLOTS, BAR_COUNT = 11 + 2 * MAX_SLOTS };
+
+// Streamed weight sub-tiles: one 32-bit word each, in consumption order (kernel parameter space -> uniform loads).
+constexpr int MAX_SUB = 2 * MAX_NC + MAX_NC * 2 * MAX_NC + MAX_NC;   // W1 + P1 + W2 blocks + W3
+constexpr uint32_t SUB_OFF_MASK = 0x1FFFu;                   // [0:13)  byte offset inside the slot / 16
 constexpr uint32_t SUB_NEW = 1u << 13;                       // first sub-tile of a ring fill: wait for the fill
 constexpr uint32_t SUB_END = 1u << 14;                       // last sub-tile of a ring fill: release the slot
-constexpr int SUB_AUX_SHIFT = 16;                            // [16:24) input chunks: K-steps to issue; W2: k-block; W3: n_lo / 16
+constexpr int SUB_AUX_SHIFT = 16;                            // [16:24) input: K-steps; W2: k-block | K-step mask << 4; W3: n_lo / 16
 
-struct ChunkOp { uint16_t bias_off; uint16_t dst_col; uint32_t kind; };   // kind 0: -> A1 at dst_col; 1: in place
+struct SmemLayout { uint32_t a1, res, bias, bars, slots, total; };
 
-struct SmemLayout { uint32_t a0, a0_bytes, res, bias, prog, chunks, bars, slots, total; };
-
-__host__ __device__ inline SmemLayout smem_layout(int KI, int H, int KO, int NC, uint32_t slot_bytes, int nslots) {
-    SmemLayout L;
+__host__ __device__ inline SmemLayout smem_layout(int H, int KO, int L, uint32_t slot_bytes, int nslots) {
+    SmemLayout S;
     uint32_t off = 0;
-    L.a0_bytes = (uint32_t)TILE_M * KI * 2;                      // [128][KI] fp16 core-matrix layout
-    L.a0 = off; off += 2 * L.a0_bytes;
-    off = (off + 1023) & ~1023u;
-    L.res = off; off += (uint32_t)NC * 2048;                     // resident P2 tiles (16 rows x 64 K, 128B swizzle)
-    L.bias = off; off += (uint32_t)(3 * H + KO + 4) * 4;
+    S.a1 = off; if (L == 2) off += (uint32_t)(H / 64) * 16384u;      // fp16 layer-1 activations, [H/64] K-blocks of 128 rows x 128 B
+    S.res = off; off += (uint32_t)(H / 64) * 1024u;                  // resident P2 tiles: 8 rows x 64 K per K-block (this CTA's half)
+    S.bias = off; off += (uint32_t)(3 * H + KO + 4) * 4;
     off = (off + 15) & ~15u;
-    L.prog = off;
-    L.chunks = off; off += 3 * MAX_NC * (uint32_t)sizeof(ChunkOp);
-    L.bars = off; off += BAR_COUNT * 8;
+    S.bars = off; off += BAR_COUNT * 8;
     off = (off + 1023) & ~1023u;
-    L.slots = off; off += slot_bytes * (uint32_t)nslots;
-    L.total = off;
-    return L;
+    S.slots = off; off += slot_bytes * (uint32_t)nslots;
+    S.total = off;
+    return S;
 }
 
 struct TcParams {
-    int n, H, NC, KI, KO;
-    uint32_t tm_d, tm_d3;                // TMEM columns: A1 at 0, D[0] at tm_d, D[1] at tm_d + 64, D3 at tm_d3
-    const uint8_t *wimg;                 // packed streamed weight tiles
-    const uint2 *fills;                  // per-tile ring fills: (byte offset, bytes), consumption order
-    int nfills;
-    uint32_t sub[MAX_SUB + 1];           // per-tile streamed sub-tiles (see SUB_*); one pad word (read-ahead)
+    int n, H, NC, KI, KO, L, nacc, nops;
+    int last_a0_op, last_l2_op;
+    uint32_t tm_d3, tm_a0;               // TMEM columns: accumulator a at a * CN, D3 at tm_d3, A0 at tm_a0
+    const uint8_t *wimg; uint32_t img_stride;     // streamed weight image of cluster rank r at wimg + r * img_stride
+    const uint2 *fills; int nfills;      // per-tile ring fills (byte offset, bytes), consumption order, same for both ranks
+    uint32_t sub[MAX_SUB + 1];
     uint8_t nblk[MAX_NC];                // layer-2 k-blocks issued per output chunk
-    const ChunkOp *chunks; int nchunks;  // per-tile accumulator chunks, in MMA order
-    const uint8_t *resimg; uint32_t res_bytes;   // resident P2 tiles
+    uint8_t l2need[MAX_NC];              // layer-2 chunk c needs A1 chunks 0 .. l2need[c]
+    uint8_t optype[MAX_OPS], opchunk[MAX_OPS];
+    uint8_t prewait[MAX_OPS];            // bit a: wait for the chunk epilogue pending on accumulator a before issuing op j
+    uint32_t cntmask;                    // bit a: accumulator a is used an odd number of times per tile
+    const uint8_t *resimg; uint32_t res_bytes;    // resident P2 tiles of rank r at resimg + r * res_bytes
     uint32_t slot_bytes; int nslots;
     const float *bias;                   // [c1 H | b1 H | b2 H | b3 KO | c2 4] fp32
     int mode;                            // 0 = logpsi, 1 = local energy
@@ -91,7 +100,20 @@ struct TcParams {
     float *eloc;                         // [B][2], pre-initialised with the f = 0 group; atomically accumulated
     unsigned *max_ratio_bits;
     long long g_begin;                   // first group that needs a forward pass (1 if group 0 is f = 0)
+#ifdef TC_PROF
+    long long *prof;                     // [grid][16] cycle counters (instrumented build only)
+#endif
 };
+
+#ifdef TC_PROF
+#define PROF_T0() const long long _t0 = clock64()
+#define PROF_ADD(v) (v) += clock64() - _t0
+#define PROF_STALL(sp) do { if (sp) { pw_stall += clock64() - _t0; ++pw_nstall; } ++pw_npoll; } while (0)
+#else
+#define PROF_T0() do {} while (0)
+#define PROF_ADD(v) do {} while (0)
+#define PROF_STALL(sp) do { (void)(sp); } while (0)
+#endif
 
 __device__ __forceinline__ unsigned long long shr128(ulonglong2 a, int s) {      // low 64 bits of a >> s, 0 <= s < 128
     if (s == 0) return a.x;
@@ -99,285 +121,360 @@ __device__ __forceinline__ unsigned long long shr128(ulonglong2 a, int s) {     
     return a.y >> (s - 64);
 }
 
-__global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_constant__ TcParams p) {
+// The per-tile op schedule, fixed at compile time so that the issuing thread runs straight-line code (it is
+// instruction-bound: the tensor pipe queues only ~100 cycles of MMAs ahead of the issuer, measured).  Two hidden
+// layers: layer-1 chunks 0..NC-1 (-> A1), then phase chunk c / layer-2 chunk c alternating; one hidden layer: layer-1
+// chunk c (in place) / phase chunk c alternating.  Op j runs in accumulator j % NACC and is handed to epilogue group
+// j & 1; the consumer of an in-place op is issued LAG = NACC - 1 ops later, just before the accumulator's next producer.
+template <int NC, int L, int NACC>
+struct Sched {
+    static constexpr int NOPS = (L == 2) ? 3 * NC : 2 * NC;
+    static constexpr int LAG = NACC - 1;
+    static constexpr int FIRST_INPLACE = (L == 2) ? NC : 0;
+    static constexpr int LAST_A0 = (L == 2) ? NOPS - 2 : NOPS - 1;
+    __host__ __device__ static constexpr int type(int j) {
+        return L == 2 ? (j < NC ? (int)T_L1S : (((j - NC) & 1) ? (int)T_L2 : (int)T_P)) : ((j & 1) ? (int)T_P : (int)T_L1I);
+    }
+    __host__ __device__ static constexpr int chunk(int j) { return L == 2 ? (j < NC ? j : (j - NC) / 2) : j / 2; }
+};
+
+template <int NC, int L, int NACC>
+__global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_constant__ TcParams p) {
+    using S = Sched<NC, L, NACC>;
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t s_tmem_base;
-    const SmemLayout L = smem_layout(p.KI, p.H, p.KO, p.NC, p.slot_bytes, p.nslots);
-    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + L.bars);
-    float *s_bias = reinterpret_cast<float *>(smem + L.bias);
+    const SmemLayout SL = smem_layout(p.H, p.KO, p.L, p.slot_bytes, p.nslots);
+    uint64_t *bars = reinterpret_cast<uint64_t *>(smem + SL.bars);
+    float *s_bias = reinterpret_cast<float *>(smem + SL.bias);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+    const uint32_t rank = cluster_ctarank();
     const int KI = p.KI, KO = p.KO, H = p.H;
+    constexpr uint32_t nops = S::NOPS;
+    const uint32_t smem_base = smem_u32(smem);
+    const uint32_t bars_addr = smem_base + SL.bars;
+#define BAR_ADDR(id) (bars_addr + (uint32_t)(id) * 8u)
 
     // ---- one-time setup ----
     if (threadIdx.x == 0) {
-        mbar_init(&bars[BAR_A0FULL], 4); mbar_init(&bars[BAR_A0FULL + 1], 4);
-        for (int b = 0; b < 2; ++b) {
-            mbar_init(&bars[BAR_DFULL + b], 1);
-            mbar_init(&bars[BAR_DFREE + b], 4);
-            mbar_init(&bars[BAR_INPL + b], 4);
+        mbar_init(&bars[BAR_A0FULL], 8); mbar_init(&bars[BAR_A0FREE], 1); mbar_init(&bars[BAR_A1FREE], 1);
+        mbar_init(&bars[BAR_D3FULL], 1); mbar_init(&bars[BAR_D3EMPTY], 8);
+        for (int a = 0; a < 3; ++a) { mbar_init(&bars[BAR_FULL + a], 1); mbar_init(&bars[BAR_EDONE + a], 8); }
+        for (int s = 0; s < p.nslots; ++s) {
+            mbar_init(&bars[BAR_WFULL + s], rank == 0 ? 2 : 1);      // leader: own producer + the peer's forwarder
+            mbar_init(&bars[BAR_WEMPTY + s], 1);
         }
-        mbar_init(&bars[BAR_D3FULL], 1);
-        mbar_init(&bars[BAR_D3EMPTY], 4);
-        for (int s = 0; s < p.nslots; ++s) { mbar_init(&bars[BAR_WFULL + s], 1); mbar_init(&bars[BAR_WEMPTY + s], 1); }
         fence_mbar_init();
     }
-    if (warp == 1) tmem_alloc(&s_tmem_base, 512);
+    if (warp == W_ISSUE) tmem_alloc_cg2(&s_tmem_base, 512);
     for (int i = threadIdx.x; i < 3 * H + KO + 4; i += NTHREADS) s_bias[i] = p.bias[i];
-    for (int i = threadIdx.x; i < p.nchunks * (int)(sizeof(ChunkOp) / 8); i += NTHREADS)
-        reinterpret_cast<uint2 *>(smem + L.chunks)[i] = reinterpret_cast<const uint2 *>(p.chunks)[i];
     for (int i = threadIdx.x; i < (int)(p.res_bytes / 16); i += NTHREADS)
-        reinterpret_cast<uint4 *>(smem + L.res)[i] = reinterpret_cast<const uint4 *>(p.resimg)[i];
+        reinterpret_cast<uint4 *>(smem + SL.res)[i] = reinterpret_cast<const uint4 *>(p.resimg + (size_t)rank * p.res_bytes)[i];
     fence_proxy_async();                                  // resident tiles are read by the tensor core (async proxy)
     tc_fence_before();
-    __syncthreads();
+    cluster_sync_all();
     tc_fence_after();
     const uint32_t tmem = s_tmem_base;
 
-    // ---- static tile schedule: contiguous range per CTA, sample-block major ----
+    // ---- static schedule: a contiguous range of tile PAIRS per cluster, sample-block major; CTA r takes tile 2q + r ----
     const long long nsb = (p.B + TILE_M - 1) / TILE_M;
     const long long Gnd = (p.mode == 1) ? (p.hm.G - p.g_begin) : 1;
     const long long ntiles = nsb * Gnd;
-    const long long t_lo = ntiles * blockIdx.x / gridDim.x, t_hi = ntiles * (blockIdx.x + 1) / gridDim.x;
+    const long long npairs = (ntiles + 1) / 2;
+    const long long ncl = gridDim.x >> 1, cl = blockIdx.x >> 1;
+    const long long q_lo = npairs * cl / ncl, q_hi = npairs * (cl + 1) / ncl;
+    const long long ntl = q_hi - q_lo;
 
-    if (warp == 0) {
-        // =========================== weight producers (TMA engine, 1-D bulk copies) ===========================
-        // One thread sustains about one ring fill per ~700 cycles (measured: the rate does not depend on the fill
-        // size), so NPROD lanes share the fills round-robin; fill q always lands in slot q % nslots.
-        // Never more lanes than slots: a lane that runs two uses of a slot ahead of the consumer would see the
-        // parity of an older phase and overwrite live data (parity waits alias after two phases).
+    if (warp == W_PROD) {
+        // =========================== weight producers (TMA engine, 1-D bulk copies), both CTAs ===========================
+        // Fill q always lands in slot q % nslots.  Never more lanes than slots: a lane two uses of a slot ahead of the
+        // consumer would pass its parity wait on an older phase and overwrite live data.
         const uint32_t nprod = (uint32_t)(p.nslots < NPROD ? p.nslots : NPROD);
         if ((uint32_t)lane < nprod) {
-            const long long total = (t_hi - t_lo) * (long long)p.nfills;
-            uint32_t e = (uint32_t)lane % (uint32_t)p.nfills, slot = (uint32_t)lane % (uint32_t)p.nslots;
-            uint32_t par = 1u ^ (((uint32_t)lane / (uint32_t)p.nslots) & 1u);   // a fresh barrier passes a parity-1 wait
+            const long long total = ntl * (long long)p.nfills;
+            const uint8_t *img = p.wimg + (size_t)rank * p.img_stride;
+            uint32_t e = (uint32_t)lane % (uint32_t)p.nfills, slot = (uint32_t)lane, par = 1u;   // a fresh barrier passes a parity-1 wait
             for (long long q = lane; q < total; q += nprod) {
                 const uint2 pe = __ldg(&p.fills[e]);
                 mbar_wait(&bars[BAR_WEMPTY + slot], par);
                 mbar_arrive_expect_tx(&bars[BAR_WFULL + slot], pe.y);
-                bulk_g2s(smem + L.slots + slot * p.slot_bytes, p.wimg + pe.x, pe.y, &bars[BAR_WFULL + slot]);
+                bulk_g2s(smem + SL.slots + slot * p.slot_bytes, img + pe.x, pe.y, &bars[BAR_WFULL + slot]);
                 e += nprod; while (e >= (uint32_t)p.nfills) e -= (uint32_t)p.nfills;
                 slot += nprod; while (slot >= (uint32_t)p.nslots) { slot -= (uint32_t)p.nslots; par ^= 1u; }
             }
         }
-    } else if (warp == 1) {
-        // =========================== MMA issuer: ONE elected thread ===========================
-        // Inside an elect.sync region ptxas knows a single thread is active and moves operands to uniform registers
-        // with plain R2UR; under `lane == 0` (or lane-predicated issue in a convergent warp) it emits a waterfall loop
-        // (ELECT / R2UR.BROADCAST / BRA.U.ANY, ~12 instructions) around every tcgen05.mma.
-        // The per-tile schedule is fixed code (stage A: layer 1 -> A1; stage P: phase hidden, in place, P2 one chunk
-        // behind; stage C: layer 2 from A1, in place, W3 one chunk behind); only the ring hand-over bits, the K-step
-        // counts and the k-block lists come from the parameter table.  Barrier parities live in the bits of `ph`.
+    } else if (warp == W_ISSUE && rank != 0) {
+        // =========================== peer CTA: ring forwarder ===========================
+        // The leader's MMAs read this CTA's half of every ring slot; a bulk copy can only signal a barrier of its own
+        // CTA, so one thread waits for each local fill and arrives on the leader's WFULL barrier of the same slot.
         if (elect_one()) {
-            const uint32_t issue = 1u;
-            const uint32_t smem_base = smem_u32(smem);
-            const uint32_t bars_addr = smem_base + L.bars;
-            const uint32_t a0_lo0 = (smem_base + L.a0) >> 4, a0_step = L.a0_bytes >> 4;
-            const uint32_t slots_lo = (smem_base + L.slots) >> 4, slot_step = p.slot_bytes >> 4, res_lo = (smem_base + L.res) >> 4;
+            const long long total = ntl * (long long)p.nfills;
+            uint32_t slot = 0, par = 0;
+            for (long long q = 0; q < total; ++q) {
+                mbar_wait(&bars[BAR_WFULL + slot], par);
+                mbar_arrive_cluster(BAR_ADDR(BAR_WFULL + slot), 0);
+                if (++slot == (uint32_t)p.nslots) { slot = 0; par ^= 1u; }
+            }
+        }
+        __syncwarp();
+    } else if (warp == W_ISSUE) {
+        // =========================== leader CTA: MMA issuer, ONE elected thread ===========================
+        // Ops of a tile are issued in the fixed order of Sched; the consumer of an in-place op (P2 / W3 MMAs reading the
+        // fp16 chunk the epilogue wrote over the accumulator) is issued LAG ops later — the tensor pipe executes in
+        // issue order, so MMA-after-MMA hazards need no barrier; only epilogue <-> MMA hand-overs do (FULL / EDONE).
+        // Every EDONE phase is waited exactly once, at a position fixed on the host (p.prewait) or at the consumer, so
+        // barrier parities are plain bits of `ph`.
+        if (elect_one()) {
+            const uint32_t a1_lo = (smem_base + SL.a1) >> 4, res_lo = (smem_base + SL.res) >> 4;
+            const uint32_t slots_lo = (smem_base + SL.slots) >> 4, slot_step = p.slot_bytes >> 4;
             // descriptor words: lo = addr/16 | (lbo/16) << 16, hi = sbo/16 | version 1 << 14 | layout << 29
             const uint32_t lo_noswz = (128u >> 4) << 16, hi_noswz = (((uint32_t)(KI / 8) * 128u) >> 4) | (1u << 14);
             const uint32_t lo_sw128 = (16u >> 4) << 16, hi_sw128 = (1024u >> 4) | (1u << 14) | (2u << 29);
-            const uint32_t id64 = idesc_f16(128, 64), id16 = idesc_f16(128, 16), id0 = idesc_f16(128, 0);
-            const uint32_t NC = (uint32_t)p.NC, nslots = (uint32_t)p.nslots;
-            const uint32_t tm_d = tmem + p.tm_d, tm_d3 = tmem + p.tm_d3, tm_ph = tm_d3 + (uint32_t)KO - 16;
-            uint32_t ph = 0, slot = 0, wpar = 0, slot_lo = slots_lo, tcount = 0;
-#define BAR_ADDR(id) (bars_addr + (uint32_t)(id) * 8u)
-#define WAIT_BAR(id) do { mbar_spin(BAR_ADDR(id), (ph >> (id)) & 1u); ph ^= 1u << (id); tc_fence_after(); } while (0)
-#define SLOT_ACQUIRE(w) do { if ((w) & SUB_NEW) { mbar_spin(BAR_ADDR(BAR_WFULL + slot), wpar); tc_fence_after(); } } while (0)
-#define SLOT_RELEASE(w) do { if ((w) & SUB_END) { mma_commit_addr_if(issue, BAR_ADDR(BAR_WEMPTY + slot)); slot_lo += slot_step; \
+            const uint32_t id128 = idesc_f16(256, CN), id16 = idesc_f16(256, 16), id0 = idesc_f16(256, 0);
+            const uint32_t nslots = (uint32_t)p.nslots;
+            const uint32_t tm_d3 = tmem + p.tm_d3, tm_ph = tm_d3 + (uint32_t)KO - 16, tm_a0 = tmem + p.tm_a0;
+            uint32_t slot = 0, wpar = 0, slot_lo = slots_lo;
+            uint32_t ph = 0;                             // parity of the next phase to wait for, one bit per barrier id
+#ifdef TC_PROF
+            long long pw_wait = 0, pw_wf = 0, pw_tot = clock64();
+#endif
+#define WAIT(id) do { PROF_T0(); mbar_spin(BAR_ADDR(id), (ph >> (id)) & 1u); ph ^= 1u << (id); tc_fence_after(); PROF_ADD(pw_wait); } while (0)
+#define SLOT_ACQUIRE(w) do { if ((w) & SUB_NEW) { PROF_T0(); mbar_spin(BAR_ADDR(BAR_WFULL + slot), wpar); tc_fence_after(); PROF_ADD(pw_wf); } } while (0)
+#define SLOT_RELEASE(w) do { if ((w) & SUB_END) { mma_commit_cg2(BAR_ADDR(BAR_WEMPTY + slot)); slot_lo += slot_step; \
                              if (++slot == nslots) { slot = 0; wpar ^= 1u; slot_lo = slots_lo; } } } while (0)
-            // input-layer chunk (SS): D[b] = A0 . Wc^T over the first nk K-steps (a prefix: masked columns are the high ones)
-            auto input_chunk = [&](uint32_t w, uint32_t a0_lo, uint32_t b) {
-                SLOT_ACQUIRE(w);
-                const uint32_t nk = (w >> SUB_AUX_SHIFT) & 0xFFu, d = tm_d + b * CH;
-                const uint32_t a_lo = a0_lo | lo_noswz, b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_noswz;
-                mma_ss2(issue, d, a_lo, hi_noswz, b_lo, hi_noswz, id64, 0u);
-                // nested so that the common exit is ONE taken branch (KI <= 128 -> at most 8 K-steps)
-#define KSTEP(k) mma_ss2(issue, d, a_lo + 16u * (k), hi_noswz, b_lo + 16u * (k), hi_noswz, id64, 1u)
-                if (nk > 1) { KSTEP(1); if (nk > 2) { KSTEP(2); if (nk > 3) { KSTEP(3); if (nk > 4) { KSTEP(4);
-                if (nk > 5) { KSTEP(5); if (nk > 6) { KSTEP(6); if (nk > 7) { KSTEP(7); } } } } } } }
-#undef KSTEP
-                SLOT_RELEASE(w);
-                mma_commit_addr_if(issue, BAR_ADDR(BAR_DFULL + b));
-            };
-            // consumer of the in-place fp16 chunk in D[b]: dst += D[b] . B^T, 4 K-steps of 16
-            auto consume = [&](uint32_t b, uint32_t b_lo, uint32_t dst, uint32_t idesc) {
-                const uint32_t a_t = tm_d + b * CH;
-                b_lo |= lo_sw128;
-#pragma unroll
-                for (uint32_t ks = 0; ks < 4; ++ks) mma_ts2(issue, dst, a_t + 8 * ks, b_lo + 2 * ks, hi_sw128, idesc, 1u);
-            };
-            auto consume_phase = [&](uint32_t c, uint32_t b) {                  // P2 tile c is resident
-                WAIT_BAR(BAR_INPL + b);
-                if (c == 0) WAIT_BAR(BAR_D3EMPTY);                               // first write into D3 of this tile
-                consume(b, res_lo + c * (2048u >> 4), tm_ph, id16);
-            };
-            auto consume_w3 = [&](uint32_t w, uint32_t b, bool last) {          // streamed layer-3 tile
-                WAIT_BAR(BAR_INPL + b);
-                SLOT_ACQUIRE(w);
-                const uint32_t nlo = ((w >> SUB_AUX_SHIFT) & 0xFFu) * 16;       // output rows below n_lo receive exactly 0
-                consume(b, slot_lo + (w & SUB_OFF_MASK) + (nlo / 8) * 64, tm_d3 + nlo, id0 | ((((uint32_t)KO - nlo) >> 3) << 17));
-                SLOT_RELEASE(w);
-                if (last) mma_commit_addr_if(issue, BAR_ADDR(BAR_D3FULL));
-            };
-            auto l2_chunk = [&](uint32_t c2, uint32_t b, uint32_t &si) {        // D[b] = A1 . W2[c2]^T over the listed k-blocks
-                const uint32_t nb = p.nblk[c2], d = tm_d + b * CH;
-                uint32_t w = p.sub[si];
-#pragma unroll 1
-                for (uint32_t j = 0; j < nb; ++j) {
-                    const uint32_t wn = p.sub[si + 1];                           // next word early: hides the constant-load latency
-                    ++si;
-                    SLOT_ACQUIRE(w);
-                    const uint32_t a_t = tmem + ((w >> SUB_AUX_SHIFT) & 0xFFu) * (CH / 2);
-                    const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_sw128;
-                    mma_ts2(issue, d, a_t, b_lo, hi_sw128, id64, j);
-                    mma_ts2(issue, d, a_t + 8, b_lo + 2, hi_sw128, id64, 1u);
-                    mma_ts2(issue, d, a_t + 16, b_lo + 4, hi_sw128, id64, 1u);
-                    mma_ts2(issue, d, a_t + 24, b_lo + 6, hi_sw128, id64, 1u);
-                    SLOT_RELEASE(w);
-                    w = wn;
-                }
-                mma_commit_addr_if(issue, BAR_ADDR(BAR_DFULL + b));
-            };
-            for (long long t = t_lo; t < t_hi; ++t, ++tcount) {
-                const uint32_t a0_lo = a0_lo0 + (tcount & 1u) * a0_step;
+            for (long long ti = 0; ti < ntl; ++ti) {
+                // (the table index goes through an opaque asm so that the compiler cannot prove the table words loop-invariant
+                // and unswitch the tile loop on them: that multiplied the issuer's code size by ten)
                 uint32_t si = 0;
-                // ---- stage A: layer 1, epilogue -> A1 (frees the accumulator) ----
-                WAIT_BAR(BAR_A0FULL + (tcount & 1u));
-                for (uint32_t c = 0; c < NC; c += 2) {
-                    if (c >= 2) WAIT_BAR(BAR_DFREE + 0);
-                    input_chunk(p.sub[si++], a0_lo, 0);
-                    if (c >= 2) WAIT_BAR(BAR_DFREE + 1);
-                    input_chunk(p.sub[si++], a0_lo, 1);
+                asm volatile("" : "+r"(si));
+                uint32_t w = p.sub[si];                      // current table word; the next one is always loaded one step ahead
+                WAIT(BAR_A0FULL);
+                // consumer of tile-local op jc (jc is a compile-time constant after unrolling)
+                auto consume = [&](const int jc) {
+                    const int type = S::type(jc);
+                    if (type == T_L1S) return;
+                    WAIT(BAR_EDONE + jc % NACC);
+                    if (jc == S::FIRST_INPLACE) WAIT(BAR_D3EMPTY);              // first write into D3 of this tile
+                    const uint32_t a_t = tmem + (uint32_t)(jc % NACC) * CN;
+                    if (type == T_P) {                                          // resident P2 tile of this chunk, N = 16
+                        const uint32_t b_lo = (res_lo + (uint32_t)S::chunk(jc) * (2048u >> 4)) | lo_sw128;
+#pragma unroll
+                        for (uint32_t ks = 0; ks < 8; ++ks)
+                            mma_ts_cg2(tm_ph, a_t + 8 * ks, b_lo + (ks >> 2) * (1024u >> 4) + 2 * (ks & 3), hi_sw128, id16, 1u);
+                    } else {                                                    // streamed layer-3 tile
+                        const uint32_t wn = p.sub[++si];
+                        SLOT_ACQUIRE(w);
+                        const uint32_t nlo = ((w >> SUB_AUX_SHIFT) & 0xFFu) * 16;      // output rows below n_lo receive exactly 0
+                        const uint32_t N = (uint32_t)KO - nlo, kb_step = (N >> 1) * (128u >> 4);
+                        const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_sw128, idesc = id0 | ((N >> 3) << 17);
+#pragma unroll
+                        for (uint32_t ks = 0; ks < 8; ++ks)
+                            mma_ts_cg2(tm_d3 + nlo, a_t + 8 * ks, b_lo + (ks >> 2) * kb_step + 2 * (ks & 3), hi_sw128, idesc, 1u);
+                        SLOT_RELEASE(w);
+                        w = wn;
+                    }
+                };
+#pragma unroll
+                for (int j = 0; j < S::NOPS; ++j) {
+                    const int type = S::type(j), c = S::chunk(j), acc = j % NACC;
+                    uint32_t jj = (uint32_t)j;
+                    asm volatile("" : "+r"(jj));
+                    const uint32_t pw = p.prewait[jj];      // pending chunk epilogues this op depends on (accumulator reuse, A1 chunks)
+                    if (pw & 1u) WAIT(BAR_EDONE + 0);
+                    if (NACC > 1 && (pw & 2u)) WAIT(BAR_EDONE + 1);
+                    if (NACC > 2 && (pw & 4u)) WAIT(BAR_EDONE + 2);
+                    const uint32_t d = tmem + (uint32_t)acc * CN;
+                    if (type == T_L2) {
+                        const uint32_t nb = p.nblk[jj - (uint32_t)(j - c)];
+                        uint32_t accum = 0;
+#pragma unroll 1
+                        for (uint32_t b = 0; b < nb; ++b) {
+                            const uint32_t wn = p.sub[++si];
+                            SLOT_ACQUIRE(w);
+                            const uint32_t aux = (w >> SUB_AUX_SHIFT) & 0xFFu, kmask = aux >> 4;
+                            const uint32_t a_lo = (a1_lo + (aux & 7u) * (16384u >> 4)) | lo_sw128;
+                            const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_sw128;
+                            if (kmask == 0xFu) {
+                                mma_ss_cg2(d, a_lo, hi_sw128, b_lo, hi_sw128, id128, accum);
+                                mma_ss_cg2(d, a_lo + 2, hi_sw128, b_lo + 2, hi_sw128, id128, 1u);
+                                mma_ss_cg2(d, a_lo + 4, hi_sw128, b_lo + 4, hi_sw128, id128, 1u);
+                                mma_ss_cg2(d, a_lo + 6, hi_sw128, b_lo + 6, hi_sw128, id128, 1u);
+                                accum = 1u;
+                            } else {
+#pragma unroll
+                                for (uint32_t ks = 0; ks < 4; ++ks)
+                                    if ((kmask >> ks) & 1u) { mma_ss_cg2(d, a_lo + 2 * ks, hi_sw128, b_lo + 2 * ks, hi_sw128, id128, accum); accum = 1u; }
+                            }
+                            SLOT_RELEASE(w);
+                            w = wn;
+                        }
+                    } else {
+                        // input layers (layer 1 / phase hidden): A = A0 in TMEM, B = this chunk's rows, K-step prefix
+                        const uint32_t wn = p.sub[++si];
+                        SLOT_ACQUIRE(w);
+                        const uint32_t nk = (w >> SUB_AUX_SHIFT) & 0xFFu;
+                        const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_noswz;
+                        mma_ts_cg2(d, tm_a0, b_lo, hi_noswz, id128, 0u);
+                        // nested so that the common exit is one taken branch (KI <= 128 -> at most 8 K-steps)
+#define KSTEP(k) mma_ts_cg2(d, tm_a0 + 8u * (k), b_lo + 16u * (k), hi_noswz, id128, 1u)
+                        if (nk > 1) { KSTEP(1); if (nk > 2) { KSTEP(2); if (nk > 3) { KSTEP(3); if (nk > 4) { KSTEP(4);
+                        if (nk > 5) { KSTEP(5); if (nk > 6) { KSTEP(6); if (nk > 7) { KSTEP(7); } } } } } } }
+#undef KSTEP
+                        SLOT_RELEASE(w);
+                        w = wn;
+                    }
+                    mma_commit_cg2(BAR_ADDR(BAR_FULL + acc));
+                    if (j == S::LAST_A0) mma_commit_cg2(BAR_ADDR(BAR_A0FREE));                 // A0 may be rebuilt for the next tile
+                    if (L == 2 && j == S::NOPS - 1) mma_commit_cg2(BAR_ADDR(BAR_A1FREE));      // A1 may be rewritten by the next tile
+                    if (j >= S::LAG) consume(j - S::LAG);
                 }
-                // ---- stage P: phase hidden layer, in place; its consumer runs one chunk behind ----
-                for (uint32_t c = 0; c < NC; c += 2) {
-                    if (c == 0) WAIT_BAR(BAR_DFREE + 0);      // last stage-A chunk of group 0 (=> all of its A1 is written)
-                    input_chunk(p.sub[si++], a0_lo, 0);
-                    if (c >= 2) consume_phase(c - 1, 1);
-                    if (c == 0) WAIT_BAR(BAR_DFREE + 1);
-                    input_chunk(p.sub[si++], a0_lo, 1);
-                    consume_phase(c, 0);
-                }
-                // ---- stage C: layer 2 from A1 (TS), in place; consumers (P2 of the last phase chunk, then W3) one behind ----
-                for (uint32_t c2 = 0; c2 < NC; c2 += 2) {
-                    l2_chunk(c2, 0, si);
-                    if (c2 == 0) consume_phase(NC - 1, 1);
-                    else consume_w3(p.sub[si++], 1, false);
-                    l2_chunk(c2 + 1, 1, si);
-                    consume_w3(p.sub[si++], 0, false);
-                }
-                consume_w3(p.sub[si++], 1, true);
+#pragma unroll
+                for (int m = S::LAG; m >= 1; --m) consume(S::NOPS - m);                       // consumers of the last ops
+                mma_commit_cg2(BAR_ADDR(BAR_D3FULL));
             }
-#undef BAR_ADDR
-#undef WAIT_BAR
+#ifdef TC_PROF
+            if (p.prof) { long long *pr = p.prof + (size_t)blockIdx.x * 32; pr[0] = clock64() - pw_tot; pr[1] = pw_wait; pr[3] = pw_wf; pr[5] = ntl; }
+#endif
+#undef WAIT
 #undef SLOT_ACQUIRE
 #undef SLOT_RELEASE
         }
         __syncwarp();
-    } else if (warp < 10) {
-        // =========================== chunk epilogue groups: group g owns accumulator D[g] ===========================
-        const int grp = (warp - 2) >> 2;
+    } else if (warp >= W_EPI) {
+        // =========================== chunk epilogue groups: ops alternate between the two groups ===========================
+        const uint32_t grp = (uint32_t)(warp - W_EPI) >> 2;
+        const uint32_t row = (uint32_t)((warp & 3) * 32 + lane);
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;     // TMEM lane quadrant of this warp
-        const uint32_t d_addr = tmem + lane_base + p.tm_d + (uint32_t)grp * CH;
-        const ChunkOp *chunks = reinterpret_cast<const ChunkOp *>(smem + L.chunks);
-        uint32_t uses = 0;
-        for (long long t = t_lo; t < t_hi; ++t) {
-            for (int j = grp; j < p.nchunks; j += 2, ++uses) {
-                const ChunkOp co = chunks[j];
-                mbar_wait(&bars[BAR_DFULL + grp], uses & 1u);
-                tc_fence_after();
-                uint32_t v[64];
-                tmem_ld32p(d_addr, v);
-                tmem_ld32p(d_addr + 32, v + 32);
-                tmem_wait_ld();
-                const float4 *bp = reinterpret_cast<const float4 *>(s_bias + co.bias_off);
-                uint32_t w[32];
+        const uint32_t a1_row = smem_base + SL.a1 + (row >> 3) * 1024u + (row & 7u) * 128u, sw = row & 7u;
+        uint32_t fb = 0;                                   // bit a: parity of accumulator a's first FULL phase of this tile
+        long long pe_wait = 0, pe_a1 = 0, pe_tot = clock64(), pe_fence = 0, pe_arr = 0;
+        (void)pe_wait; (void)pe_a1; (void)pe_tot; (void)pe_fence; (void)pe_arr;
+        for (long long ti = 0; ti < ntl; ++ti, fb ^= p.cntmask)
+        for (uint32_t j = grp; j < nops; j += 2) {
+            const uint32_t type = p.optype[j], c = p.opchunk[j];
+            const uint32_t q = (NACC == 2) ? (j >> 1) : ((NACC == 3) ? ((j * 11u) >> 5) : j), acc = j - q * NACC;   // j / NACC, j % NACC (j < 32)
+            { PROF_T0(); mbar_wait(&bars[BAR_FULL + acc], ((fb >> acc) ^ q) & 1u); PROF_ADD(pe_wait); }
+            tc_fence_after();
+            if (L == 2 && ti > 0 && j == grp) {            // once per tile: the previous tile's layer-2 MMAs have read A1
+                PROF_T0(); mbar_wait(&bars[BAR_A1FREE], (uint32_t)(ti - 1) & 1u); PROF_ADD(pe_a1);
+            }
+            const uint32_t d_addr = tmem + lane_base + acc * CN;
+            const float *bias = s_bias + (type == T_P ? 0 : (type == T_L2 ? 2 * H : H)) + c * CN;
+            uint32_t va[32], vb[32];
+            tmem_ld32p(d_addr, va);
 #pragma unroll
-                for (int j4 = 0; j4 < 16; ++j4) {
+            for (int pc = 0; pc < 4; ++pc) {
+                uint32_t *v = (pc & 1) ? vb : va;
+                tmem_wait_ld();
+                if (pc < 3) tmem_ld32p(d_addr + 32 * (pc + 1), (pc & 1) ? va : vb);     // next piece in flight
+                const float4 *bp = reinterpret_cast<const float4 *>(bias + 32 * pc);
+                uint32_t w[16];
+#pragma unroll
+                for (int j4 = 0; j4 < 8; ++j4) {
                     const float4 bb = bp[j4];
                     w[2 * j4] = cvt_relu_f16x2(__uint_as_float(v[4 * j4]) + bb.x, __uint_as_float(v[4 * j4 + 1]) + bb.y);
                     w[2 * j4 + 1] = cvt_relu_f16x2(__uint_as_float(v[4 * j4 + 2]) + bb.z, __uint_as_float(v[4 * j4 + 3]) + bb.w);
                 }
-                const bool inplace = co.kind != 0;
-                tmem_st32(inplace ? d_addr : (tmem + lane_base + co.dst_col), w);
-                tmem_wait_st();
-                tc_fence_before();
-                __syncwarp();
-                if (lane == 0) mbar_arrive(&bars[(inplace ? BAR_INPL : BAR_DFREE) + grp]);
+                if (type == T_L1S) {
+                    // 32 hidden units = 64 B of this row: four 16-byte pieces of K-block 2c + pc/2, 128B swizzle
+                    const uint32_t kb_addr = a1_row + (2 * c + (uint32_t)(pc >> 1)) * 16384u;
+#pragma unroll
+                    for (uint32_t i = 0; i < 4; ++i) {
+                        const uint32_t jj = (uint32_t)(pc & 1) * 4 + i;
+                        st_shared_v4(kb_addr + ((jj ^ sw) << 4), w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
+                    }
+                } else {
+                    tmem_st16p(d_addr + 16 * pc, w);          // in place: columns [16 pc, 16 pc + 16) were read by piece pc / 2 <= pc
+                }
             }
+            { PROF_T0();
+            if (type == T_L1S) fence_proxy_async(); else tmem_wait_st();
+            tc_fence_before();
+            __syncwarp(); PROF_ADD(pe_fence); }
+            { PROF_T0();
+            if (lane == 0) mbar_arrive_leader(BAR_ADDR(BAR_EDONE + acc), rank);
+            __syncwarp(); PROF_ADD(pe_arr); }
         }
+#ifdef TC_PROF
+        if (p.prof && lane == 0 && (warp == W_EPI || warp == W_EPI + 4)) { long long *pr = p.prof + (size_t)blockIdx.x * 32 + (warp == W_EPI ? 6 : 11); pr[0] = clock64() - pe_tot; pr[1] = pe_wait; pr[2] = pe_a1; pr[3] = pe_fence; pr[4] = pe_arr; }
+#endif
     } else {
-        // =========================== tile warps: A0 of the next tile, final epilogue of the current ===========================
+        // =========================== tile warps: A0 of the next tile, contraction, final epilogue ===========================
         const int q = warp & 3;
         const int row = q * 32 + lane;
         const uint32_t lane_base = (uint32_t)(q * 32) << 16;
-        const uint32_t d3_addr = tmem + lane_base + p.tm_d3;
-        const uint32_t a0_sbo = (uint32_t)(KI / 8) * 128;
+        const uint32_t d3_addr = tmem + lane_base + p.tm_d3, a0_addr = tmem + lane_base + p.tm_a0;
         const float *s_b3 = s_bias + 3 * H, *s_c2 = s_bias + 3 * H + KO;
         const uint32_t zero16[16] = {0};
 
         struct RowState { long long sb, i; ulonglong2 xp, xq; float2 b0; };
-        auto load_row = [&](long long sb, RowState &r) {
-            r.sb = sb; r.i = sb * TILE_M + row;
+        auto load_row = [&](long long sb, bool valid, RowState &r) {
+            r.sb = sb; r.i = valid ? sb * TILE_M + row : p.B;
             if (r.i < p.B) {
                 r.xp = p.xpos[r.i];
                 if (p.mode == 1) { r.xq = p.x[r.i]; r.b0 = p.base[r.i]; }
                 else { r.xq = make_ulonglong2(0, 0); r.b0 = make_float2(0.f, 0.f); }
-            } else { r.xp = make_ulonglong2(0, 0); r.xq = r.xp; r.b0 = make_float2(0.f, 0.f); }
+            } else { r.i = p.B; r.xp = make_ulonglong2(0, 0); r.xq = r.xp; r.b0 = make_float2(0.f, 0.f); }
         };
-        // (a2) A0: +-1 fp16 tile, core-matrix K-major layout, one row per thread
-        auto build_a0 = [&](uint32_t buf, ulonglong2 zp) {
-            uint8_t *a0 = smem + L.a0 + buf * L.a0_bytes + (row >> 3) * a0_sbo + (row & 7) * 16;
-            for (int kc = 0; kc < KI / 8; ++kc) {
-                const uint32_t bits = (uint32_t)(shr128(zp, kc * 8) & 0xFFull);
-                uint4 w;
-                w.x = 0xBC00BC00u ^ ((bits & 1u) << 15) ^ ((bits & 2u) << 30);
-                w.y = 0xBC00BC00u ^ ((bits & 4u) << 13) ^ ((bits & 8u) << 28);
-                w.z = 0xBC00BC00u ^ ((bits & 16u) << 11) ^ ((bits & 32u) << 26);
-                w.w = 0xBC00BC00u ^ ((bits & 64u) << 9) ^ ((bits & 128u) << 24);
-                *reinterpret_cast<uint4 *>(a0 + kc * 128) = w;
+        // (a2) A0: +-1 fp16, one row per thread = one TMEM lane, 16 inputs = 8 columns per K-step
+        auto build_a0 = [&](ulonglong2 zp) {
+            for (int kc = 0; kc < KI / 16; ++kc) {
+                const uint32_t bits = (uint32_t)(shr128(zp, kc * 16) & 0xFFFFull);
+                uint32_t w[8];
+#pragma unroll
+                for (int jj = 0; jj < 8; ++jj)
+                    w[jj] = 0xBC00BC00u ^ (((bits >> (2 * jj)) & 1u) << 15) ^ (((bits >> (2 * jj + 1)) & 1u) << 31);
+                tmem_st8p(a0_addr + 8 * kc, w);
             }
-            fence_proxy_async();
+            tmem_wait_st();
+            tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(&bars[BAR_A0FULL + buf]);
+            if (lane == 0) mbar_arrive_leader(BAR_ADDR(BAR_A0FULL), rank);
         };
-        auto flip_of = [&](long long t) -> ulonglong2 {
-            if (p.mode != 1) return make_ulonglong2(0, 0);
+        auto flip_of = [&](long long t, bool valid) -> ulonglong2 {
+            if (p.mode != 1 || !valid) return make_ulonglong2(0, 0);
             return __ldg(&p.fpos[p.g_begin + (t % Gnd)]);
         };
 
         // D3 accumulates from zero (every MMA into it has accumulate = 1)
-        for (int c = 0; c < KO; c += 16) tmem_st16(d3_addr + c, zero16);
+        for (int c = 0; c < KO; c += 16) tmem_st16p(d3_addr + c, zero16);
         tmem_wait_st();
         tc_fence_before();
         __syncwarp();
-        if (lane == 0) mbar_arrive(&bars[BAR_D3EMPTY]);
+        if (lane == 0) mbar_arrive_leader(BAR_ADDR(BAR_D3EMPTY), rank);
 
         RowState cur{}, nxt{};
         ulonglong2 zp = make_ulonglong2(0, 0), zp_n = zp;
         float2 E = make_float2(0.f, 0.f);
         float mr = (p.mode == 1 && p.hm.has_diag) ? 1.0f : 0.0f;     // the f = 0 group has ratio exactly 1
-        uint32_t tcount = 0;
-        if (t_lo < t_hi) {
-            load_row(t_lo / Gnd, cur);
-            const ulonglong2 f = flip_of(t_lo);
+        long long pt_a0 = 0, pt_d3 = 0, pt_tot = clock64(), pt_s = 0, pt_fin = 0;
+        (void)pt_a0; (void)pt_d3; (void)pt_tot; (void)pt_s; (void)pt_fin;
+        if (ntl > 0) {
+            const long long t = 2 * q_lo + rank;
+            const bool valid = t < ntiles;
+            load_row(t / Gnd, valid, cur);
+            const ulonglong2 f = flip_of(t, valid);
             zp = make_ulonglong2(cur.xp.x ^ f.x, cur.xp.y ^ f.y);
-            build_a0(0, zp);
+            build_a0(zp);
         }
-        for (long long t = t_lo; t < t_hi; ++t, ++tcount) {
+        for (long long ti = 0; ti < ntl; ++ti) {
+            const long long t = 2 * (q_lo + ti) + rank;
+            const bool valid = t < ntiles;
             const long long g = p.g_begin + (t % Gnd);
-            // ---- operand tile of the NEXT tile (its buffer was last read by tile t-1, whose D3FULL we have seen) ----
-            const bool has_next = t + 1 < t_hi;
+            const bool has_next = ti + 1 < ntl;
             if (has_next) {
-                const long long sbn = (t + 1) / Gnd;
-                if (sbn != cur.sb) load_row(sbn, nxt); else nxt = cur;
-                const ulonglong2 f = flip_of(t + 1);
+                const long long tn = t + 2;
+                const bool validn = tn < ntiles;
+                const long long sbn = tn / Gnd;
+                if (sbn != cur.sb || !validn) load_row(sbn, validn, nxt); else nxt = cur;
+                const ulonglong2 f = flip_of(tn, validn);
                 zp_n = make_ulonglong2(nxt.xp.x ^ f.x, nxt.xp.y ^ f.y);
-                build_a0((tcount + 1) & 1u, zp_n);
             }
             // ---- (a3) S = sum_{t in g} c_t (-i)^{r_t} (-1)^{popcount(x & s_t)}: independent of the MMAs, done while they run ----
             float2 S = make_float2(0.f, 0.f);
-            if (p.mode == 1 && cur.i < p.B) {
+#ifdef TC_PROF
+            const long long _ts = clock64();
+#endif
+            if (p.mode == 1 && valid && cur.i < p.B) {
                 const uint32_t t1 = __ldg(&p.hm.offsets[g + 1]);
                 for (uint32_t tt = __ldg(&p.hm.offsets[g]); tt < t1; ++tt) {
                     const ulonglong2 zy = __ldg(&p.hm.zy[tt]);
@@ -387,9 +484,21 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_const
                     S.y += neg ? -c.y : c.y;
                 }
             }
+#ifdef TC_PROF
+            pt_s += (long long)__float_as_int(S.x) * 0 + clock64() - _ts;
+#endif
+            // ---- operand tile of the NEXT tile, once the last MMA that reads the current one has completed ----
+            if (has_next) {
+                { PROF_T0(); mbar_wait(&bars[BAR_A0FREE], (uint32_t)ti & 1u); PROF_ADD(pt_a0); }
+                tc_fence_after();
+                build_a0(zp_n);
+            }
             // ---- final epilogue: log|psi| = 1/2 sum_d log sigmoid(+-a_d), phi = o[2 z_{n-2} + z_{n-1}] ----
-            mbar_wait(&bars[BAR_D3FULL], tcount & 1u);
+            { PROF_T0(); mbar_wait(&bars[BAR_D3FULL], (uint32_t)ti & 1u); PROF_ADD(pt_d3); }
             tc_fence_after();
+#ifdef TC_PROF
+            const long long _tf = clock64();
+#endif
             // sum_d log sigmoid(t_d) = sum_d min(t_d, 0) - ln prod_d (1 + exp(-|t_d|)): every factor is in (1, 2], so a
             // 16-term product cannot overflow and costs one LG2 per 16 conditionals; the 16 chains are independent (ILP).
             float msum = 0.0f, lg = 0.0f, phi = 0.0f;
@@ -397,7 +506,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_const
                 uint32_t v[16];
                 tmem_ld16p(d3_addr + c0, v);
                 tmem_wait_ld();
-                tmem_st16(d3_addr + c0, zero16);              // D3 restarts from zero for the next tile
+                tmem_st16p(d3_addr + c0, zero16);              // D3 restarts from zero for the next tile
                 if (c0 + 16 >= KO) {
                     const int sel = (int)((shr128(zp, p.n - 2) & 1ull) * 2 + (shr128(zp, p.n - 1) & 1ull));
                     const float o0 = __uint_as_float(v[12]) + s_c2[0], o1 = __uint_as_float(v[13]) + s_c2[1];
@@ -416,11 +525,11 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_const
                     for (int kk = 0; kk < 4; ++kk) {
                         const int k = 4 * k4 + kk;
                         const float a = __uint_as_float(v[k]) + bk[kk];
-                        float t = ((zb >> k) & 1u) ? a : -a;
-                        t = (k < nv) ? t : 1e30f;              // padding column: factor 1, min 0
-                        const float e = ex2_ftz(fabsf(t) * -1.4426950408889634f);
-                        if (k & 1) { prod1 *= 1.0f + e; m1 += fminf(t, 0.0f); }
-                        else       { prod0 *= 1.0f + e; m0 += fminf(t, 0.0f); }
+                        float tt = ((zb >> k) & 1u) ? a : -a;
+                        tt = (k < nv) ? tt : 1e30f;            // padding column: factor 1, min 0
+                        const float e = ex2_ftz(fabsf(tt) * -1.4426950408889634f);
+                        if (k & 1) { prod1 *= 1.0f + e; m1 += fminf(tt, 0.0f); }
+                        else       { prod0 *= 1.0f + e; m0 += fminf(tt, 0.0f); }
                     }
                 }
                 msum += m0 + m1;
@@ -430,7 +539,7 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_const
             tmem_wait_st();
             tc_fence_before();
             __syncwarp();
-            if (lane == 0) mbar_arrive(&bars[BAR_D3EMPTY]);
+            if (lane == 0) mbar_arrive_leader(BAR_ADDR(BAR_D3EMPTY), rank);
             const float lp = 0.5f * part;
             if (p.mode == 0) {
                 if (cur.i < p.B) p.out[cur.i] = make_float2(lp, phi);
@@ -444,20 +553,27 @@ __global__ void __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_const
                 E.x += S.x * rr - S.y * ri;
                 E.y += S.x * ri + S.y * rr;
             }
-            if (!has_next || nxt.sb != cur.sb) {
+            if (!has_next || nxt.sb != cur.sb || nxt.i != cur.i) {
                 if (p.mode == 1 && cur.i < p.B) {
                     atomicAdd(&p.eloc[2 * cur.i], E.x);
                     atomicAdd(&p.eloc[2 * cur.i + 1], E.y);
                 }
                 E = make_float2(0.f, 0.f);
             }
+#ifdef TC_PROF
+            pt_fin += clock64() - _tf;
+#endif
             cur = nxt; zp = zp_n;
         }
         if (p.mode == 1) atomicMax(p.max_ratio_bits, __float_as_uint(mr));
+#ifdef TC_PROF
+        if (p.prof && lane == 0 && warp == 0) { long long *pr = p.prof + (size_t)blockIdx.x * 32 + 16; pr[0] = clock64() - pt_tot; pr[1] = pt_a0; pr[2] = pt_d3; pr[3] = pt_s; pr[4] = pt_fin; }
+#endif
     }
+#undef BAR_ADDR
     tc_fence_before();
-    __syncthreads();
-    if (warp == 1) tmem_dealloc(tmem, 512);
+    cluster_sync_all();
+    if (warp == W_ISSUE) tmem_dealloc_cg2(tmem, 512);
 }
 
 // position-ordered copy of 128-bit configurations: out bit d = in bit order[d]
@@ -498,39 +614,56 @@ __global__ void diag_init_kernel(HamDev hm, const ulonglong2 *__restrict__ x, lo
 
 // ------------------------------------------------------------------------------------------------------------
 struct TcPack {
-    int KI = 0, KO = 0, NC = 0, nsub = 0, nchunks = 0, nfills = 0, nslots = 0;
-    uint32_t slot_bytes = 0, res_bytes = 0, tm_d = 0, tm_d3 = 0;
-    void *d_wimg = nullptr, *d_fills = nullptr, *d_chunks = nullptr, *d_res = nullptr, *d_bias = nullptr;
+    int KI = 0, KO = 0, NC = 0, nacc = 0, nops = 0, nsub = 0, nfills = 0, nslots = 0, last_a0_op = -1, last_l2_op = -1;
+    uint32_t slot_bytes = 0, res_bytes = 0, img_stride = 0, tm_d3 = 0, tm_a0 = 0;
+    void *d_wimg = nullptr, *d_fills = nullptr, *d_res = nullptr, *d_bias = nullptr;
     void *d_fpos = nullptr; size_t fpos_cap = 0;
     void *d_xpos = nullptr; size_t xpos_cap = 0;
     SmemLayout L{};
     uint32_t sub[MAX_SUB + 1] = {0};
-    uint8_t nblk[MAX_NC] = {0};
+    uint8_t nblk[MAX_NC] = {0}, l2need[MAX_NC] = {0}, optype[MAX_OPS] = {0}, opchunk[MAX_OPS] = {0}, prewait[MAX_OPS] = {0};
+    uint32_t cntmask = 0;
     int sms = 148;
-    long long mma_issued = 0, mma_dense = 0;                   // K-steps issued / K-steps of the dense chain, per tile
+    long long mma_issued = 0, mma_dense = 0;                   // 16-wide K-steps x N issued / of the dense chain, per tile (MACs / 2048)
 };
 
 static inline int round16(int v) { return (v + 15) / 16 * 16; }
 
-static bool tc_shape(const nqs_made *M, int *KI_, int *KO_, uint32_t *slot_, int *nslots_) {
-    if (M->L != 2 || M->h % (2 * CH) != 0 || M->h < 2 * CH || M->h > CH * MAX_NC) return false;
-    const int KI = round16(M->n), KO = round16(M->n + 4), NC = M->h / CH;
-    if (KI > 128 || KO > 128 || M->h / 2 + 2 * CH + KO > 512) return false;
-    uint32_t slot = (uint32_t)CH * KI * 2;                                  // input sub-tile (64 rows x KI)
-    if ((uint32_t)CH * 128 > slot) slot = CH * 128;                          // layer-2 sub-tile (64 x 64)
-    if ((uint32_t)KO * 128 > slot) slot = (uint32_t)KO * 128;                // layer-3 sub-tile (KO x 64)
-    slot = ((2 * slot) + 1023) & ~1023u;                                     // at least two sub-tiles per fill
-    if (slot < 81920u) slot = 81920u;                                        // few, large bulk copies (a thread sustains ~1 copy / 700 cycles)
-    int ns = MAX_SLOTS;
-    while (ns > 0 && smem_layout(KI, M->h, KO, NC, slot, ns).total > 227 * 1024 - 1024) --ns;
-    if (ns < 2) return false;
-    *KI_ = KI; *KO_ = KO; *slot_ = slot; *nslots_ = ns;
+struct TcShape { int KI, KO, NC, nacc, nslots; uint32_t slot; };
+
+static bool tc_shape(const nqs_made *M, TcShape *out) {
+    if ((M->L != 1 && M->L != 2) || M->h % CN != 0 || M->h < CN || M->h > CN * MAX_NC) return false;
+    TcShape s;
+    s.KI = round16(M->n); s.KO = round16(M->n + 4); s.NC = M->h / CN;
+    if (s.KI > 128 || s.KO > 144) return false;
+    // TMEM: nacc accumulators of CN columns, D3 (KO), A0 (KI/2)
+    s.nacc = 3;
+    if (s.nacc * CN + s.KO + s.KI / 2 > 512) s.nacc = 2;
+    if (s.nacc * CN + s.KO + s.KI / 2 > 512) return false;
+    uint32_t need = (uint32_t)HALF * s.KI * 2;                                 // input sub-tile (64 rows x KI)
+    if ((uint32_t)HALF * 128 > need) need = HALF * 128;                        // layer-2 sub-tile (64 x 64)
+    if ((uint32_t)s.KO * 128 > need) need = (uint32_t)s.KO * 128;              // layer-3 tile (KO/2 rows x 128 K)
+    const uint32_t budget = 227 * 1024 - 1024;
+    const uint32_t fixed = smem_layout(M->h, s.KO, M->L, 0, 0).total;
+    if (fixed + 2 * need > budget) return false;
+    const uint32_t ring = budget - fixed;
+    int ns = 4;                                                                // few, large fills: every ring hand-over costs the issuer a poll
+    while (ns > 2 && (ring / ns) / 1024 * 1024 < 2 * need) --ns;
+    uint32_t slot = (ring / ns) / 1024 * 1024;
+    if (slot < need) return false;
+    if (slot > 0x1FFFu * 16u) slot = 0x1FFFu * 16u / 1024 * 1024;
+#ifdef TC_PROF
+    if (const char *e = getenv("NQS_TC_SLOT_KB")) { slot = (uint32_t)atoi(e) * 1024; }
+    if (const char *e = getenv("NQS_TC_NSLOTS")) { ns = atoi(e); }
+#endif
+    s.slot = slot; s.nslots = ns;
+    *out = s;
     return true;
 }
 
 bool tc_supported(const nqs_made *M) {
-    int KI, KO, ns; uint32_t slot;
-    return tc_shape(M, &KI, &KO, &slot, &ns);
+    TcShape s;
+    return tc_shape(M, &s);
 }
 
 static inline uint32_t noswz_offset(uint32_t r, uint32_t k, uint32_t KI) {
@@ -539,21 +672,39 @@ static inline uint32_t noswz_offset(uint32_t r, uint32_t k, uint32_t KI) {
 
 int tc_pack_upload(const nqs_made *M) {
     if (M->tc) return NQS_OK;
-    int KI, KO, ns; uint32_t slot;
-    if (!tc_shape(M, &KI, &KO, &slot, &ns)) return NQS_EUNSUPPORTED;
+    TcShape sh;
+    if (!tc_shape(M, &sh)) return NQS_EUNSUPPORTED;
     TcPack *P = new (std::nothrow) TcPack();
     if (!P) return NQS_ENOMEM;
-    const int n = M->n, H = M->h, NC = H / CH;
-    P->KI = KI; P->KO = KO; P->NC = NC; P->slot_bytes = slot; P->nslots = ns;
-    P->tm_d = (uint32_t)H / 2; P->tm_d3 = (uint32_t)H / 2 + 2 * CH;
-    P->L = smem_layout(KI, H, KO, NC, slot, ns);
-    const uint32_t in_bytes = (uint32_t)CH * KI * 2, w2_bytes = CH * 128, w3_bytes = (uint32_t)KO * 128;
+    const int n = M->n, H = M->h, NC = sh.NC, KI = sh.KI, KO = sh.KO, L = M->L;
+    P->KI = KI; P->KO = KO; P->NC = NC; P->nacc = sh.nacc; P->slot_bytes = sh.slot; P->nslots = sh.nslots;
+    P->tm_d3 = (uint32_t)sh.nacc * CN; P->tm_a0 = P->tm_d3 + (uint32_t)KO;
+    P->L = smem_layout(H, KO, L, sh.slot, sh.nslots);
+    const uint32_t slot = sh.slot;
+    const uint32_t in_bytes = (uint32_t)HALF * KI * 2, w2_bytes = HALF * 128;
+    const std::vector<float> &W1 = M->wm[0], &W3 = M->wm[L];
 
-    std::vector<uint8_t> img, res((size_t)NC * 2048, 0);
+    // ---- the per-tile op list (must match the issuer / epilogue loops of eloc_tc_kernel) ----
+    int nops = 0;
+    if (L == 2) {
+        for (int c = 0; c < NC; ++c) { P->optype[nops] = T_L1S; P->opchunk[nops++] = (uint8_t)c; }
+        for (int c = 0; c < NC; ++c) {
+            P->optype[nops] = T_P; P->opchunk[nops] = (uint8_t)c; P->last_a0_op = nops++;
+            P->optype[nops] = T_L2; P->opchunk[nops] = (uint8_t)c; P->last_l2_op = nops++;
+        }
+    } else {
+        for (int c = 0; c < NC; ++c) {
+            P->optype[nops] = T_L1I; P->opchunk[nops++] = (uint8_t)c;
+            P->optype[nops] = T_P; P->opchunk[nops] = (uint8_t)c; P->last_a0_op = nops++;
+        }
+    }
+    P->nops = nops;
+
+    std::vector<uint8_t> img[2], res[2];
+    res[0].assign((size_t)(H / 64) * 1024, 0); res[1] = res[0];
     std::vector<uint2> fills;
     std::vector<uint32_t> sub;
-    std::vector<ChunkOp> chunks;
-    auto put = [](std::vector<uint8_t> &buf, uint32_t off, float v) { __half hv = __float2half_rn(v); memcpy(&buf[off], &hv, 2); };
+    auto put = [](std::vector<uint8_t> &buf, size_t off, float v) { __half hv = __float2half_rn(v); memcpy(&buf[off], &hv, 2); };
 
     // ---- streamed sub-tiles are appended to the open ring fill (<= slot bytes, in consumption order) ----
     uint32_t fill_start = 0, fill_bytes = 0;
@@ -563,122 +714,153 @@ int tc_pack_upload(const nqs_made *M) {
         sub.back() |= SUB_END;
         fill_bytes = 0;
     };
-    // reserve `bytes` of streamed image for the next sub-tile; pushes its table word, returns its image offset
     auto stream_alloc = [&](uint32_t bytes, uint32_t aux) -> uint32_t {
         if (fill_bytes + bytes > slot) close_fill();
         uint32_t w = (aux & 0xFFu) << SUB_AUX_SHIFT;
-        if (fill_bytes == 0) { fill_start = (uint32_t)img.size(); w |= SUB_NEW; }
+        if (fill_bytes == 0) { fill_start = (uint32_t)img[0].size(); w |= SUB_NEW; }
         w |= (fill_bytes >> 4) & SUB_OFF_MASK;
         const uint32_t base = fill_start + fill_bytes;
-        img.resize(img.size() + bytes, 0);
+        img[0].resize(img[0].size() + bytes, 0); img[1].resize(img[1].size() + bytes, 0);
         fill_bytes += bytes;
         sub.push_back(w);
         return base;
     };
 
-    // input-layer chunk c (layer 1 or phase hidden): D = A0 . Wc^T.  Masked layer-1 columns are the high ones
-    // (M1[j][d] = deg[j] >= d+1), so the K-steps to issue are a prefix.
+    // input-layer chunk c (layer 1 or phase hidden): rank r holds units 128 c + 64 r .. + 63.  Masked layer-1 columns
+    // are the high ones for sorted degrees; in general the issued K-steps are the prefix up to the last non-zero one.
     auto input_chunk = [&](int c, bool phase) {
         const uint32_t base = stream_alloc(in_bytes, 0);
         int nk = 1;                                             // the accumulator must be overwritten even if all zero
-        for (int r = 0; r < CH; ++r) {
-            const int j = c * CH + r;
-            for (int k = 0; k < KI; ++k) {
-                float v = 0.f;
-                if (phase) { if (k < n - 2) v = M->p1[(size_t)j * (n - 2) + k]; }
-                else if (k < n) v = M->wm[0][(size_t)j * n + k];
-                put(img, base + noswz_offset(r, k, KI), v);
-                if (v != 0.0f && k / 16 + 1 > nk) nk = k / 16 + 1;
+        for (int r = 0; r < 2; ++r)
+            for (int rr = 0; rr < HALF; ++rr) {
+                const int j = c * CN + r * HALF + rr;
+                for (int k = 0; k < KI; ++k) {
+                    float v = 0.f;
+                    if (phase) { if (k < n - 2) v = M->p1[(size_t)j * (n - 2) + k]; }
+                    else if (k < n) v = W1[(size_t)j * n + k];
+                    put(img[r], base + noswz_offset(rr, k, KI), v);
+                    if (v != 0.0f && k / 16 + 1 > nk) nk = k / 16 + 1;
+                }
             }
-        }
         sub.back() |= (uint32_t)nk << SUB_AUX_SHIFT;
-        P->mma_issued += nk; P->mma_dense += KI / 16;
-        ChunkOp co{};
-        co.bias_off = (uint16_t)((phase ? 0 : H) + c * CH);
-        co.kind = phase ? 1 : 0;
-        co.dst_col = (uint16_t)(c * (CH / 2));
-        chunks.push_back(co);
+        P->mma_issued += (long long)nk * CN; P->mma_dense += (long long)(KI / 16) * CN;
     };
-    // resident P2 tile of phase chunk c: rows 12..15 of a 16-row tile hold the 4 phase outputs
+    // resident P2 tile of phase chunk c: rows 12..15 of the 16-row tile hold the 4 phase outputs -> rank 1, rows 4..7
     auto phase_out_tile = [&](int c) {
         for (int o = 0; o < 4; ++o)
-            for (int k = 0; k < CH; ++k) put(res, (uint32_t)c * 2048 + sw128_offset(12 + o, k), M->p2[(size_t)o * H + c * CH + k]);
-        P->mma_issued += 4; P->mma_dense += 4;
+            for (int k = 0; k < CN; ++k)
+                put(res[1], (size_t)c * 2048 + (size_t)(k / 64) * 1024 + sw128_offset(4 + o, k % 64), M->p2[(size_t)o * H + c * CN + k]);
+        P->mma_issued += 8 * 16; P->mma_dense += 8 * 16;
     };
-    // streamed layer-3 tile of hidden chunk c; output rows below the first nonzero one receive exactly 0 from this
-    // chunk, so the MMA starts at a 16-row boundary n_lo (Mout[d][j] = d+1 > deg[j])
-    auto w3_tile = [&](int c) {
-        const uint32_t base = stream_alloc(w3_bytes, 0);
-        int row_lo = KO;
-        for (int d = 0; d < n; ++d)
-            for (int k = 0; k < CH; ++k) {
-                const float v = M->wm[2][(size_t)d * H + c * CH + k];
-                put(img, base + sw128_offset(d, k), v);
-                if (v != 0.0f && d < row_lo) row_lo = d;
-            }
-        const int n_lo = row_lo >= KO ? 0 : (row_lo / 16) * 16;
-        sub.back() |= (uint32_t)(n_lo / 16) << SUB_AUX_SHIFT;
-        P->mma_issued += 4; P->mma_dense += 4;
-    };
-
-    // ---- the per-tile schedule (must match the MMA issuer in eloc_tc_kernel) ----
-    for (int c = 0; c < NC; ++c) input_chunk(c, false);                          // stage A: layer 1 -> A1
-    for (int c = 0; c < NC; ++c) { input_chunk(c, true); phase_out_tile(c); }     // stage P: phase hidden, in place
-    uint8_t nblk[MAX_NC] = {0};
-    for (int c2 = 0; c2 < NC; ++c2) {                                             // stage C: layer 2 (TS), in place
-        int nb = 0;
-        for (int kb = 0; kb < NC; ++kb) {
-            bool any = false;
-            for (int r = 0; r < CH && !any; ++r)
-                for (int k = 0; k < CH; ++k)
-                    if (M->wm[1][(size_t)(c2 * CH + r) * H + kb * CH + k] != 0.0f) { any = true; break; }
-            P->mma_dense += 4;
-            if (!any && !(nb == 0 && kb == NC - 1)) continue;                     // exact: an all-zero block adds 0
-            const uint32_t base = stream_alloc(w2_bytes, (uint32_t)kb);
-            for (int r = 0; r < CH; ++r)
-                for (int k = 0; k < CH; ++k)
-                    put(img, base + sw128_offset(r, k), M->wm[1][(size_t)(c2 * CH + r) * H + kb * CH + k]);
-            P->mma_issued += 4;
+    // layer-2 chunk c2: k-blocks of 64 with any non-zero weight, and inside a block only the non-zero K-steps
+    auto l2_chunk = [&](int c2) {
+        const std::vector<float> &W2 = M->wm[1];
+        int nb = 0, need = 0;
+        for (int kb = 0; kb < H / 64; ++kb) {
+            uint32_t kmask = 0;
+            for (int r = 0; r < CN; ++r)
+                for (int k = 0; k < 64; ++k)
+                    if (W2[(size_t)(c2 * CN + r) * H + kb * 64 + k] != 0.0f) kmask |= 1u << (k / 16);
+            P->mma_dense += 4 * CN;
+            if (!kmask && !(nb == 0 && kb == H / 64 - 1)) continue;      // exact: an all-zero block adds 0
+            if (!kmask) kmask = 1;                                       // nothing at all: still overwrite the accumulator
+            const uint32_t base = stream_alloc(w2_bytes, (uint32_t)kb | (kmask << 4));
+            for (int r = 0; r < 2; ++r)
+                for (int rr = 0; rr < HALF; ++rr)
+                    for (int k = 0; k < 64; ++k)
+                        put(img[r], base + sw128_offset(rr, k), W2[(size_t)(c2 * CN + r * HALF + rr) * H + kb * 64 + k]);
+            P->mma_issued += (long long)__builtin_popcount(kmask) * CN;
+            need = kb / 2;
             ++nb;
         }
-        nblk[c2] = (uint8_t)nb;
-        ChunkOp co{};
-        co.bias_off = (uint16_t)(2 * H + c2 * CH); co.kind = 1; co.dst_col = 0;
-        chunks.push_back(co);
-        if (c2 >= 1) w3_tile(c2 - 1);                                             // consumer of the previous layer-2 chunk
-    }
-    w3_tile(NC - 1);
+        P->nblk[c2] = (uint8_t)nb; P->l2need[c2] = (uint8_t)need;
+    };
+    // streamed layer-3 tile of hidden chunk c: N = KO - n_lo output rows (rows below the first non-zero one receive
+    // exactly 0 from this chunk), rank r holds rows n_lo + r N/2 .. ; two K-blocks of N/2 rows x 128 B
+    auto w3_tile = [&](int c) {
+        int row_lo = KO;
+        for (int d = 0; d < n; ++d)
+            for (int k = 0; k < CN; ++k)
+                if (W3[(size_t)d * H + c * CN + k] != 0.0f && d < row_lo) row_lo = d;
+        const int n_lo = row_lo >= KO ? KO - 16 : (row_lo / 16) * 16;
+        const int N = KO - n_lo, Nh = N / 2;
+        const uint32_t base = stream_alloc((uint32_t)2 * Nh * 128, (uint32_t)(n_lo / 16));
+        for (int r = 0; r < 2; ++r)
+            for (int rr = 0; rr < Nh; ++rr) {
+                const int d = n_lo + r * Nh + rr;
+                if (d >= n) continue;
+                for (int k = 0; k < CN; ++k)
+                    put(img[r], base + (size_t)(k / 64) * Nh * 128 + sw128_offset(rr, k % 64), W3[(size_t)d * H + c * CN + k]);
+            }
+        P->mma_issued += (long long)8 * N; P->mma_dense += (long long)8 * KO;
+    };
+    auto emit_op = [&](int j) {
+        const int c = P->opchunk[j];
+        switch (P->optype[j]) {
+            case T_L1S: case T_L1I: input_chunk(c, false); break;
+            case T_P: input_chunk(c, true); phase_out_tile(c); break;
+            default: l2_chunk(c); break;
+        }
+    };
+    auto emit_consumer = [&](int j) {
+        if (P->optype[j] == T_L2 || P->optype[j] == T_L1I) w3_tile(P->opchunk[j]);
+    };
+    const int lag = sh.nacc - 1;
+    for (int j = 0; j < nops; ++j) { emit_op(j); if (j >= lag) emit_consumer(j - lag); }
+    for (int m = lag; m >= 1; --m) if (nops >= m) emit_consumer(nops - m);
     close_fill();
-    P->nsub = (int)sub.size(); P->nchunks = (int)chunks.size(); P->nfills = (int)fills.size();
-    P->res_bytes = (uint32_t)res.size();
-    if (P->nsub > MAX_SUB || (P->nchunks & 1)) { delete P; return NQS_EUNSUPPORTED; }
+    // ---- where the issuer waits for chunk epilogues that have no consumer MMA (layer-1 chunks written to A1): before
+    // the accumulator's next producer or the first layer-2 op that reads the chunk, whichever is issued first ----
+    if (L == 2) P->l2need[NC - 1] = (uint8_t)(NC - 1);          // every layer-1 epilogue is waited for inside its own tile
+    {
+        int pending[3] = {-1, -1, -1};
+        auto consumed = [&](int j) { if (P->optype[j] != T_L1S && pending[j % sh.nacc] == j) pending[j % sh.nacc] = -1; };
+        for (int j = 0; j < nops; ++j) {
+            const int a = j % sh.nacc;
+            uint8_t pw = 0;
+            if (pending[a] >= 0) { pw |= (uint8_t)(1u << a); pending[a] = -1; }
+            if (P->optype[j] == T_L2)
+                for (int cn = 0; cn <= P->l2need[P->opchunk[j]]; ++cn)
+                    if (pending[cn % sh.nacc] == cn) { pw |= (uint8_t)(1u << (cn % sh.nacc)); pending[cn % sh.nacc] = -1; }
+            P->prewait[j] = pw;
+            pending[a] = j;
+            if (j >= lag) consumed(j - lag);
+        }
+        for (int m = lag; m >= 1; --m) if (nops >= m) consumed(nops - m);
+        if (pending[0] >= 0 || pending[1] >= 0 || pending[2] >= 0) { delete P; return NQS_EUNSUPPORTED; }
+        for (int a = 0; a < sh.nacc; ++a) {
+            int cnt = 0;
+            for (int j = a; j < nops; j += sh.nacc) ++cnt;
+            if (cnt & 1) P->cntmask |= 1u << a;
+        }
+    }
+    P->nsub = (int)sub.size(); P->nfills = (int)fills.size();
+    P->res_bytes = (uint32_t)res[0].size();
+    if (P->nsub > MAX_SUB) { delete P; return NQS_EUNSUPPORTED; }
     memcpy(P->sub, sub.data(), sub.size() * 4);
-    memcpy(P->nblk, nblk, sizeof(nblk));
+    P->img_stride = (uint32_t)((img[0].size() + 255) & ~(size_t)255);
 
     // biases: [c1 | b1 | b2 | b3 (KO) | c2]
     std::vector<float> bias((size_t)3 * H + KO + 4, 0.f);
-    for (int j = 0; j < H; ++j) { bias[j] = M->c1[j]; bias[H + j] = M->bias[0][j]; bias[2 * H + j] = M->bias[1][j]; }
-    for (int d = 0; d < n; ++d) bias[3 * H + d] = M->bias[2][d];
+    for (int j = 0; j < H; ++j) { bias[j] = M->c1[j]; bias[H + j] = M->bias[0][j]; if (L == 2) bias[2 * H + j] = M->bias[1][j]; }
+    for (int d = 0; d < n; ++d) bias[3 * H + d] = M->bias[L][d];
     for (int o = 0; o < 4; ++o) bias[3 * H + KO + o] = M->c2[o];
 
+    std::vector<uint8_t> wboth((size_t)2 * P->img_stride, 0), rboth((size_t)2 * P->res_bytes, 0);
+    for (int r = 0; r < 2; ++r) {
+        memcpy(&wboth[(size_t)r * P->img_stride], img[r].data(), img[r].size());
+        memcpy(&rboth[(size_t)r * P->res_bytes], res[r].data(), res[r].size());
+    }
     int dev = 0; cudaGetDevice(&dev);
     cudaDeviceGetAttribute(&P->sms, cudaDevAttrMultiProcessorCount, dev);
     auto up = [](void **dst, const void *src, size_t bytes) {
         return cudaMalloc(dst, bytes ? bytes : 16) == cudaSuccess && (bytes == 0 || cudaMemcpy(*dst, src, bytes, cudaMemcpyHostToDevice) == cudaSuccess);
     };
-    bool ok = up(&P->d_wimg, img.data(), img.size()) && up(&P->d_fills, fills.data(), fills.size() * sizeof(uint2)) &&
-              up(&P->d_chunks, chunks.data(), chunks.size() * sizeof(ChunkOp)) &&
-              up(&P->d_res, res.data(), res.size()) && up(&P->d_bias, bias.data(), bias.size() * 4);
-    {   // the attribute belongs to the kernel, not to the model: keep the largest request
-        static int max_smem = 0;
-        if ((int)P->L.total > max_smem) {
-            ok = ok && cudaFuncSetAttribute(eloc_tc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)P->L.total) == cudaSuccess;
-            if (ok) max_smem = (int)P->L.total;
-        }
-    }
+    const bool ok = up(&P->d_wimg, wboth.data(), wboth.size()) && up(&P->d_fills, fills.data(), fills.size() * sizeof(uint2)) &&
+                    up(&P->d_res, rboth.data(), rboth.size()) && up(&P->d_bias, bias.data(), bias.size() * 4);
     if (!ok) {
         cudaGetLastError();
-        cudaFree(P->d_wimg); cudaFree(P->d_fills); cudaFree(P->d_chunks); cudaFree(P->d_res); cudaFree(P->d_bias);
+        cudaFree(P->d_wimg); cudaFree(P->d_fills); cudaFree(P->d_res); cudaFree(P->d_bias);
         delete P;
         return NQS_ECUDA;
     }
@@ -689,7 +871,7 @@ int tc_pack_upload(const nqs_made *M) {
 void tc_pack_free(const nqs_made *M) {
     if (!M->tc) return;
     TcPack *P = M->tc;
-    cudaFree(P->d_wimg); cudaFree(P->d_fills); cudaFree(P->d_chunks); cudaFree(P->d_res); cudaFree(P->d_bias);
+    cudaFree(P->d_wimg); cudaFree(P->d_fills); cudaFree(P->d_res); cudaFree(P->d_bias);
     if (P->d_fpos) cudaFree(P->d_fpos);
     if (P->d_xpos) cudaFree(P->d_xpos);
     delete P;
@@ -703,11 +885,14 @@ void tc_mma_counts(const nqs_made *M, long long *issued, long long *dense) {
 
 static void fill_common(const nqs_made *M, TcParams &p) {
     const TcPack *P = M->tc;
-    p.n = M->n; p.H = M->h; p.NC = P->NC; p.KI = P->KI; p.KO = P->KO;
-    p.tm_d = P->tm_d; p.tm_d3 = P->tm_d3;
-    p.wimg = (const uint8_t *)P->d_wimg; p.fills = (const uint2 *)P->d_fills; p.nfills = P->nfills;
-    memcpy(p.sub, P->sub, sizeof(p.sub)); memcpy(p.nblk, P->nblk, sizeof(p.nblk));
-    p.chunks = (const ChunkOp *)P->d_chunks; p.nchunks = P->nchunks;
+    p.n = M->n; p.H = M->h; p.NC = P->NC; p.KI = P->KI; p.KO = P->KO; p.L = M->L; p.nacc = P->nacc; p.nops = P->nops;
+    p.last_a0_op = P->last_a0_op; p.last_l2_op = P->last_l2_op;
+    p.tm_d3 = P->tm_d3; p.tm_a0 = P->tm_a0;
+    p.wimg = (const uint8_t *)P->d_wimg; p.img_stride = P->img_stride;
+    p.fills = (const uint2 *)P->d_fills; p.nfills = P->nfills;
+    memcpy(p.sub, P->sub, sizeof(p.sub)); memcpy(p.nblk, P->nblk, sizeof(p.nblk)); memcpy(p.l2need, P->l2need, sizeof(p.l2need));
+    memcpy(p.optype, P->optype, sizeof(p.optype)); memcpy(p.opchunk, P->opchunk, sizeof(p.opchunk));
+    memcpy(p.prewait, P->prewait, sizeof(p.prewait)); p.cntmask = P->cntmask;
     p.resimg = (const uint8_t *)P->d_res; p.res_bytes = P->res_bytes;
     p.slot_bytes = P->slot_bytes; p.nslots = P->nslots;
     p.bias = (const float *)P->d_bias;
@@ -728,6 +913,44 @@ static int permuted(const nqs_made *M, const ulonglong2 *in, long long N, ulongl
     return cudaGetLastError() == cudaSuccess ? NQS_OK : NQS_ECUDA;
 }
 
+#ifdef TC_PROF
+long long *g_tc_prof = nullptr;   // [148][16], set by the profiling harness through nqs_tc_prof_buffer()
+extern "C" void nqs_tc_prof_buffer(long long *dev_buf) { g_tc_prof = dev_buf; }
+#endif
+
+template <int NC, int L, int NACC>
+static int launch_inst(const TcParams &p, int grid, uint32_t smem_bytes, cudaStream_t st) {
+    // the attribute is per device and per kernel; setting it is a cheap host call, so no process-wide cache
+    if (cudaFuncSetAttribute(eloc_tc_kernel<NC, L, NACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes) != cudaSuccess) {
+        cudaGetLastError();
+        return NQS_ECUDA;
+    }
+    eloc_tc_kernel<NC, L, NACC><<<grid, NTHREADS, smem_bytes, st>>>(p);
+    return NQS_OK;
+}
+
+static int launch_chain(const TcPack *P, TcParams &p, long long ntiles, cudaStream_t st) {
+#ifdef TC_PROF
+    p.prof = g_tc_prof;
+#endif
+    const long long npairs = (ntiles + 1) / 2;
+    const long long ncl_max = P->sms / 2;
+    const int grid = 2 * (int)(npairs < ncl_max ? npairs : ncl_max);
+    int rc = NQS_EUNSUPPORTED;
+#define TC_CASE(NC_, L_, NA_) case (NC_ * 16 + L_ * 4 + NA_): rc = launch_inst<NC_, L_, NA_>(p, grid, P->L.total, st); break;
+    switch (p.NC * 16 + p.L * 4 + p.nacc) {
+        TC_CASE(1, 1, 2) TC_CASE(2, 1, 2) TC_CASE(3, 1, 2) TC_CASE(4, 1, 2)
+        TC_CASE(1, 2, 2) TC_CASE(2, 2, 2) TC_CASE(3, 2, 2) TC_CASE(4, 2, 2)
+        TC_CASE(1, 1, 3) TC_CASE(2, 1, 3) TC_CASE(3, 1, 3) TC_CASE(4, 1, 3)
+        TC_CASE(1, 2, 3) TC_CASE(2, 2, 3) TC_CASE(3, 2, 3) TC_CASE(4, 2, 3)
+        default: break;
+    }
+#undef TC_CASE
+    if (rc) return rc;
+    ++g_launch_count;
+    return cudaGetLastError() == cudaSuccess ? NQS_OK : NQS_ECUDA;
+}
+
 int launch_logpsi_tc(const nqs_made *M, const ulonglong2 *cfg, long long B, float2 *out, cudaStream_t st) {
     if (B <= 0) return NQS_OK;
     TcPack *P = M->tc;
@@ -738,17 +961,13 @@ int launch_logpsi_tc(const nqs_made *M, const ulonglong2 *cfg, long long B, floa
     TcParams p{};
     fill_common(M, p);
     p.mode = 0; p.xpos = (const ulonglong2 *)P->d_xpos; p.B = B; p.out = out;
-    const long long ntiles = (B + TILE_M - 1) / TILE_M;
-    const int grid = (int)(ntiles < P->sms ? ntiles : P->sms);
-    eloc_tc_kernel<<<grid, NTHREADS, P->L.total, st>>>(p);
-    ++g_launch_count;
-    return cudaGetLastError() == cudaSuccess ? NQS_OK : NQS_ECUDA;
+    return launch_chain(P, p, (B + TILE_M - 1) / TILE_M, st);
 }
 
 size_t eloc_tc_ws_bytes(long long, const HamDev &) { return 256; }
 
 int launch_eloc_tc(const HamDev &hm, const nqs_made *M, const ulonglong2 *x, const float2 *base, long long B,
-                   float2 *eloc, unsigned *max_ratio_bits, cudaStream_t st) {
+                    float2 *eloc, unsigned *max_ratio_bits, cudaStream_t st) {
     if (B <= 0) return NQS_OK;
     TcPack *P = M->tc;
     if (!P) return NQS_EUNSUPPORTED;
@@ -770,11 +989,6 @@ int launch_eloc_tc(const HamDev &hm, const nqs_made *M, const ulonglong2 *x, con
     p.g_begin = hm.has_diag ? 1 : 0;
     const long long nsb = (B + TILE_M - 1) / TILE_M;
     const long long ntiles = nsb * (hm.G - p.g_begin);
-    if (ntiles > 0) {
-        const int grid = (int)(ntiles < P->sms ? ntiles : P->sms);
-        eloc_tc_kernel<<<grid, NTHREADS, P->L.total, st>>>(p);
-        ++g_launch_count;
-        if (cudaGetLastError() != cudaSuccess) return NQS_ECUDA;
-    }
+    if (ntiles > 0) return launch_chain(P, p, ntiles, st);
     return NQS_OK;
 }

@@ -49,8 +49,7 @@ struct nqs_ham {
     mutable void *d_flips = nullptr, *d_offsets = nullptr, *d_zy = nullptr, *d_cph = nullptr;
 };
 
-struct TcPack;   // tensor-core weight tiles (kernels_tc.cu)
-struct Tc2Pack;  // CTA-pair tensor-core weight tiles (kernels_tc2.cu)
+struct TcPack;   // tensor-core weight tiles of the CTA-pair kernel (kernels_tc.cu)
 
 struct nqs_made {
     int n = 0, h = 0, L = 0, npad = 0;
@@ -65,7 +64,6 @@ struct nqs_made {
     mutable std::vector<void *> d_allocs;
     mutable MadeDev dev{};
     mutable TcPack *tc = nullptr;
-    mutable Tc2Pack *tc2 = nullptr;
     // workspace (grown on demand, reused across calls)
     mutable void  *ws = nullptr;
     mutable size_t ws_bytes = 0;
@@ -101,11 +99,3 @@ int  launch_eloc_tc(const HamDev &hm, const nqs_made *made, const ulonglong2 *x,
 size_t eloc_tc_ws_bytes(long long B, const HamDev &hm);
 void tc_mma_counts(const nqs_made *made, long long *issued, long long *dense);   // K-steps per tile: issued / dense chain
 
-// kernels_tc2.cu (CTA-pair kernel)
-bool tc2_supported(const nqs_made *made);
-int  tc2_pack_upload(const nqs_made *made);
-void tc2_pack_free(const nqs_made *made);
-int  launch_logpsi_tc2(const nqs_made *made, const ulonglong2 *cfg, long long B, float2 *out, cudaStream_t st);
-int  launch_eloc_tc2(const HamDev &hm, const nqs_made *made, const ulonglong2 *x, const float2 *base, long long B,
-                     float2 *eloc, unsigned *max_ratio_bits, cudaStream_t st);
-void tc2_mma_counts(const nqs_made *made, long long *issued, long long *dense);

@@ -64,7 +64,12 @@ def _paths(M, min_hidden_tc=384):
 
 @pytest.mark.parametrize("n,h,L,order", [(8, 32, 2, "reverse"), (20, 128, 2, "reverse"), (30, 256, 2, "identity"),
                                          (76, 512, 2, "reverse"), (13, 48, 1, "random"), (128, 64, 2, "random"),
-                                         (65, 16, 2, "reverse"), (3, 8, 1, "identity")])
+                                         (65, 16, 2, "reverse"), (3, 8, 1, "identity"),
+                                         # tensor-core shape limits: one hidden layer (the paper's own architecture,
+                                         # PAPER.md:84), n = 3 / 77 (two accumulators) / 96 / 112 / 128, odd chunk counts
+                                         (30, 128, 1, "identity"), (52, 512, 1, "reverse"), (76, 384, 1, "random"),
+                                         (3, 128, 2, "identity"), (77, 512, 2, "reverse"), (96, 512, 2, "random"),
+                                         (112, 512, 2, "reverse"), (128, 512, 2, "random"), (128, 384, 1, "reverse")])
 def test_logpsi_parity(n, h, L, order):
     p = wl.make_made_params(n, h, 100 + n, n_hidden_layers=L, order=order)
     rng = np.random.default_rng(n)
@@ -81,7 +86,7 @@ def test_logpsi_parity(n, h, L, order):
     assert nqs.made_logpsi(M, torch.zeros((0, 2), dtype=torch.int64, device=DEV)).shape == (0, 2)   # B = 0
 
 
-@pytest.mark.parametrize("n,h", [(20, 128), (76, 128), (40, 256), (76, 512)])
+@pytest.mark.parametrize("n,h", [(20, 128), (76, 128), (40, 256), (76, 512), (100, 384)])
 def test_logpsi_tensor_core_many_tiles_per_cta(n, h):
     """Persistent-kernel paths that a few-tile launch never reaches: every CTA walks several 128-row tiles, so
     the weight ring wraps, the double-buffered operand tile and every barrier parity are re-used (a producer
