@@ -12,6 +12,7 @@ Rules:
     what the paper's definition states (chunking over terms only bounds memory);
   * every function is pinned in tests/test_oracle_*.py to something other than itself (dense
     Kronecker matrices, Slater-Condon, normalisation over 2^n, closed forms).
-    Parity unpinned: the phase-MLP output o(x) itself (direct formula only; its selector and its
-    independence from the last two inputs ARE pinned) — SURVEY.md §8(c).
+    Every function has such a pin: the phase net, "parity unpinned" in round 1, is pinned through an independent
+    torch fp64 evaluation and a position-order test (tests/test_oracle_made.py); oracle.grad (Eq. 7) by
+    finite differences, torch autograd and exact enumeration against the dense Hamiltonian (tests/test_oracle_grad.py).
 """
