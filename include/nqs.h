@@ -165,6 +165,31 @@ int nqs_local_energy_host(const nqs_ham_t *ham, const nqs_made_t *made, const ui
                           const int64_t *counts_host, int64_t B, int64_t minibatch, int path,
                           float *eloc_out_host, double *stats_out_host);
 
+/* ---- gradient of the energy objective: PAPER.md:71 Eq. 7, :73 (baseline), :202 (accumulation) ----------
+ *   grad L(theta) = Re E[(l_theta(x) - b) conj(grad_theta log f(x))],   b = E[l_theta(x)],
+ * the expectation taken over the unique samples weighted by their multiplicities (:105, :200).  log f = log|psi| + i phi
+ * (:96 Eq. 10), so the MADE parameters receive Re(E - b) through log|psi|, the phase-net parameters Im(E - b) through phi.
+ *
+ * nqs_made_num_params : number of parameters = length of the flat gradient.  Flat order: for k = 0..n_hidden_layers:
+ *   W_k (row-major [out][in]) then b_k; then P1 [hidden][n-2], c1 [hidden], P2 [4][hidden], c2 [4] -- the tensors of
+ *   nqs_made_create in its argument order.  The gradient is with respect to the UNMASKED weights nqs_made_create takes:
+ *   masked entries receive exactly 0.
+ * nqs_energy_grad :
+ *   samples_dev  device uint64 [B][2];  counts_dev device int64 [B] or NULL (= ones);
+ *   eloc_dev     device float [B][2], the local energies of these samples (the output of nqs_local_energy);
+ *   minibatch    rows per accumulation pass (0 = 8192): bounds the workspace (~ 6 * hidden * minibatch floats);
+ *   global_stats_host  NULL, or host double [3] = { sum n, sum n Re E, sum n Im E } over the samples of ALL
+ *                data-parallel replicas (:146): b and the normalisation are then taken from it, so that the SUM of the
+ *                replicas' gradients is the gradient of the whole batch (paper_2208_05637_b200/distributed.py);
+ *   grad_out_dev device float [n_params], overwritten;
+ *   baseline_out_host host double [2] = (Re b, Im b) or NULL; when non-NULL the call synchronises the stream.
+ * fp32 on CUDA cores (the B sampled rows are ~1e-5 of the E_loc work), fixed reduction order: bit-reproducible.
+ * B = 0 gives a zero gradient. */
+int nqs_made_num_params(const nqs_made_t *made, int64_t *n_params);
+int nqs_energy_grad(const nqs_made_t *made, const uint64_t *samples_dev, const int64_t *counts_dev,
+                    const float *eloc_dev, int64_t B, int64_t minibatch, const double *global_stats_host,
+                    float *grad_out_dev, double *baseline_out_host, void *cuda_stream);
+
 /* Number of kernels this library has launched in the calling process since load (monotonic). */
 int64_t nqs_kernel_launch_count(void);
 

@@ -50,6 +50,8 @@ def lib():
                                        c_void_p, c_void_p, c_void_p]
         L.nqs_local_energy_host.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int64, c_int64, c_int,
                                             c_void_p, c_void_p]
+        L.nqs_made_num_params.argtypes = [c_void_p, ctypes.POINTER(c_int64)]
+        L.nqs_energy_grad.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int64, c_int64, c_void_p, c_void_p, c_void_p, c_void_p]
         L.nqs_kernel_launch_count.restype = c_int64
         L.nqs_kernel_launch_count.argtypes = []
         L.nqs_last_chain_kernel_ms.argtypes = [c_void_p, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(c_int)]
@@ -126,6 +128,11 @@ class Made:
         if r < 0:
             raise NqsError(r, "nqs_made_path")
         return r
+
+    def num_params(self):
+        k = c_int64()
+        _chk(lib().nqs_made_num_params(self._h, k), "nqs_made_num_params")
+        return k.value
 
     def last_chain_kernel_ms(self):
         ms, k = ctypes.c_float(), c_int()
@@ -214,6 +221,20 @@ def local_energy_host(ham, made, samples, counts=None, minibatch=0, path=PATH_AU
                                      B, minibatch, path, out.ctypes.data, stats.ctypes.data if want_stats else None),
          "nqs_local_energy_host")
     return out, stats
+
+
+def energy_grad(made, samples, counts, eloc, minibatch=0, want_baseline=True, stream=None, global_stats=None):
+    """Gradient of Eq. 7.  samples torch.int64 CUDA [B, 2], counts torch.int64 CUDA [B] or None, eloc torch.float32 CUDA
+    [B, 2] -> (grad torch.float32 [n_params], baseline complex or None)."""
+    import torch
+    B = samples.shape[0]
+    grad = torch.empty((made.num_params(),), dtype=torch.float32, device=samples.device)
+    base = np.zeros(2, np.float64) if want_baseline else None
+    gs = _np(global_stats, np.float64) if global_stats is not None else None
+    _chk(lib().nqs_energy_grad(made._h, samples.data_ptr(), counts.data_ptr() if counts is not None else None,
+                               eloc.data_ptr(), B, minibatch, gs.ctypes.data if gs is not None else None, grad.data_ptr(),
+                               base.ctypes.data if want_baseline else None, _stream_ptr(stream)), "nqs_energy_grad")
+    return grad, (complex(base[0], base[1]) if want_baseline else None)
 
 
 def kernel_launch_count():

@@ -134,6 +134,7 @@ extern "C" void nqs_made_free(nqs_made_t *M) {
     if (M->ws) cudaFree(M->ws);
     for (cudaEvent_t e : M->ev) cudaEventDestroy(e);
     tc_pack_free(M);
+    grad_pack_free(M);
     delete M;
 }
 

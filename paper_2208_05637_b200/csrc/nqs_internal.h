@@ -50,6 +50,7 @@ struct nqs_ham {
 };
 
 struct TcPack;   // tensor-core weight tiles of the CTA-pair kernel (kernels_tc.cu)
+struct GradPack; // degree tables + workspace of the gradient path (kernels_grad.cu)
 
 struct nqs_made {
     int n = 0, h = 0, L = 0, npad = 0;
@@ -64,6 +65,7 @@ struct nqs_made {
     mutable std::vector<void *> d_allocs;
     mutable MadeDev dev{};
     mutable TcPack *tc = nullptr;
+    mutable GradPack *grad = nullptr;
     // workspace (grown on demand, reused across calls)
     mutable void  *ws = nullptr;
     mutable size_t ws_bytes = 0;
@@ -99,3 +101,5 @@ int  launch_eloc_tc(const HamDev &hm, const nqs_made *made, const ulonglong2 *x,
 size_t eloc_tc_ws_bytes(long long B, const HamDev &hm);
 void tc_mma_counts(const nqs_made *made, long long *issued, long long *dense);   // K-steps per tile: issued / dense chain
 
+// kernels_grad.cu
+void grad_pack_free(const nqs_made *made);

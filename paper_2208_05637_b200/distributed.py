@@ -1,8 +1,11 @@
 """Data-parallel plumbing of the E_loc path (the model and the Hamiltonian tensors are
 replicated on every GPU, the batch of unique samples is split; the only exchange is the reduction of the
 per-rank statistics).  One process per GPU under `torch.distributed` (NCCL on the GPUs, gloo in the CPU tests).
-No arithmetic of the method lives here: row partitions, the mini-batch a rank takes at a step, and the
-reduction of the five statistics `[sum n, sum n Re E, sum n Im E, sum n |E|^2, max |ratio|]` (include/nqs.h).
+No arithmetic of the method lives here: row partitions, the mini-batch a rank takes at a step, the
+reduction of the five statistics `[sum n, sum n Re E, sum n Im E, sum n |E|^2, max |ratio|]` (include/nqs.h), and
+the gradient exchange of PAPER.md:146 ("gradients from each node are averaged"): every rank evaluates Eq. 7 on its
+shard with the GLOBAL baseline and normalisation (`global_stats` of nqs_energy_grad), so the all-reduce SUM of the
+per-rank gradients is the gradient of the whole batch.
 """
 import torch
 import torch.distributed as dist
@@ -41,3 +44,11 @@ def max_over_ranks(value: float, device="cpu", group=None) -> float:
     if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
         dist.all_reduce(t, op=dist.ReduceOp.MAX, group=group)
     return float(t.item())
+
+
+def all_reduce_gradient(grad, group=None):
+    """Sum the per-rank gradients in place (each computed with the global statistics, see module docstring).
+    `grad` is a float tensor on the backend's device."""
+    if dist.is_available() and dist.is_initialized() and dist.get_world_size(group) > 1:
+        dist.all_reduce(grad, op=dist.ReduceOp.SUM, group=group)
+    return grad

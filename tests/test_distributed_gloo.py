@@ -18,8 +18,10 @@ if ROOT not in sys.path:
     sys.path.insert(0, ROOT)
 
 from paper_2208_05637_b200 import workloads as wl
-from paper_2208_05637_b200.distributed import all_reduce_stats, max_over_ranks, minibatch_of_step, shard_rows
+from paper_2208_05637_b200.distributed import (all_reduce_gradient, all_reduce_stats, max_over_ranks, minibatch_of_step,
+                                               shard_rows)
 from oracle import eloc as oeloc
+from oracle import grad as ograd
 
 
 def _free_port():
@@ -49,6 +51,13 @@ def _worker(rank, world, port, out_dir):
         all_reduce_stats(stats)
         slowest = max_over_ranks(10.0 + rank)
         np.save(os.path.join(out_dir, f"rank{rank}.npy"), np.concatenate([stats.numpy(), [slowest, lo, hi]]))
+        # gradient exchange: Eq. 7 on the shard with the GLOBAL baseline / normalisation, then a SUM
+        tot, b = stats[0].item(), complex(stats[1].item(), stats[2].item()) / stats[0].item()
+        cs = counts[lo:hi].astype(np.float64)
+        g = ograd.flatten(ograd.dlogpsi_weighted(params, samples[lo:hi], cs * (e.real - b.real) / tot, cs * (e.imag - b.imag) / tot))
+        g = torch.from_numpy(g)
+        all_reduce_gradient(g)
+        np.save(os.path.join(out_dir, f"grad{rank}.npy"), g.numpy())
     finally:
         dist.destroy_process_group()
 
@@ -64,6 +73,10 @@ def test_two_rank_statistics_equal_unsharded(tmp_path):
         assert got[r][4] == 2.0                                                      # max |ratio| over ranks
         assert got[r][5] == 11.0                                                     # timing rule: max over ranks
     assert (got[0][6], got[0][7], got[1][6], got[1][7]) == (0, 18, 18, 37)           # contiguous, disjoint, complete
+    # the summed per-rank gradients equal Eq. 7 on the whole batch
+    gref, _ = ograd.energy_gradient(params, samples, counts, oeloc.local_energy(codes, c, params, samples))
+    for r in range(world):
+        np.testing.assert_allclose(np.load(tmp_path / f"grad{r}.npy"), gref, rtol=1e-11, atol=1e-13)
 
 
 def test_partitions_and_step_schedule():

@@ -440,3 +440,102 @@ def test_pauli_contract_output_layout_raw_ctypes():
         cc = t["coef"][sl].astype(np.float64)
         ref = (cc[None, :] * matrix_element(samples[:, None, :], t["zy"][sl][None, :, :], t["ycount"][sl].astype(np.int64))).sum(axis=1)
         np.testing.assert_allclose(S[gi - g0, :, 0] + 1j * S[gi - g0, :, 1], ref, atol=1e-5 * np.abs(cc).sum())
+
+
+# ---- gradient of Eq. 7 -----------------------------------------------------------------------------
+def _grad_tensor_slices(p):
+    sizes = []
+    for W, b in zip(p.weights, p.biases):
+        sizes += [W.size, b.size]
+    sizes += [p.phase_weights[0].size, p.phase_biases[0].size, p.phase_weights[1].size, p.phase_biases[1].size]
+    offs = np.concatenate([[0], np.cumsum(sizes)])
+    return [slice(int(offs[i]), int(offs[i + 1])) for i in range(len(sizes))]
+
+
+def _check_grad(params, samples, counts, eloc_c64, minibatch, tag):
+    """CUDA gradient against oracle.grad on the SAME (fp32) local energies.  Tolerance per parameter tensor: the kernel
+    forms each entry as an fp32 sum over the B rows of products of fp32 activations (relative error ~ sqrt(B) 2^-24 on
+    sum |terms|, far below the bound) -- bound 2e-5 * max|g| of the tensor + 1e-9."""
+    from oracle import grad as ograd
+    M = nqs.made_create(params)
+    e32 = np.stack([eloc_c64.real, eloc_c64.imag], axis=1).astype(np.float32)
+    g, b = nqs.energy_grad(M, _dev_u64(samples), torch.from_numpy(counts).to(DEV) if counts is not None else None,
+                           torch.from_numpy(e32).to(DEV), minibatch=minibatch)
+    g = g.cpu().numpy().astype(np.float64)
+    cnt = counts if counts is not None else np.ones(len(samples))
+    ref, bref = ograd.energy_gradient(params, samples, cnt, e32[:, 0].astype(np.float64) + 1j * e32[:, 1].astype(np.float64))
+    assert g.shape == ref.shape == (M.num_params(),)
+    assert abs(b - bref) <= 1e-12 * max(1.0, abs(bref))
+    worst = 0.0
+    for t, sl in enumerate(_grad_tensor_slices(params)):
+        scale = np.abs(ref[sl]).max()
+        err = np.abs(g[sl] - ref[sl]).max()
+        worst = max(worst, err / (scale + 1e-30))
+        assert err <= 2e-5 * scale + 1e-9, (tag, t, err, scale)
+    # masked entries are exactly zero
+    masks = omade.build_masks(params.n_qubits, params.deg_hidden)
+    sls = _grad_tensor_slices(params)
+    for k, mk in enumerate(masks):
+        assert np.all(g[sls[2 * k]].reshape(mk.shape)[mk == 0] == 0.0)
+    print(f"[parity] gradient {tag}: max rel err over tensors {worst:.2e}")
+    return g
+
+
+@pytest.mark.parametrize("cfg,B,mb", [(1, 256, 100), (2, 4096, 1500), (3, 3000, 0)])
+def test_energy_gradient_all_samples(cfg, B, mb):
+    """Every sample of cfg 1-2 (3,000 of cfg 3), all parameter tensors, E_loc from the library itself (AUTO path), with
+    gradient-accumulation mini-batches that do not divide B."""
+    w, (x, z, c), params, H, M = workload(cfg)
+    samples, counts = wl.make_samples(w.n_spatial, w.n_alpha, w.n_beta, B, w.max_count, w.seed_samples, w.unique)
+    e, _ = nqs.local_energy(H, M, _dev_u64(samples), torch.from_numpy(counts).to(DEV))
+    e = e.cpu().numpy().astype(np.float64)
+    _check_grad(params, samples, counts, e[:, 0] + 1j * e[:, 1], mb, f"cfg {cfg}")
+
+
+def test_energy_gradient_cfg5_sampled_rows_and_complex_energies():
+    """cfg 5 shape (76 qubits, h = 512): 700 samples with synthetic COMPLEX local energies (so that the phase-net
+    tensors get a non-zero gradient), unit counts, two mini-batches."""
+    w = wl.WORKLOADS[5]
+    params = wl.make_made_params(w.n_qubits, w.hidden, w.seed_weights)
+    samples, _ = wl.make_samples(w.n_spatial, w.n_alpha, w.n_beta, 700, w.max_count, w.seed_samples, w.unique)
+    rng = np.random.default_rng(55)
+    e = -300.0 + rng.standard_normal(700) + 1j * rng.standard_normal(700)
+    g = _check_grad(params, samples, None, e, 512, "cfg 5 shape, complex E")
+    sls = _grad_tensor_slices(params)
+    assert np.abs(g[sls[-4]]).max() > 0 and np.abs(g[sls[-2]]).max() > 0      # P1, P2 gradients are exercised
+
+
+@pytest.mark.parametrize("n,h,L,order", [(13, 48, 1, "random"), (65, 100, 2, "random"), (128, 64, 2, "reverse"), (3, 8, 1, "identity")])
+def test_energy_gradient_shapes(n, h, L, order):
+    """One hidden layer (the paper's own architecture), random degrees, widths that are not multiples of the tile."""
+    p = wl.make_made_params(n, h, 200 + n, n_hidden_layers=L, order=order)
+    rng = np.random.default_rng(n)
+    p.deg_hidden = rng.integers(1, n, size=(L, h)).astype(np.int32)
+    samples = wl.pack_bits(rng.integers(0, 2, size=(333, n)).astype(np.uint8))
+    counts = rng.integers(1, 50, size=333).astype(np.int64)
+    e = rng.standard_normal(333) + 1j * rng.standard_normal(333)
+    _check_grad(p, samples, counts, e, 128, f"n={n} h={h} L={L}")
+    # B = 0
+    M = nqs.made_create(p)
+    g0, _ = nqs.energy_grad(M, _dev_u64(samples[:0]), None, torch.zeros((0, 2), device=DEV))
+    assert torch.all(g0 == 0)
+
+
+def test_energy_gradient_global_stats_shards_sum_to_whole_batch():
+    """nqs_energy_grad(global_stats_host = ...) on two shards: the SUM equals the gradient of the whole batch
+    (the data-parallel exchange of PAPER.md:146, distributed.all_reduce_gradient)."""
+    p = wl.make_made_params(20, 128, 5)
+    rng = np.random.default_rng(12)
+    samples = wl.pack_bits(rng.integers(0, 2, size=(500, 20)).astype(np.uint8))
+    counts = rng.integers(1, 30, size=500).astype(np.int64)
+    e = (rng.standard_normal((500, 2)) + np.array([-20.0, 0.0])).astype(np.float32)
+    M = nqs.made_create(p)
+    xs, cs, es = _dev_u64(samples), torch.from_numpy(counts).to(DEV), torch.from_numpy(e).to(DEV)
+    g_all, b_all = nqs.energy_grad(M, xs, cs, es)
+    cd = counts.astype(np.float64)
+    gstats = np.array([cd.sum(), (cd * e[:, 0]).sum(), (cd * e[:, 1]).sum()])
+    g0, b0 = nqs.energy_grad(M, xs[:180], cs[:180], es[:180], global_stats=gstats)
+    g1, b1 = nqs.energy_grad(M, xs[180:], cs[180:], es[180:], global_stats=gstats, minibatch=100)
+    assert abs(b0 - b_all) < 1e-12 and abs(b1 - b_all) < 1e-12
+    d = (g0 + g1 - g_all).abs().max().item()
+    assert d <= 2e-6 * g_all.abs().max().item() + 1e-10, d
