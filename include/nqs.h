@@ -190,6 +190,28 @@ int nqs_energy_grad(const nqs_made_t *made, const uint64_t *samples_dev, const i
                     const float *eloc_dev, int64_t B, int64_t minibatch, const double *global_stats_host,
                     float *grad_out_dev, double *baseline_out_host, void *cuda_stream);
 
+/* ---- batched autoregressive sampler: PAPER.md:105-107, :109-120, :136-142 (Eq. 11-14) -----------------------
+ * "keep track of a sample buffer ... associated with a counter storing the number of occurrences ... At each of the
+ * n iterations, we first double the size of the buffer ... update the counter ... through Bernoulli sampling with
+ * probabilities computed by forward pass ... eliminate the samples ... that have the lowest numbers of occurrences."
+ * Positions are visited in the model's autoregressive order (the paper's reversed order, :107, is `order` of
+ * nqs_made_create).  Readings where the paper is silent or garbled (A13 / A25):
+ *   - the split of a counter of c occurrences is c Bernoulli trials, one per DRAW s in [0, n_draws): at position d the
+ *     draw uses u = (w + 1/2) 2^-32, w = first word of Philox4x32-10(key = (seed lo, seed hi), counter = (s lo, s hi,
+ *     d, 0)), and takes bit 1 iff u < pi_hat (conditionals in fp32) -- replayable, independent of buffer order;
+ *   - children of buffer entry i sit at 2i (bit 0) and 2i + 1 (bit 1); zero counters leave the buffer; if more than
+ *     max_unique remain the largest counters stay (ties: buffer order) and the other draws are discarded
+ *     (max_unique = 0: no elimination);
+ *   - n_up, n_down >= 0 switch on the Hamming-weight clamp of Eq. 14 (even qubits = up spins, odd = down, Eq. 12): at
+ *     a position of spin s with c spin-s bits already set and m spin-s positions left, pi_hat(1) = 0 if c = n_s,
+ *     = 1 if n_s - c = m, else the network's conditional.  n_up = n_down = -1: unconstrained.
+ * samples_out_dev : device uint64 [cap][2], counts_out_dev : device int64 [cap], cap = max_unique if 0 < max_unique <
+ *   n_draws else n_draws; the first *n_unique_out_host rows are written, in buffer order (unique, bit j = qubit j).
+ * Synchronous (n readbacks of the buffer size).  n_draws <= 2^30. */
+int nqs_made_sample(const nqs_made_t *made, int64_t n_draws, uint64_t seed, int n_up, int n_down,
+                    int64_t max_unique, uint64_t *samples_out_dev, int64_t *counts_out_dev,
+                    int64_t *n_unique_out_host, void *cuda_stream);
+
 /* Number of kernels this library has launched in the calling process since load (monotonic). */
 int64_t nqs_kernel_launch_count(void);
 

@@ -52,6 +52,8 @@ def lib():
                                             c_void_p, c_void_p]
         L.nqs_made_num_params.argtypes = [c_void_p, ctypes.POINTER(c_int64)]
         L.nqs_energy_grad.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int64, c_int64, c_void_p, c_void_p, c_void_p, c_void_p]
+        L.nqs_made_sample.argtypes = [c_void_p, c_int64, ctypes.c_uint64, c_int, c_int, c_int64, c_void_p, c_void_p,
+                                      ctypes.POINTER(c_int64), c_void_p]
         L.nqs_kernel_launch_count.restype = c_int64
         L.nqs_kernel_launch_count.argtypes = []
         L.nqs_last_chain_kernel_ms.argtypes = [c_void_p, ctypes.POINTER(ctypes.c_float), ctypes.POINTER(c_int)]
@@ -235,6 +237,18 @@ def energy_grad(made, samples, counts, eloc, minibatch=0, want_baseline=True, st
                                eloc.data_ptr(), B, minibatch, gs.ctypes.data if gs is not None else None, grad.data_ptr(),
                                base.ctypes.data if want_baseline else None, _stream_ptr(stream)), "nqs_energy_grad")
     return grad, (complex(base[0], base[1]) if want_baseline else None)
+
+
+def made_sample(made, n_draws, seed, n_up=-1, n_down=-1, max_unique=0, device="cuda", stream=None):
+    """Buffer / counter sampler -> (samples torch.int64 [U, 2] holding the uint64 bit patterns, counts torch.int64 [U])."""
+    import torch
+    cap = max_unique if 0 < max_unique < n_draws else n_draws
+    samples = torch.zeros((max(cap, 1), 2), dtype=torch.int64, device=device)
+    counts = torch.zeros((max(cap, 1),), dtype=torch.int64, device=device)
+    nu = c_int64()
+    _chk(lib().nqs_made_sample(made._h, n_draws, seed, n_up, n_down, max_unique, samples.data_ptr(), counts.data_ptr(),
+                               ctypes.byref(nu), _stream_ptr(stream)), "nqs_made_sample")
+    return samples[:nu.value], counts[:nu.value]
 
 
 def kernel_launch_count():

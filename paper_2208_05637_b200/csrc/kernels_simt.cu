@@ -143,6 +143,44 @@ __global__ void __launch_bounds__(NT) logpsi_simt_kernel(MadeDev m, const ulongl
     }
 }
 
+// Sampler support: pi_hat(z_d = 1 | z_<d) for every buffer entry — the conditional of
+// autoregressive position d with the Hamming-weight clamp of Eq. 14 (reading A13: with c spin-sigma bits set before d and
+// m spin-sigma positions left, force 0 if c = n_sigma, force 1 if n_sigma - c = m).  Entries are 128-bit prefixes in qubit
+// order with the undecided positions zero: by the MADE masks logit d does not depend on them.
+__global__ void __launch_bounds__(NT) cond_kernel(MadeDev m, const ulonglong2 *__restrict__ cfg, long long E, int d,
+                                                  int n_up, int n_down, float *__restrict__ p1_out) {
+    extern __shared__ __align__(16) unsigned char smem_raw[];
+    const Smem s = carve(smem_raw, m);
+    const int sig = __ldg(m.order + d) & 1;                      // spin of this position: even qubit = up, odd = down (Eq. 12)
+    for (long long blk = blockIdx.x; blk * TR < E; blk += gridDim.x) {
+        if (threadIdx.x < TR) {
+            const long long i = blk * TR + threadIdx.x;
+            s.cfg[threadIdx.x] = (i < E) ? cfg[i] : make_ulonglong2(0, 0);
+        }
+        __syncthreads();
+        forward_tile(m, s);                                      // leaves the logits in s.A, the +-1 inputs in s.U
+        if (threadIdx.x < TR) {
+            const int r = threadIdx.x;
+            const long long i = blk * TR + r;
+            if (i < E) {
+                float p1 = 1.0f / (1.0f + expf(-s.A[d * TR + r]));
+                if (n_up >= 0) {
+                    int c = 0, left = 0;
+                    for (int k = 0; k < m.n; ++k) {
+                        if ((__ldg(m.order + k) & 1) != sig) continue;
+                        if (k < d) c += s.U[k * TR + r] > 0.0f; else ++left;
+                    }
+                    const int target = sig == 0 ? n_up : n_down;
+                    if (c >= target) p1 = 0.0f;
+                    if (target - c >= left) p1 = 1.0f;
+                }
+                p1_out[i] = p1;
+            }
+        }
+        __syncthreads();
+    }
+}
+
 // Fused (a2)-(a5) on CUDA cores.  CTA = TR samples x a contiguous range of unique-flip groups.
 __global__ void __launch_bounds__(NT) eloc_simt_kernel(HamDev hm, MadeDev m, const ulonglong2 *__restrict__ x,
                                                        const float2 *__restrict__ base, long long B,
@@ -305,6 +343,19 @@ int launch_logpsi_simt(const MadeDev &m, const ulonglong2 *cfg, long long B, flo
     const long long nblk = (B + TR - 1) / TR;
     const int grid = (int)(nblk < (long long)num_sms() * 8 ? nblk : (long long)num_sms() * 8);
     logpsi_simt_kernel<<<grid, NT, sb, st>>>(m, cfg, B, out);
+    ++g_launch_count;
+    return cudaGetLastError() == cudaSuccess ? NQS_OK : NQS_ECUDA;
+}
+
+int launch_cond_simt(const MadeDev &m, const ulonglong2 *cfg, long long E, int d, int n_up, int n_down, float *p1,
+                     cudaStream_t st) {
+    if (E <= 0) return NQS_OK;
+    const size_t sb = smem_bytes(m);
+    if (sb > 227 * 1024) return NQS_EUNSUPPORTED;
+    if (cudaFuncSetAttribute(cond_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)sb) != cudaSuccess) return NQS_ECUDA;
+    const long long nblk = (E + TR - 1) / TR;
+    const int grid = (int)(nblk < (long long)num_sms() * 8 ? nblk : (long long)num_sms() * 8);
+    cond_kernel<<<grid, NT, sb, st>>>(m, cfg, E, d, n_up, n_down, p1);
     ++g_launch_count;
     return cudaGetLastError() == cudaSuccess ? NQS_OK : NQS_ECUDA;
 }

@@ -90,6 +90,8 @@ int launch_eloc_simt(const HamDev &hm, const MadeDev &m, const ulonglong2 *x, co
                      float2 *eloc, float2 *partial, int nsplit, unsigned *max_ratio_bits, cudaStream_t st);
 int launch_stats(const float2 *eloc, const long long *counts, long long B, double *stats4, cudaStream_t st);
 size_t eloc_simt_partial_bytes(long long B, int *nsplit, const HamDev &hm);
+int launch_cond_simt(const MadeDev &m, const ulonglong2 *cfg, long long E, int d, int n_up, int n_down, float *p1,
+                     cudaStream_t st);
 
 // kernels_tc.cu
 bool tc_supported(const nqs_made *made);

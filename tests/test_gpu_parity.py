@@ -539,3 +539,72 @@ def test_energy_gradient_global_stats_shards_sum_to_whole_batch():
     assert abs(b0 - b_all) < 1e-12 and abs(b1 - b_all) < 1e-12
     d = (g0 + g1 - g_all).abs().max().item()
     assert d <= 2e-6 * g_all.abs().max().item() + 1e-10, d
+
+
+# ---- batched autoregressive sampler ---------------------------------------------------
+def _check_sampler(params, n_draws, seed, n_up, n_down, cap, tag):
+    """CUDA sampler against oracle.sampler on the same Philox-keyed draws.  Integer work is bit-exact EXCEPT where
+    floating point decides a bit: a draw whose uniform lies within EPS of a conditional may fall on the other side in
+    the kernel's fp32 forward pass (measured |p_gpu - p_oracle| <~ 3e-6).  The oracle reports the margin |u - p| of
+    every draw; with a of them below EPS, the two count tables may differ by at most 2a in L1 (each ambiguous draw can
+    leave one entry and join another), and must be identical when a = 0 and no elimination tie is affected."""
+    from oracle import sampler as osamp
+    EPS = 2e-5
+    M = nqs.made_create(params)
+    s_gpu, c_gpu = nqs.made_sample(M, n_draws, seed, n_up, n_down, cap, device=DEV)
+    s_gpu = s_gpu.cpu().numpy().view(np.uint64)
+    c_gpu = c_gpu.cpu().numpy()
+    s_ref, c_ref, margins = osamp.sample(params, n_draws, seed, n_up, n_down, cap)
+    amb = int((margins < EPS).sum())
+    # validity that holds whatever the rounding: unique rows, positive counts, total, cap, constraint
+    assert len(set(map(tuple, s_gpu.tolist()))) == len(s_gpu)
+    assert np.all(c_gpu > 0)
+    assert (c_gpu.sum() == n_draws) if cap == 0 else (c_gpu.sum() <= n_draws and len(c_gpu) <= cap)
+    n = params.n_qubits
+    bits = wl.unpack_bits(s_gpu, n)
+    assert not np.any(s_gpu[:, 1] >> np.uint64(max(n - 64, 0))) if n > 64 else np.all(s_gpu[:, 1] == 0)
+    if n_up >= 0:
+        assert np.all(bits[:, 0::2].sum(axis=1) == n_up) and np.all(bits[:, 1::2].sum(axis=1) == n_down)
+    tab_g = {tuple(r): int(c) for r, c in zip(s_gpu.tolist(), c_gpu)}
+    tab_r = {tuple(r): int(c) for r, c in zip(s_ref.tolist(), c_ref)}
+    l1 = sum(abs(tab_g.get(k, 0) - tab_r.get(k, 0)) for k in set(tab_g) | set(tab_r))
+    print(f"[parity] sampler {tag}: {len(c_gpu)} unique (oracle {len(c_ref)}), ambiguous draws {amb}, L1 count distance {l1}")
+    if cap == 0:
+        assert l1 <= 2 * amb, (l1, amb)
+        if amb == 0:
+            assert np.array_equal(s_gpu, s_ref) and np.array_equal(c_gpu, c_ref)      # same rows, same buffer order
+    else:
+        # elimination decides by counter rank: an ambiguous draw can swap which of two tied entries survives
+        assert l1 <= 2 * amb * max(1, int(c_ref.max())) + 2 * amb, (l1, amb)
+        if amb == 0:
+            assert np.array_equal(s_gpu, s_ref) and np.array_equal(c_gpu, c_ref)
+
+
+@pytest.mark.parametrize("n,h,L,order,nu,nd,N,cap", [
+    (8, 32, 2, "reverse", 2, 2, 4000, 0),            # cfg 1 model shape: the whole 36-state sector gets populated
+    (8, 32, 2, "reverse", -1, -1, 4000, 0),          # unconstrained
+    (20, 128, 2, "reverse", 5, 5, 20000, 0),         # cfg 2 shape
+    (20, 128, 2, "random", 5, 5, 20000, 300),        # elimination of the lowest counters
+    (30, 64, 1, "random", 7, 7, 5000, 1000),         # one hidden layer, cap below the draws
+    (76, 128, 2, "reverse", 15, 15, 3000, 0),        # 76 qubits: two mask words, 15 + 15 electrons
+    (11, 16, 2, "identity", 3, 2, 2000, 0),          # odd n: 6 up positions, 5 down
+])
+def test_sampler_replays_the_oracle_draws(n, h, L, order, nu, nd, N, cap):
+    p = wl.make_made_params(n, h, 700 + n + cap, n_hidden_layers=L, order=order)
+    _check_sampler(p, N, 4242 + n, nu, nd, cap, f"n={n} h={h} L={L} {order} ({nu},{nd}) N={N} cap={cap}")
+
+
+def test_sampler_feeds_the_local_energy_path():
+    """sample -> E_loc -> gradient through the ABI only: the sampler's output is what nqs_local_energy consumes."""
+    w, (x, z, c), params, H, M = workload(2)
+    s, cnt = nqs.made_sample(M, 50000, 7, w.n_alpha, w.n_beta, 2048, device=DEV)
+    assert 0 < s.shape[0] <= 2048 and cnt.sum().item() <= 50000
+    e, st = nqs.local_energy(H, M, s, cnt)
+    assert np.isfinite(st).all() and st[0] == cnt.sum().item()
+    g, b = nqs.energy_grad(M, s, cnt, e)
+    assert torch.isfinite(g).all() and abs(b.real - st[1] / st[0]) < 1e-9 * abs(b.real)
+    # edge cases: zero draws, bad constraint
+    s0, c0 = nqs.made_sample(M, 0, 1, device=DEV)
+    assert s0.shape[0] == 0
+    with pytest.raises(nqs.NqsError):
+        nqs.made_sample(M, 10, 1, 3, -1, device=DEV)
