@@ -86,6 +86,13 @@ int nqs_ham_compile(int n_qubits, int64_t n_terms, const uint8_t *codes, const d
 int nqs_ham_compile_packed(int n_qubits, int64_t n_terms, const uint64_t *fmask, const uint64_t *smask,
                            const double *coeffs, nqs_ham_t **out);
 
+/* Same, from text (the paper's Hamiltonians are "stored in a string format", parsed by a "string
+ * parser", :154; the syntax is not given -- reading A4): one term per line, the real coefficient first (plain,
+ * parenthesised, or a complex literal with zero imaginary part such as "(0.5+0j)"), then either a dense word of
+ * n_qubits letters from IXYZ (letter j = qubit j) or sparse factors "X0 Y3 Z12"; '[' ']' '*' ',' separate, '#'
+ * comments.  Malformed lines, a qubit named twice or a non-zero imaginary part: NQS_EINVAL. */
+int nqs_ham_compile_text(int n_qubits, const char *text, nqs_ham_t **out);
+
 /* K = merged term count, G = number of unique flips, sum_abs_coeff = sum_t |c_t| (fp64, merged, the
  * tolerance scale of BASELINE.json).  Any output pointer may be NULL. */
 int nqs_ham_info(const nqs_ham_t *ham, int *n_qubits, int64_t *K, int64_t *G, double *sum_abs_coeff);

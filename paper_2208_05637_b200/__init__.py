@@ -6,10 +6,10 @@ Public API = thin binding over the C ABI in include/nqs.h:
     made_logpsi, pauli_contract, local_energy, local_energy_host, energy_grad, made_sample
 The CUDA library is loaded on first use and there is no CPU fallback.
 """
-from .binding import (PATH_AUTO, PATH_SIMT, PATH_TC, NqsError, Hamiltonian, Made, ham_compile,
+from .binding import (PATH_AUTO, PATH_SIMT, PATH_TC, NqsError, Hamiltonian, Made, ham_compile, ham_compile_text,
                       ham_compile_packed, made_create, made_logpsi, pauli_contract, local_energy,
                       local_energy_host, energy_grad, made_sample, kernel_launch_count, lib, LIB_PATH)
 
-__all__ = ["PATH_AUTO", "PATH_SIMT", "PATH_TC", "NqsError", "Hamiltonian", "Made", "ham_compile",
+__all__ = ["PATH_AUTO", "PATH_SIMT", "PATH_TC", "NqsError", "Hamiltonian", "Made", "ham_compile", "ham_compile_text",
            "ham_compile_packed", "made_create", "made_logpsi", "pauli_contract", "local_energy",
            "local_energy_host", "energy_grad", "made_sample", "kernel_launch_count", "lib", "LIB_PATH"]

@@ -33,6 +33,7 @@ def lib():
         L.nqs_strerror.argtypes = [c_int]
         L.nqs_ham_compile.argtypes = [c_int, c_int64, c_void_p, c_void_p, ctypes.POINTER(c_void_p)]
         L.nqs_ham_compile_packed.argtypes = [c_int, c_int64, c_void_p, c_void_p, c_void_p, ctypes.POINTER(c_void_p)]
+        L.nqs_ham_compile_text.argtypes = [c_int, ctypes.c_char_p, ctypes.POINTER(c_void_p)]
         L.nqs_ham_info.argtypes = [c_void_p, ctypes.POINTER(c_int), ctypes.POINTER(c_int64),
                                    ctypes.POINTER(c_int64), ctypes.POINTER(ctypes.c_double)]
         L.nqs_ham_export.argtypes = [c_void_p] * 6
@@ -101,6 +102,13 @@ def ham_compile(codes, coeffs, n_qubits=None):
     n = int(n_qubits if n_qubits is not None else codes.shape[1])
     h = c_void_p()
     _chk(lib().nqs_ham_compile(n, K, codes.ctypes.data, coeffs.ctypes.data, ctypes.byref(h)), "nqs_ham_compile")
+    return Hamiltonian(h)
+
+
+def ham_compile_text(n_qubits, text):
+    """Hamiltonian from text: 'coeff IXYZ...' or 'coeff [X0 Y3 Z12]' per line (include/nqs.h)."""
+    h = c_void_p()
+    _chk(lib().nqs_ham_compile_text(int(n_qubits), text.encode(), ctypes.byref(h)), "nqs_ham_compile_text")
     return Hamiltonian(h)
 
 

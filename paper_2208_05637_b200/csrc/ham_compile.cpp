@@ -5,6 +5,8 @@
 #include <cmath>
 #include <new>
 #include <numeric>
+#include <cstdlib>
+#include <string>
 #include "nqs_internal.h"
 
 namespace {
@@ -105,6 +107,79 @@ extern "C" int nqs_ham_compile_packed(int n_qubits, int64_t n_terms, const uint6
         terms[(size_t)k] = t;
     }
     return finish(n_qubits, terms, coeffs, out);
+}
+
+// Text form of a qubit Hamiltonian (PAPER.md:36 "stored in a string format", :154 "string parser"; the syntax is not
+// given, reading A4): one term per line, coefficient first, then EITHER a dense word of n_qubits letters from IXYZ
+// (letter j = qubit j) OR sparse factors "X0 Y3 Z12" (identity = nothing).  The coefficient may be written plainly
+// ("-0.25"), in parentheses, or as a complex literal with a zero imaginary part ("(0.5+0j)", the OpenFermion print
+// form); '[' ']' '*' ',' are separators; '#' starts a comment.
+extern "C" int nqs_ham_compile_text(int n_qubits, const char *text, nqs_ham_t **out) {
+    if (!out || !text) return NQS_EINVAL;
+    if (n_qubits < 3 || n_qubits > NQS_MAX_QUBITS) return NQS_ERANGE;
+    std::vector<Term> terms;
+    std::vector<double> coeffs;
+    try {
+        const char *p = text;
+        while (*p) {
+            const char *eol = p;
+            while (*eol && *eol != '\n') ++eol;
+            std::string line(p, eol);
+            p = *eol ? eol + 1 : eol;
+            const size_t hash = line.find('#');
+            if (hash != std::string::npos) line.resize(hash);
+            for (char &ch : line) if (ch == '[' || ch == ']' || ch == '*' || ch == ',' || ch == '(' || ch == ')' || ch == '\t' || ch == '\r') ch = ' ';
+            size_t i = line.find_first_not_of(' ');
+            if (i == std::string::npos) continue;
+            char *end = nullptr;
+            const double c = strtod(line.c_str() + i, &end);
+            if (end == line.c_str() + i) return NQS_EINVAL;
+            // optional imaginary part "+0j" / "-0.0j": must be zero (real coefficients)
+            if (*end == '+' || *end == '-') {
+                char *e2 = nullptr;
+                const double im = strtod(end, &e2);
+                if (e2 != end && (*e2 == 'j' || *e2 == 'i')) { if (im != 0.0) return NQS_EINVAL; end = e2 + 1; }
+            }
+            Term t{{0, 0}, {0, 0}, (int64_t)terms.size()};
+            const char *q = end;
+            bool dense_seen = false;
+            while (*q) {
+                while (*q == ' ') ++q;
+                if (!*q) break;
+                const char *w = q;
+                while (*q && *q != ' ') ++q;
+                const size_t len = (size_t)(q - w);
+                auto put = [&](char letter, int j) -> bool {
+                    if (j < 0 || j >= n_qubits) return false;
+                    const uint64_t bit = 1ull << (j & 63);
+                    if ((t.f[j >> 6] | t.s[j >> 6]) & bit) return false;          // qubit named twice
+                    switch (letter) {
+                        case 'I': return true;
+                        case 'X': t.f[j >> 6] |= bit; return true;
+                        case 'Y': t.f[j >> 6] |= bit; t.s[j >> 6] |= bit; return true;
+                        case 'Z': t.s[j >> 6] |= bit; return true;
+                        default: return false;
+                    }
+                };
+                bool all_letters = true;
+                for (size_t k = 0; k < len; ++k) if (!(w[k] == 'I' || w[k] == 'X' || w[k] == 'Y' || w[k] == 'Z')) all_letters = false;
+                if (all_letters && (int)len == n_qubits && !dense_seen) {
+                    for (int j = 0; j < n_qubits; ++j) if (!put(w[j], j)) return NQS_EINVAL;
+                    dense_seen = true;
+                } else if (len >= 2 && (w[0] == 'X' || w[0] == 'Y' || w[0] == 'Z' || w[0] == 'I')) {
+                    char *e3 = nullptr;
+                    const long j = strtol(w + 1, &e3, 10);
+                    if (e3 != q || !put(w[0], (int)j)) return NQS_EINVAL;
+                } else {
+                    return NQS_EINVAL;
+                }
+            }
+            terms.push_back(t);
+            coeffs.push_back(c);
+        }
+    } catch (const std::bad_alloc &) { return NQS_ENOMEM; }
+    if (terms.size() > 0xFFFFFFF0ull) return NQS_ERANGE;
+    return finish(n_qubits, terms, coeffs.data(), out);
 }
 
 extern "C" int nqs_ham_info(const nqs_ham_t *ham, int *n_qubits, int64_t *K, int64_t *G, double *sum_abs_coeff) {

@@ -5,7 +5,7 @@ only the recipes that produce integrals, the Jordan-Wigner Pauli list, random mo
 parameters and samples.  See DESIGN.md "Input recipe".
 """
 from .configs import WORKLOADS, Workload
-from .integrals import make_integrals
+from .integrals import make_integrals, make_integrals_symmetric
 from .jw import jw_pauli_terms, masks_to_codes, codes_to_strings, build_jwgen
 from .made_params import MadeParams, make_made_params, default_degrees
 from .samples import make_samples, pack_bits, unpack_bits

@@ -37,3 +37,18 @@ def make_integrals(n_spatial: int, seed: int):
     g = 0.1 * ztab[hi, lo] * decay
     g[idx, idx, idx, idx] = 0.5 + diag_u
     return np.ascontiguousarray(h), np.ascontiguousarray(g)
+
+
+def make_integrals_symmetric(n_spatial: int, seed: int, n_irreps: int = 2):
+    """Second workload: the same recipe with the SPARSITY of a molecule that has point-group
+    symmetry.  Orbital p carries an irrep label p mod n_irreps of an abelian group (Z2 or Z2 x Z2, product = XOR); h_pq
+    vanishes unless the labels agree and (pq|rs) unless the four labels multiply to the identity — the selection rule
+    that makes the paper's molecular Hamiltonians far sparser than generic integrals (Table 1:
+    K = 1,625,991 at n = 76, against 3.08 M for dense integrals).  Shapes only; no method arithmetic."""
+    if n_irreps not in (1, 2, 4):
+        raise ValueError("n_irreps must be 1, 2 or 4")
+    h, g = make_integrals(n_spatial, seed)
+    lab = np.arange(int(n_spatial)) % n_irreps
+    h = h * (lab[:, None] == lab[None, :])
+    keep = (lab[:, None, None, None] ^ lab[None, :, None, None] ^ lab[None, None, :, None] ^ lab[None, None, None, :]) == 0
+    return np.ascontiguousarray(h), np.ascontiguousarray(g * keep)

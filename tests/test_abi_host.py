@@ -148,3 +148,34 @@ def test_tensor_core_path_shape_limits():
             M.resolved_path(nqs.PATH_TC)
         assert ei.value.status == -6
         assert M.resolved_path(nqs.PATH_AUTO) == nqs.PATH_SIMT
+
+
+def test_text_loader_equals_operator_matrix_compile():
+    """nqs_ham_compile_text (dense words, sparse factors, OpenFermion-style complex literals, comments) gives the same
+    grouped tensors, bit for bit, as nqs_ham_compile on the parsed Operator Matrix."""
+    rng = np.random.default_rng(4)
+    n, K = 9, 60
+    codes = rng.integers(0, 4, size=(K, n)).astype(np.uint8)
+    codes[5] = 0
+    codes[7] = codes[3]
+    coeffs = rng.standard_normal(K)
+    letters = "IXYZ"
+    lines = ["# a comment line", ""]
+    for t in range(K):
+        c = repr(float(coeffs[t]))
+        if t % 3 == 0:
+            lines.append(f"{c} {''.join(letters[v] for v in codes[t])}")
+        elif t % 3 == 1:
+            lines.append(f"({c}+0j) [" + " ".join(f"{letters[v]}{j}" for j, v in enumerate(codes[t]) if v) + "]  # sparse")
+        else:
+            lines.append(f"{c} * " + " ".join(f"{letters[v]}{j}" for j, v in reversed(list(enumerate(codes[t]))) if v))
+    Ht = nqs.ham_compile_text(n, "\n".join(lines) + "\n")
+    Hc = nqs.ham_compile(codes, coeffs)
+    a, b = Ht.export(), Hc.export()
+    assert (Ht.K, Ht.G) == (Hc.K, Hc.G)
+    for k in a:
+        assert a[k].tobytes() == b[k].tobytes(), k
+    for bad in ("0.5 XX", "0.5 X0 Y0", "(0.5+1j) X0", "abc X0", "0.5 Q1", "0.5 X99"):
+        with pytest.raises(nqs.NqsError):
+            nqs.ham_compile_text(n, bad)
+    assert nqs.ham_compile_text(n, "# nothing\n").K == 0

@@ -608,3 +608,35 @@ def test_sampler_feeds_the_local_energy_path():
     assert s0.shape[0] == 0
     with pytest.raises(nqs.NqsError):
         nqs.made_sample(M, 10, 1, 3, -1, device=DEV)
+
+
+# ---- second workload: symmetry-sparse Hamiltonian + the paper's one-hidden-layer architecture ------
+@pytest.mark.parametrize("N,n_irreps,h", [(10, 2, 512), (13, 4, 384)])
+def test_symmetric_workload_one_hidden_layer_on_tensor_cores(N, n_irreps, h):
+    """Integrals with point-group selection rules (the sparsity of Table 1's molecules), the paper's own
+    modulus net with ONE hidden layer, Hamiltonian handed over as TEXT; E_loc on the tensor-core path
+    against the oracle at the north_star bound, all rows against the fp32 CUDA-core path."""
+    n = 2 * N
+    hh, gg = wl.make_integrals_symmetric(N, 991 + N, n_irreps)
+    x, z, c = wl.jw_pauli_terms(hh, gg)
+    codes = wl.masks_to_codes(x, z, n)
+    text = "\n".join(f"{repr(float(cc))} [" + " ".join("IXYZ"[v] + str(j) for j, v in enumerate(row) if v) + "]" for row, cc in zip(codes, c))
+    H = nqs.ham_compile_text(n, text)
+    H2 = nqs.ham_compile_packed(n, x, z, c)
+    assert (H.K, H.G) == (H2.K, H2.G) and H.export()["coef"].tobytes() == H2.export()["coef"].tobytes()
+    p = wl.make_made_params(n, h, 55 + N, n_hidden_layers=1)
+    M = nqs.made_create(p)
+    assert M.resolved_path(nqs.PATH_AUTO) == nqs.PATH_TC
+    samples, counts = wl.make_samples(N, N // 2, N // 2, 700, 64, 5, True)
+    e_tc, st = nqs.local_energy(H, M, _dev_u64(samples), torch.from_numpy(counts).to(DEV))
+    e_si, _ = nqs.local_energy(H, M, _dev_u64(samples), None, path=nqs.PATH_SIMT)
+    tol = 1e-5 * H.sum_abs_coeff
+    pick = _spread_rows(700, 12, N)
+    ref = oeloc.local_energy(codes, c, p, samples[pick], memo=True)
+    et = e_tc.cpu().numpy().astype(np.float64)
+    err = np.abs(et[pick, 0] + 1j * et[pick, 1] - ref).max()
+    d = (e_tc - e_si).cpu().numpy().astype(np.float64)
+    print(f"[parity] symmetric workload n={n} ({n_irreps} irreps) K={H.K} G={H.G}, 1 hidden layer h={h}, TC: max|dE_loc|/tol = {err / tol:.4f}; "
+          f"max|TC - SIMT|/tol = {np.hypot(d[:, 0], d[:, 1]).max() / tol:.4f}")
+    assert err <= tol
+    assert np.hypot(d[:, 0], d[:, 1]).max() <= 2 * tol
