@@ -26,9 +26,11 @@ def _sigmoid(t):
     return 0.5 * (1.0 + np.tanh(0.5 * t))
 
 
-def dlogpsi_weighted(params, configs, w_mod, w_phase):
+def dlogpsi_weighted(params, configs, w_mod, w_phase, n_up=-1, n_down=-1):
     """sum_i [ w_mod[i] * grad log|psi|(x_i) + w_phase[i] * grad phi(x_i) ] as a list of arrays shaped like the
-    parameters: [dW_0, db_0, ..., dW_L, db_L, dP1, dc1, dP2, dc2].  Manual backward pass through Eq. 8-10."""
+    parameters: [dW_0, db_0, ..., dW_L, db_L, dP1, dc1, dP2, dc2].  Manual backward pass through Eq. 8-10.
+    With n_up, n_down >= 0 the model is the constrained one: a conditional that Eq. 14 clamps to 0 / 1
+    is a constant, so its logit receives no gradient (strings that violate Eq. 12 have psi = 0 and must not be passed)."""
     n = params.n_qubits
     bits = unpack_mask(np.asarray(configs, dtype=np.uint64), n)
     z = bits[:, np.asarray(params.order, dtype=np.int64)].astype(np.float64)      # [B, n] by position
@@ -50,6 +52,12 @@ def dlogpsi_weighted(params, configs, w_mod, w_phase):
     # log|psi| = 1/2 sum_d log sigmoid(s_d a_d), s_d = +1 if z_d = 1 else -1;  d/da log sigmoid(s a) = s sigmoid(-s a)
     s = u
     g = w_mod[:, None] * 0.5 * s * _sigmoid(-s * a_out)                            # d loss / d logits
+    if n_up >= 0:
+        from .sampler import forced_positions
+        forced, valid = forced_positions(params, z.astype(np.int64), n_up, n_down)
+        if not valid.all():
+            raise ValueError("a sample violates the Hamming-weight constraint: psi = 0 there")
+        g = np.where(forced, 0.0, g)
     grads = [None] * (2 * nl)
     for k in range(nl - 1, -1, -1):
         grads[2 * k] = (g.T @ acts[k]) * masks[k]                                  # dW_k (masked entries: exactly 0)
@@ -78,7 +86,7 @@ def flatten(grads):
     return np.concatenate([np.asarray(g, dtype=np.float64).reshape(-1) for g in grads])
 
 
-def energy_gradient(params, samples, counts, eloc):
+def energy_gradient(params, samples, counts, eloc, n_up=-1, n_down=-1):
     """Eq. 7 with b = weighted mean of E_loc: returns (flat gradient fp64, b complex).
 
     samples uint64 [B,2], counts [B] (multiplicities; any non-negative weights), eloc complex [B]."""
@@ -88,4 +96,4 @@ def energy_gradient(params, samples, counts, eloc):
     b = (c * e).sum() / tot
     w_mod = c * (e.real - b.real) / tot
     w_phase = c * (e.imag - b.imag) / tot
-    return flatten(dlogpsi_weighted(params, samples, w_mod, w_phase)), b
+    return flatten(dlogpsi_weighted(params, samples, w_mod, w_phase, n_up, n_down)), b

@@ -108,6 +108,35 @@ def constrained_logprob(params, configs: np.ndarray, n_up: int, n_down: int) -> 
     return out
 
 
+def forced_positions(params, z: np.ndarray, n_up: int, n_down: int):
+    """(forced [B, n] bool, valid [B] bool): positions whose conditional Eq. 14 clamps to 0 or 1 given the bits before
+    them, and whether the string respects every clamp (i.e. satisfies Eq. 12).  z [B, n] in POSITION order."""
+    B, n = z.shape
+    forced = np.zeros((B, n), dtype=bool)
+    valid = np.ones(B, dtype=bool)
+    if n_up < 0:
+        return forced, valid
+    spin = _spin_of_positions(params)
+    for d in range(n):
+        sig = spin[d]
+        target = n_up if sig == 0 else n_down
+        c = z[:, :d][:, spin[:d] == sig].sum(axis=1)
+        m = int((spin[d:] == sig).sum())
+        f0, f1 = c >= target, (target - c) >= m
+        forced[:, d] = f0 | f1
+        valid &= ~(f0 & (z[:, d] == 1)) & ~(f1 & (z[:, d] == 0))
+    return forced, valid
+
+
+def constrained_logpsi(params, configs: np.ndarray, n_up: int, n_down: int) -> np.ndarray:
+    """log f of the CONSTRAINED model (PAPER.md:138-142 with :96 Eq. 10): log|psi| = 1/2 sum_d log pi_hat_d, phase
+    unchanged.  -inf + i phi for strings that violate Eq. 12 (psi = 0 there)."""
+    n = params.n_qubits
+    bits = unpack_mask(np.asarray(configs, dtype=np.uint64), n)
+    z = bits[:, np.asarray(params.order, dtype=np.int64)]
+    return 0.5 * constrained_logprob(params, configs, n_up, n_down) + 1j * _made.phase(params, z)
+
+
 def sample(params, n_draws: int, seed: int, n_up: int = -1, n_down: int = -1, max_unique: int = 0):
     """The buffer / counter sampler.  Returns (samples uint64 [U, 2] in qubit order, counts int64 [U]) in buffer order,
     and the list of |u - p| margins of every draw taken (for the parity test's ambiguity budget)."""

@@ -114,3 +114,37 @@ def test_sampled_frequencies_follow_pi_hat(nu, nd):
     sigma = np.sqrt(prob * (1 - prob) / N)
     assert np.all(np.abs(freq - prob) <= 5 * sigma + 1e-12)
     assert np.all(freq[prob == 0] == 0)
+
+
+def test_constrained_logpsi_forced_positions_and_its_gradient():
+    """forced_positions restates Eq. 14's clamps: skipping them in the plain MADE sum reproduces constrained_logprob;
+    the gradient of the constrained log f (oracle.grad with n_up, n_down) equals central differences of it."""
+    from oracle import grad as ograd
+    n, nu, nd = 8, 2, 3
+    p = wl.make_made_params(n, 12, 5, order="random")
+    p.weights = [w.astype(np.float64) for w in p.weights]; p.biases = [b.astype(np.float64) for b in p.biases]
+    p.phase_weights = [w.astype(np.float64) for w in p.phase_weights]; p.phase_biases = [b.astype(np.float64) for b in p.phase_biases]
+    xs = bf.all_configs(n)
+    z = unpack_mask(xs, n)[:, p.order].astype(np.int64)
+    forced, valid = osamp.forced_positions(p, z, nu, nd)
+    lp = osamp.constrained_logpsi(p, xs, nu, nd)
+    assert np.array_equal(valid, np.isfinite(lp.real))
+    a = omade.conditionals_logits(p, z)
+    terms = np.where(z == 1, omade.log_sigmoid(a), omade.log_sigmoid(-a))
+    np.testing.assert_allclose(0.5 * np.where(forced, 0.0, terms).sum(axis=1)[valid], lp.real[valid], atol=1e-13)
+    np.testing.assert_allclose(lp.imag, omade.logpsi(p, xs).imag, atol=1e-14)
+    # gradient by central differences on three valid strings
+    vi = np.flatnonzero(valid)[[0, 7, 20]]
+    cf = xs[vi]
+    rng = np.random.default_rng(0)
+    for i in range(3):
+        one = np.zeros(3); one[i] = 1
+        g = ograd.dlogpsi_weighted(p, cf, one, np.zeros(3), nu, nd)
+        for T, gt in zip([p.weights[0], p.weights[1], p.weights[2], p.biases[2]], [g[0], g[2], g[4], g[5]]):
+            flat = T.reshape(-1)
+            for k in rng.choice(flat.size, size=8, replace=False):
+                old = flat[k]
+                flat[k] = old + 1e-6; lpl = osamp.constrained_logpsi(p, cf[i:i + 1], nu, nd)[0].real
+                flat[k] = old - 1e-6; lmi = osamp.constrained_logpsi(p, cf[i:i + 1], nu, nd)[0].real
+                flat[k] = old
+                assert abs((lpl - lmi) / 2e-6 - gt.reshape(-1)[k]) < 1e-8
