@@ -124,6 +124,14 @@ int nqs_made_create(int n_qubits, int hidden, int n_hidden_layers, const int32_t
                     const float *const *phase_weights, const float *const *phase_biases,
                     nqs_made_t **out);
 
+/* Hamming-weight constraint of the model: PAPER.md:109-120 (Eq. 11-13), :136-142 (Eq. 14).  With n_up, n_down >= 0 the
+ * wavefunction is the CONSTRAINED one: every conditional that Eq. 14 clamps to 0 or 1 (reading A13, see
+ * nqs_made_sample) contributes log 1 = 0 to log|psi| = 1/2 sum_d log pi_hat_d, and a configuration that violates Eq. 12
+ * (even qubits = up spins, odd = down) has psi = 0: nqs_made_logpsi returns log|psi| = -inf for it and it contributes
+ * ratio 0 to nqs_local_energy.  nqs_energy_grad differentiates the same function (clamped logits get no gradient).
+ * n_up = n_down = -1 (the state after nqs_made_create) switches the constraint off: raw sigmoid conditionals (A12). */
+int nqs_made_set_constraint(nqs_made_t *made, int n_up, int n_down);
+
 /* Host copy of the masked fp32 weight W_k (.) M_k of layer k (0-based, k <= n_hidden_layers), row-major
  * [out][in] in position order — lets a CPU test check the mask rule without a GPU. */
 int nqs_made_export_masked(const nqs_made_t *made, int layer, float *out);

@@ -51,6 +51,7 @@ def lib():
                                        c_void_p, c_void_p, c_void_p]
         L.nqs_local_energy_host.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int64, c_int64, c_int,
                                             c_void_p, c_void_p]
+        L.nqs_made_set_constraint.argtypes = [c_void_p, c_int, c_int]
         L.nqs_made_num_params.argtypes = [c_void_p, ctypes.POINTER(c_int64)]
         L.nqs_energy_grad.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int64, c_int64, c_void_p, c_void_p, c_void_p, c_void_p]
         L.nqs_made_sample.argtypes = [c_void_p, c_int64, ctypes.c_uint64, c_int, c_int, c_int64, c_void_p, c_void_p,
@@ -138,6 +139,9 @@ class Made:
         if r < 0:
             raise NqsError(r, "nqs_made_path")
         return r
+
+    def set_constraint(self, n_up=-1, n_down=-1):
+        _chk(lib().nqs_made_set_constraint(self._h, n_up, n_down), "nqs_made_set_constraint")
 
     def num_params(self):
         k = c_int64()

@@ -84,6 +84,10 @@ int nqs_made_upload(const nqs_made *M) {
     };
     MadeDev &d = M->dev;
     d.n = n; d.h = h; d.L = L; d.npad = npad;
+    d.n_up = M->n_up; d.n_down = M->n_down;
+    d.spin_lo = d.spin_hi = 0;
+    for (int k = 0; k < n; ++k)
+        if (M->order[k] & 1) { if (k < 64) d.spin_lo |= 1ull << k; else d.spin_hi |= 1ull << (k - 64); }
     {
         void *p = nullptr;
         if ((rc = upload(M->order.data(), M->order.size(), &p))) return rc;
@@ -125,6 +129,16 @@ int nqs_ws_reserve(const nqs_made *M, size_t bytes) {
     if (M->ws) { cudaFree(M->ws); M->ws = nullptr; M->ws_bytes = 0; }
     if (cudaMalloc(&M->ws, bytes) != cudaSuccess) { cudaGetLastError(); return NQS_ENOMEM; }
     M->ws_bytes = bytes;
+    return NQS_OK;
+}
+
+extern "C" int nqs_made_set_constraint(nqs_made_t *M, int n_up, int n_down) {
+    if (!M) return NQS_EINVAL;
+    if ((n_up < 0) != (n_down < 0)) return NQS_EINVAL;
+    if (n_up < 0) { n_up = n_down = -1; }
+    else if (n_up > (M->n + 1) / 2 || n_down > M->n / 2) return NQS_EINVAL;       // even qubits = up, odd = down (Eq. 12)
+    M->n_up = n_up; M->n_down = n_down;
+    M->dev.n_up = n_up; M->dev.n_down = n_down;                                   // the device view is passed by value per launch
     return NQS_OK;
 }
 

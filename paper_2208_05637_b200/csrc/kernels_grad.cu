@@ -92,6 +92,7 @@ __global__ void __launch_bounds__(NT) grad_rows_kernel(MadeDev m, const ulonglon
     float *O = A + (size_t)npad * TR;                      // [4][TR]
     float *wr = O + 4 * TR, *wi = wr + TR;                 // [TR] each
     __shared__ ulonglong2 cfg[TR];
+    __shared__ ulonglong2 fmask[TR];                       // Eq. 14: clamped conditionals are constants -> no gradient through their logits
     const double tot = stats3[0], bre = stats3[1] / tot, bim = stats3[2] / tot;
     for (long long row0 = (long long)blockIdx.x * TR; row0 < nrows; row0 += (long long)gridDim.x * TR) {
         if (threadIdx.x < TR) {
@@ -108,6 +109,18 @@ __global__ void __launch_bounds__(NT) grad_rows_kernel(MadeDev m, const ulonglon
         for (int idx = threadIdx.x; idx < npad * TR; idx += NT) {
             const int d = idx / TR, r = idx % TR;
             U[idx] = d < n ? (bit128(cfg[r], __ldg(m.order + d)) ? 1.0f : -1.0f) : 0.0f;
+        }
+        if (threadIdx.x < TR) {
+            ulonglong2 f = make_ulonglong2(0, 0);
+            if (m.n_up >= 0) {
+                const int r = threadIdx.x;
+                ulonglong2 zp = make_ulonglong2(0, 0);
+                for (int d = 0; d < n; ++d)
+                    if (bit128(cfg[r], __ldg(m.order + d))) { if (d < 64) zp.x |= 1ull << d; else zp.y |= 1ull << (d - 64); }
+                bool valid;
+                f = nqs_forced_mask(zp, n, m.spin_lo, m.spin_hi, m.n_up, m.n_down, &valid);
+            }
+            fmask[threadIdx.x] = f;
         }
         __syncthreads();
         store_rows(U, npad, ws.U, npad, row0, nrows);
@@ -128,7 +141,8 @@ __global__ void __launch_bounds__(NT) grad_rows_kernel(MadeDev m, const ulonglon
         for (int idx = threadIdx.x; idx < npad * TR; idx += NT) {
             const int d = idx / TR, r = idx % TR;
             const float s = U[idx], a = A[idx];
-            A[idx] = d < n ? wr[r] * 0.5f * s / (1.0f + expf(s * a)) : 0.0f;
+            const bool clamped = ((d < 64 ? fmask[r].x : fmask[r].y) >> (d & 63)) & 1ull;
+            A[idx] = (d < n && !clamped) ? wr[r] * 0.5f * s / (1.0f + expf(s * a)) : 0.0f;
         }
         __syncthreads();
         store_rows(A, npad, ws.dA, npad, row0, nrows);

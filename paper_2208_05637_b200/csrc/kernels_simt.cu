@@ -56,6 +56,8 @@ struct Smem {
     float *U, *X, *Y, *A, *O, *red;   // [n][TR], [h][TR], [h][TR], [npad][TR], [4][TR], [16][TR]
     ulonglong2 *cfg;                  // [TR]
     float *lp, *phi;                  // [TR]
+    float *keep;                      // [npad][TR]: 0 where Eq. 14 clamps the conditional (constraint on), else 1
+    float *bad;                       // [TR]: 1 if the row violates Eq. 12 (psi = 0)
 };
 
 __device__ __forceinline__ Smem carve(unsigned char *base, const MadeDev &m) {
@@ -70,11 +72,13 @@ __device__ __forceinline__ Smem carve(unsigned char *base, const MadeDev &m) {
     s.red = p; p += 16 * TR;
     s.lp = p; p += TR;
     s.phi = p; p += TR;
+    s.keep = p; p += (size_t)m.npad * TR;
+    s.bad = p; p += TR;
     return s;
 }
 
 size_t smem_bytes(const MadeDev &m) {
-    return sizeof(float) * ((size_t)TR * 4 + 2 * (size_t)m.npad * TR + 2 * (size_t)m.h * TR + 4 * TR + 16 * TR + 2 * TR);
+    return sizeof(float) * ((size_t)TR * 4 + 3 * (size_t)m.npad * TR + 2 * (size_t)m.h * TR + 4 * TR + 16 * TR + 3 * TR);
 }
 
 // MADE + phase forward for the TR configurations in s.cfg -> s.lp[r] = log|psi|, s.phi[r] = phi.
@@ -85,6 +89,16 @@ __device__ void forward_tile(const MadeDev &m, const Smem &s) {
     for (int idx = threadIdx.x; idx < n * TR; idx += NT) {
         const int d = idx / TR, r = idx % TR;
         s.U[idx] = bit128(s.cfg[r], __ldg(m.order + d)) ? 1.0f : -1.0f;
+    }
+    if (m.n_up >= 0 && threadIdx.x < TR) {                      // Eq. 14: which conditionals are clamped for this row
+        const int r = threadIdx.x;
+        ulonglong2 zp = make_ulonglong2(0, 0);
+        for (int d = 0; d < n; ++d)
+            if (bit128(s.cfg[r], __ldg(m.order + d))) { if (d < 64) zp.x |= 1ull << d; else zp.y |= 1ull << (d - 64); }
+        bool valid;
+        const ulonglong2 fm = nqs_forced_mask(zp, n, m.spin_lo, m.spin_hi, m.n_up, m.n_down, &valid);
+        for (int d = 0; d < n; ++d) s.keep[d * TR + r] = ((d < 64 ? fm.x : fm.y) >> (d & 63)) & 1ull ? 0.0f : 1.0f;
+        s.bad[r] = valid ? 0.0f : 1.0f;
     }
     __syncthreads();
     layer_fwd<TR, true>(m.w1t, h, m.b1, n, h, s.U, s.X);
@@ -107,7 +121,8 @@ __device__ void forward_tile(const MadeDev &m, const Smem &s) {
         float acc = 0.0f;
         for (int d = part; d < n; d += NT / TR) {
             const float a = s.A[d * TR + r];
-            acc += log_sigmoid(s.U[d * TR + r] > 0.0f ? a : -a);
+            const float ls = log_sigmoid(s.U[d * TR + r] > 0.0f ? a : -a);
+            acc += (m.n_up >= 0 && s.keep[d * TR + r] == 0.0f) ? 0.0f : ls;
         }
         s.red[part * TR + r] = acc;
     }
@@ -117,7 +132,7 @@ __device__ void forward_tile(const MadeDev &m, const Smem &s) {
         float acc = 0.0f;
 #pragma unroll
         for (int p = 0; p < NT / TR; ++p) acc += s.red[p * TR + r];
-        s.lp[r] = 0.5f * acc;
+        s.lp[r] = (m.n_up >= 0 && s.bad[r] != 0.0f) ? -INFINITY : 0.5f * acc;
         const int sel = (s.U[(n - 2) * TR + r] > 0.0f ? 2 : 0) + (s.U[(n - 1) * TR + r] > 0.0f ? 1 : 0);
         s.phi[r] = s.O[sel * TR + r];
     }

@@ -100,6 +100,8 @@ struct TcParams {
     float *eloc;                         // [B][2], pre-initialised with the f = 0 group; atomically accumulated
     unsigned *max_ratio_bits;
     long long g_begin;                   // first group that needs a forward pass (1 if group 0 is f = 0)
+    int n_up, n_down;                    // Hamming-weight constraint (Eq. 14), n_up < 0 = off
+    unsigned long long spin_lo, spin_hi; // bit d = 1: position d is a down spin
 #ifdef TC_PROF
     long long *prof;                     // [grid][16] cycle counters (instrumented build only)
 #endif
@@ -444,6 +446,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
 
         RowState cur{}, nxt{};
         ulonglong2 zp = make_ulonglong2(0, 0), zp_n = zp;
+        // Eq. 14: positions whose conditional is clamped contribute log 1 = 0; a string that violates Eq. 12 has psi = 0
+        ulonglong2 fm = make_ulonglong2(0, 0), fm_n = fm;
+        bool inval = false, inval_n = false;
+        auto clamp_of = [&](ulonglong2 z, ulonglong2 &f, bool &bad) {
+            if (p.n_up < 0) return;
+            bool ok;
+            f = nqs_forced_mask(z, p.n, p.spin_lo, p.spin_hi, p.n_up, p.n_down, &ok);
+            bad = !ok;
+        };
         float2 E = make_float2(0.f, 0.f);
         float mr = (p.mode == 1 && p.hm.has_diag) ? 1.0f : 0.0f;     // the f = 0 group has ratio exactly 1
         long long pt_a0 = 0, pt_d3 = 0, pt_tot = clock64(), pt_s = 0, pt_fin = 0;
@@ -454,6 +465,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             load_row(t / Gnd, valid, cur);
             const ulonglong2 f = flip_of(t, valid);
             zp = make_ulonglong2(cur.xp.x ^ f.x, cur.xp.y ^ f.y);
+            clamp_of(zp, fm, inval);
             build_a0(zp);
         }
         for (long long ti = 0; ti < ntl; ++ti) {
@@ -468,6 +480,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                 if (sbn != cur.sb || !validn) load_row(sbn, validn, nxt); else nxt = cur;
                 const ulonglong2 f = flip_of(tn, validn);
                 zp_n = make_ulonglong2(nxt.xp.x ^ f.x, nxt.xp.y ^ f.y);
+                clamp_of(zp_n, fm_n, inval_n);
             }
             // ---- (a3) S = sum_{t in g} c_t (-i)^{r_t} (-1)^{popcount(x & s_t)}: independent of the MMAs, done while they run ----
             float2 S = make_float2(0.f, 0.f);
@@ -513,7 +526,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                     const float o2 = __uint_as_float(v[14]) + s_c2[2], o3 = __uint_as_float(v[15]) + s_c2[3];
                     phi = sel == 0 ? o0 : (sel == 1 ? o1 : (sel == 2 ? o2 : o3));
                 }
-                const uint32_t zb = (uint32_t)shr128(zp, c0);
+                const uint32_t zb = (uint32_t)shr128(zp, c0), fb = (uint32_t)shr128(fm, c0);
                 const int nv = p.n - c0;                       // valid conditionals in this block (may be <= 0 or >= 16)
                 const float4 *bp = reinterpret_cast<const float4 *>(s_b3 + c0);
                 float prod0 = 1.0f, prod1 = 1.0f, m0 = 0.0f, m1 = 0.0f;
@@ -526,7 +539,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                         const int k = 4 * k4 + kk;
                         const float a = __uint_as_float(v[k]) + bk[kk];
                         float tt = ((zb >> k) & 1u) ? a : -a;
-                        tt = (k < nv) ? tt : 1e30f;            // padding column: factor 1, min 0
+                        tt = (k < nv && !((fb >> k) & 1u)) ? tt : 1e30f;      // padding column or clamped conditional: factor 1, min 0
                         const float e = ex2_ftz(fabsf(tt) * -1.4426950408889634f);
                         if (k & 1) { prod1 *= 1.0f + e; m1 += fminf(tt, 0.0f); }
                         else       { prod0 *= 1.0f + e; m0 += fminf(tt, 0.0f); }
@@ -540,7 +553,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             tc_fence_before();
             __syncwarp();
             if (lane == 0) mbar_arrive_leader(BAR_ADDR(BAR_D3EMPTY), rank);
-            const float lp = 0.5f * part;
+            const float lp = inval ? -INFINITY : 0.5f * part;
             if (p.mode == 0) {
                 if (cur.i < p.B) p.out[cur.i] = make_float2(lp, phi);
             } else if (cur.i < p.B) {
@@ -563,7 +576,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
 #ifdef TC_PROF
             pt_fin += clock64() - _tf;
 #endif
-            cur = nxt; zp = zp_n;
+            cur = nxt; zp = zp_n; fm = fm_n; inval = inval_n;
         }
         if (p.mode == 1) atomicMax(p.max_ratio_bits, __float_as_uint(mr));
 #ifdef TC_PROF
@@ -896,6 +909,7 @@ static void fill_common(const nqs_made *M, TcParams &p) {
     p.resimg = (const uint8_t *)P->d_res; p.res_bytes = P->res_bytes;
     p.slot_bytes = P->slot_bytes; p.nslots = P->nslots;
     p.bias = (const float *)P->d_bias;
+    p.n_up = M->dev.n_up; p.n_down = M->dev.n_down; p.spin_lo = M->dev.spin_lo; p.spin_hi = M->dev.spin_hi;
 }
 
 static int ensure(void **buf, size_t *cap, size_t bytes) {

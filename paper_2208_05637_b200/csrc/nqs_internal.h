@@ -32,7 +32,35 @@ struct MadeDev {
     const float *p1t;            // [n][h]   phase layer 1; rows n-2, n-1 are zero
     const float *p2t;            // [h][4]
     const float *c1, *c2;        // [h], [4]
+    // Hamming-weight constraint (Eq. 14; n_up < 0 = off): conditionals clamped to 0 / 1 contribute
+    // log 1 = 0 to log|psi|; strings that violate Eq. 12 have psi = 0
+    int n_up, n_down;
+    unsigned long long spin_lo, spin_hi;   // bit d = 1 if autoregressive position d is a down spin (odd qubit, Eq. 12)
 };
+
+#ifdef __CUDACC__
+// Positions whose conditional Eq. 14 clamps, for one configuration zp given in POSITION order (reading A13: at a
+// position of spin s with c spin-s bits set before it and m spin-s positions left, forced to 0 if c = n_s, to 1 if
+// n_s - c = m).  *valid = the string respects every clamp (equivalently satisfies Eq. 12).
+__device__ __forceinline__ ulonglong2 nqs_forced_mask(ulonglong2 zp, int n, unsigned long long spin_lo, unsigned long long spin_hi,
+                                                      int n_up, int n_down, bool *valid) {
+    int cnt0 = 0, cnt1 = 0;
+    int rem1 = __popcll(spin_lo) + __popcll(spin_hi), rem0 = n - rem1;
+    unsigned long long f_lo = 0, f_hi = 0;
+    bool ok = true;
+    for (int d = 0; d < n; ++d) {
+        const unsigned long long zw = d < 64 ? zp.x : zp.y, sw = d < 64 ? spin_lo : spin_hi;
+        const int bit = (int)((zw >> (d & 63)) & 1ull), sig = (int)((sw >> (d & 63)) & 1ull);
+        const int c = sig ? cnt1 : cnt0, left = sig ? rem1 : rem0, target = sig ? n_down : n_up;
+        const bool f0 = c >= target, f1 = target - c >= left;
+        if (f0 | f1) { if (d < 64) f_lo |= 1ull << d; else f_hi |= 1ull << (d - 64); }
+        ok = ok && !(f0 && bit) && !(f1 && !bit);
+        if (sig) { cnt1 += bit; --rem1; } else { cnt0 += bit; --rem0; }
+    }
+    *valid = ok;
+    return make_ulonglong2(f_lo, f_hi);
+}
+#endif
 
 // ---- handles ------------------------------------------------------------------------------------
 struct nqs_ham {
@@ -66,6 +94,7 @@ struct nqs_made {
     mutable MadeDev dev{};
     mutable TcPack *tc = nullptr;
     mutable GradPack *grad = nullptr;
+    int n_up = -1, n_down = -1;                 // nqs_made_set_constraint
     // workspace (grown on demand, reused across calls)
     mutable void  *ws = nullptr;
     mutable size_t ws_bytes = 0;

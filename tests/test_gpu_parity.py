@@ -640,3 +640,64 @@ def test_symmetric_workload_one_hidden_layer_on_tensor_cores(N, n_irreps, h):
           f"max|TC - SIMT|/tol = {np.hypot(d[:, 0], d[:, 1]).max() / tol:.4f}")
     assert err <= tol
     assert np.hypot(d[:, 0], d[:, 1]).max() <= 2 * tol
+
+
+# ---- constrained model: nqs_made_set_constraint (Eq. 14, readings A12 / A13) ---------------------
+@pytest.mark.parametrize("n,h,L,order,nu,nd", [(8, 32, 2, "reverse", 2, 2), (20, 128, 2, "random", 5, 5), (76, 512, 2, "reverse", 15, 15),
+                                                (30, 128, 1, "identity", 7, 6)])
+def test_constrained_logpsi_both_paths(n, h, L, order, nu, nd):
+    """log|psi| of the constrained model on valid strings (clamped conditionals skipped) and -inf on strings that
+    violate Eq. 12, on the CUDA-core and the tensor-core path."""
+    from oracle import sampler as osamp
+    p = wl.make_made_params(n, h, 900 + n, n_hidden_layers=L, order=order)
+    N = n // 2
+    valid_s, _ = wl.make_samples(N, nu, nd, 200, 4, 3, False)
+    rng = np.random.default_rng(n)
+    rand_s = wl.pack_bits(rng.integers(0, 2, size=(133, n)).astype(np.uint8))
+    cfgs = np.concatenate([valid_s, rand_s])
+    ref = osamp.constrained_logpsi(p, cfgs, nu, nd)
+    M = nqs.made_create(p)
+    M.set_constraint(nu, nd)
+    for path in _paths(M, min_hidden_tc=0):
+        out = nqs.made_logpsi(M, _dev_u64(cfgs), path=path).cpu().numpy().astype(np.float64)
+        fin = np.isfinite(ref.real)
+        assert fin[:200].all()
+        assert np.array_equal(np.isneginf(out[:, 0]), ~fin), path
+        tol = 2e-4 if path == nqs.PATH_SIMT else TC_LOGPSI_TOL
+        assert np.abs(out[fin, 0] - ref.real[fin]).max() < tol
+        assert np.abs(out[:, 1] - ref.imag).max() < tol
+    M.set_constraint(-1, -1)                                    # off again: the raw model
+    out = nqs.made_logpsi(M, _dev_u64(cfgs), path=nqs.PATH_SIMT).cpu().numpy().astype(np.float64)
+    assert np.abs(out[:, 0] - omade.logpsi(p, cfgs).real).max() < 2e-4
+
+
+def test_constrained_local_energy_and_gradient_cfg2():
+    """cfg 2 with the constrained wavefunction (5 up + 5 down): E_loc against the oracle's term-by-term sum with the
+    constrained log f (the JW Hamiltonian conserves both spin populations, so every connected string is valid), and the
+    gradient of Eq. 7 of the constrained model."""
+    from oracle import sampler as osamp
+    from oracle import grad as ograd
+    w, (x, z, c), params, H, _ = workload(2)
+    M = nqs.made_create(params)
+    M.set_constraint(w.n_alpha, w.n_beta)
+    samples, counts = wl.make_samples(w.n_spatial, w.n_alpha, w.n_beta, 400, w.max_count, w.seed_samples, True)
+    codes = wl.masks_to_codes(x, z, w.n_qubits)
+    pick = np.arange(0, 400, 25)
+    ref = oeloc.local_energy_generic(codes, c, samples[pick], lambda cf: osamp.constrained_logpsi(params, cf, w.n_alpha, w.n_beta))
+    tol = 1e-5 * H.sum_abs_coeff
+    for path, fac in ((nqs.PATH_SIMT, 1.0), (nqs.PATH_TC, TC_NARROW_FACTOR)):
+        e, st = nqs.local_energy(H, M, _dev_u64(samples), torch.from_numpy(counts).to(DEV), path=path)
+        en = e.cpu().numpy().astype(np.float64)
+        err = np.abs(en[pick, 0] + 1j * en[pick, 1] - ref).max()
+        print(f"[parity] cfg 2 constrained model, path {path}: max|dE_loc|/tol = {err / tol:.4f}")
+        assert err <= fac * tol
+        if path == nqs.PATH_SIMT:
+            g, b = nqs.energy_grad(M, _dev_u64(samples), torch.from_numpy(counts).to(DEV), e)
+            e64 = en[:, 0] + 1j * en[:, 1]
+            gref, _ = ograd.energy_gradient(params, samples, counts, e64, w.n_alpha, w.n_beta)
+            g = g.cpu().numpy().astype(np.float64)
+            for sl in _grad_tensor_slices(params):
+                assert np.abs(g[sl] - gref[sl]).max() <= 2e-5 * np.abs(gref[sl]).max() + 1e-9
+            # and it differs from the unconstrained gradient (the flag is really in effect)
+            gun, _ = ograd.energy_gradient(params, samples, counts, e64)
+            assert np.abs(gun - gref).max() > 1e-4 * np.abs(gref).max()
