@@ -87,7 +87,7 @@ struct TcParams {
     uint8_t prewait[MAX_OPS];            // bit a: wait for the chunk epilogue pending on accumulator a before issuing op j
     uint32_t cntmask;                    // bit a: accumulator a is used an odd number of times per tile
     const uint8_t *resimg; uint32_t res_bytes;    // resident P2 tiles of rank r at resimg + r * res_bytes
-    uint32_t slot_bytes; int nslots;
+    uint32_t slot_bytes; int nslots, nprod;
     const float *bias;                   // [c1 H | b1 H | b2 H | b3 KO | c2 4] fp32
     int mode;                            // 0 = logpsi, 1 = local energy
     const ulonglong2 *xpos;              // [B] configurations, bits in autoregressive POSITION order
@@ -190,19 +190,23 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
         // =========================== weight producers (TMA engine, 1-D bulk copies), both CTAs ===========================
         // Fill q always lands in slot q % nslots.  Never more lanes than slots: a lane two uses of a slot ahead of the
         // consumer would pass its parity wait on an older phase and overwrite live data.
-        const uint32_t nprod = (uint32_t)(p.nslots < NPROD ? p.nslots : NPROD);
+        const uint32_t nprod = (uint32_t)p.nprod;
         if ((uint32_t)lane < nprod) {
             const long long total = ntl * (long long)p.nfills;
             const uint8_t *img = p.wimg + (size_t)rank * p.img_stride;
             uint32_t e = (uint32_t)lane % (uint32_t)p.nfills, slot = (uint32_t)lane, par = 1u;   // a fresh barrier passes a parity-1 wait
+            long long pp_wait = 0; (void)pp_wait;
             for (long long q = lane; q < total; q += nprod) {
                 const uint2 pe = __ldg(&p.fills[e]);
-                mbar_wait(&bars[BAR_WEMPTY + slot], par);
+                { PROF_T0(); mbar_wait(&bars[BAR_WEMPTY + slot], par); PROF_ADD(pp_wait); }
                 mbar_arrive_expect_tx(&bars[BAR_WFULL + slot], pe.y);
                 bulk_g2s(smem + SL.slots + slot * p.slot_bytes, img + pe.x, pe.y, &bars[BAR_WFULL + slot]);
                 e += nprod; while (e >= (uint32_t)p.nfills) e -= (uint32_t)p.nfills;
                 slot += nprod; while (slot >= (uint32_t)p.nslots) { slot -= (uint32_t)p.nslots; par ^= 1u; }
             }
+#ifdef TC_PROF
+            if (p.prof && lane == 0) p.prof[(size_t)blockIdx.x * 32 + 21] = pp_wait;
+#endif
         }
     } else if (warp == W_ISSUE && rank != 0) {
         // =========================== peer CTA: ring forwarder ===========================
@@ -211,11 +215,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
         if (elect_one()) {
             const long long total = ntl * (long long)p.nfills;
             uint32_t slot = 0, par = 0;
+            long long pf_wait = 0; (void)pf_wait;
             for (long long q = 0; q < total; ++q) {
-                mbar_wait(&bars[BAR_WFULL + slot], par);
+                { PROF_T0(); mbar_wait(&bars[BAR_WFULL + slot], par); PROF_ADD(pf_wait); }
                 mbar_arrive_cluster(BAR_ADDR(BAR_WFULL + slot), 0);
                 if (++slot == (uint32_t)p.nslots) { slot = 0; par ^= 1u; }
             }
+#ifdef TC_PROF
+            if (p.prof) p.prof[(size_t)blockIdx.x * 32 + 22] = pf_wait;
+#endif
         }
         __syncwarp();
     } else if (warp == W_ISSUE) {
@@ -908,6 +916,10 @@ static void fill_common(const nqs_made *M, TcParams &p) {
     memcpy(p.prewait, P->prewait, sizeof(p.prewait)); p.cntmask = P->cntmask;
     p.resimg = (const uint8_t *)P->d_res; p.res_bytes = P->res_bytes;
     p.slot_bytes = P->slot_bytes; p.nslots = P->nslots;
+    p.nprod = P->nslots < NPROD ? P->nslots : NPROD;
+#ifdef TC_PROF
+    if (const char *e = getenv("NQS_TC_NPROD")) { p.nprod = atoi(e); if (p.nprod > p.nslots) p.nprod = p.nslots; }
+#endif
     p.bias = (const float *)P->d_bias;
     p.n_up = M->dev.n_up; p.n_down = M->dev.n_down; p.spin_lo = M->dev.spin_lo; p.spin_hi = M->dev.spin_hi;
 }
