@@ -33,7 +33,7 @@ namespace {
 constexpr int TILE_M = 128;
 constexpr int CN = 128;                  // hidden-unit chunk = accumulator columns = MMA N of the pair
 constexpr int HALF = CN / 2;             // weight rows per CTA and chunk
-constexpr int NTHREADS = 448;
+constexpr int NTHREADS = 576;
 constexpr int MAX_NC = 4;                // hidden <= 512
 constexpr int MAX_SLOTS = 8;
 constexpr int NPROD = 4;                 // producer lanes (bulk-copy issuers), never more than slots
@@ -42,7 +42,7 @@ constexpr int MAX_OPS = 3 * MAX_NC;
 // warps, and every sub-partition hosts epilogue warps (a warp reaches only TMEM lane quadrant id % 4): the one thread
 // that issues all MMAs therefore lives in the highest warp id of its sub-partition, or it only gets the issue slots
 // the epilogue warps leave over.
-constexpr int W_EPI = 4, W_PROD = 12, W_ISSUE = 13;      // warps 0-3: tile warps
+constexpr int W_EPI = 4, W_PROD = 16, W_ISSUE = 17;      // warps 0-3: tile warps, 4-15: three chunk-epilogue groups
 
 enum : uint8_t { T_L1S = 0, T_L1I = 1, T_P = 2, T_L2 = 3 };   // layer 1 -> smem A1 | layer 1 in place | phase hidden | layer 2
 
@@ -52,7 +52,7 @@ enum { BAR_A0FULL = 0, BAR_A0FREE = 1, BAR_A1FREE = 2, BAR_D3FULL = 3, BAR_D3EMP
        BAR_WFULL = 11, BAR_WEMPTY = 11 + MAX_SLOTS, BAR_COUNT = 11 + 2 * MAX_SLOTS };
 
 // Streamed weight sub-tiles: one 32-bit word each, in consumption order (kernel parameter space -> uniform loads).
-constexpr int MAX_SUB = 2 * MAX_NC + MAX_NC * 2 * MAX_NC + MAX_NC;   // W1 + P1 + W2 blocks + W3
+constexpr int MAX_SUB = 2 * MAX_NC + MAX_NC * (1 + 2 * MAX_NC) + MAX_NC;   // W1 + P1 + (b2 rows + W2 blocks) + W3
 constexpr uint32_t SUB_OFF_MASK = 0x1FFFu;                   // [0:13)  byte offset inside the slot / 16
 constexpr uint32_t SUB_NEW = 1u << 13;                       // first sub-tile of a ring fill: wait for the fill
 constexpr uint32_t SUB_END = 1u << 14;                       // last sub-tile of a ring fill: release the slot
@@ -65,7 +65,7 @@ __host__ __device__ inline SmemLayout smem_layout(int H, int KO, int L, uint32_t
     uint32_t off = 0;
     S.a1 = off; if (L == 2) off += (uint32_t)(H / 64) * 16384u;      // fp16 layer-1 activations, [H/64] K-blocks of 128 rows x 128 B
     S.res = off; off += (uint32_t)(H / 64) * 1024u;                  // resident P2 tiles: 8 rows x 64 K per K-block (this CTA's half)
-    S.bias = off; off += (uint32_t)(3 * H + KO + 4) * 4;
+    S.bias = off; off += (uint32_t)(KO + 4) * 4;                 // b3 | c2 (hidden-layer biases ride in the weight images)
     off = (off + 15) & ~15u;
     S.bars = off; off += BAR_COUNT * 8;
     off = (off + 1023) & ~1023u;
@@ -88,7 +88,7 @@ struct TcParams {
     uint32_t cntmask;                    // bit a: accumulator a is used an odd number of times per tile
     const uint8_t *resimg; uint32_t res_bytes;    // resident P2 tiles of rank r at resimg + r * res_bytes
     uint32_t slot_bytes; int nslots, nprod;
-    const float *bias;                   // [c1 H | b1 H | b2 H | b3 KO | c2 4] fp32
+    const float *bias;                   // [b3 KO | c2 4] fp32
     int mode;                            // 0 = logpsi, 1 = local energy
     const ulonglong2 *xpos;              // [B] configurations, bits in autoregressive POSITION order
     long long B;
@@ -103,7 +103,8 @@ struct TcParams {
     int n_up, n_down;                    // Hamming-weight constraint (Eq. 14), n_up < 0 = off
     unsigned long long spin_lo, spin_hi; // bit d = 1: position d is a down spin
 #ifdef TC_PROF
-    long long *prof;                     // [grid][16] cycle counters (instrumented build only)
+    long long *prof;                     // [grid][32] cycle counters (instrumented build only)
+    int test_mode;                       // 1: issuer waits for the weight ring only; 2: for nothing (timing probes, results are garbage)
 #endif
 };
 
@@ -111,7 +112,11 @@ struct TcParams {
 #define PROF_T0() const long long _t0 = clock64()
 #define PROF_ADD(v) (v) += clock64() - _t0
 #define PROF_STALL(sp) do { if (sp) { pw_stall += clock64() - _t0; ++pw_nstall; } ++pw_npoll; } while (0)
+#define PROF_SITE(x) pw_site = (x)
+#define TESTMODE (p.test_mode)
 #else
+#define PROF_SITE(x) do {} while (0)
+#define TESTMODE 0
 #define PROF_T0() do {} while (0)
 #define PROF_ADD(v) do {} while (0)
 #define PROF_STALL(sp) do { (void)(sp); } while (0)
@@ -123,21 +128,34 @@ __device__ __forceinline__ unsigned long long shr128(ulonglong2 a, int s) {     
     return a.y >> (s - 64);
 }
 
-// The per-tile op schedule, fixed at compile time so that the issuing thread runs straight-line code (it is
-// instruction-bound: the tensor pipe queues only ~100 cycles of MMAs ahead of the issuer, measured).  Two hidden
-// layers: layer-1 chunks 0..NC-1 (-> A1), then phase chunk c / layer-2 chunk c alternating; one hidden layer: layer-1
-// chunk c (in place) / phase chunk c alternating.  Op j runs in accumulator j % NACC and is handed to epilogue group
-// j & 1; the consumer of an in-place op is issued LAG = NACC - 1 ops later, just before the accumulator's next producer.
+// The per-tile op schedule, fixed at compile time so that the issuing thread runs straight-line code (the tensor pipe
+// queues only ~100 cycles of MMAs ahead of the issuer, measured).  Two hidden layers: short ops (layer-1 chunk -> A1,
+// phase chunk) are interleaved with the long layer-2 chunks, each as early as its inputs allow, so that a chunk
+// epilogue (~1 us hand-over round trip) always runs under the MMAs of the next two ops; one hidden layer: layer-1
+// chunk c (in place) / phase chunk c alternating.  Op j runs in accumulator j % NACC, whose epilogue group (warps
+// W_EPI + 4 a ..) handles every op of that accumulator; the consumer of an in-place op is issued LAG = NACC - 1 ops
+// later, just before the accumulator's next producer.
 template <int NC, int L, int NACC>
 struct Sched {
     static constexpr int NOPS = (L == 2) ? 3 * NC : 2 * NC;
     static constexpr int LAG = NACC - 1;
-    static constexpr int FIRST_INPLACE = (L == 2) ? NC : 0;
+    static constexpr int FIRST_INPLACE = (L == 2) ? (NC > 1 ? 2 : 1) : 0;
     static constexpr int LAST_A0 = (L == 2) ? NOPS - 2 : NOPS - 1;
+    // two hidden layers: L1S 0 | (L1S c+1, P c, L2 c) for c < NC-1 | P NC-1, L2 NC-1
     __host__ __device__ static constexpr int type(int j) {
-        return L == 2 ? (j < NC ? (int)T_L1S : (((j - NC) & 1) ? (int)T_L2 : (int)T_P)) : ((j & 1) ? (int)T_P : (int)T_L1I);
+        if (L != 2) return (j & 1) ? (int)T_P : (int)T_L1I;
+        if (j == 0) return (int)T_L1S;
+        const int jj = j - 1;
+        if (jj < 3 * (NC - 1)) return jj % 3 == 0 ? (int)T_L1S : (jj % 3 == 1 ? (int)T_P : (int)T_L2);
+        return (jj - 3 * (NC - 1)) == 0 ? (int)T_P : (int)T_L2;
     }
-    __host__ __device__ static constexpr int chunk(int j) { return L == 2 ? (j < NC ? j : (j - NC) / 2) : j / 2; }
+    __host__ __device__ static constexpr int chunk(int j) {
+        if (L != 2) return j / 2;
+        if (j == 0) return 0;
+        const int jj = j - 1;
+        if (jj < 3 * (NC - 1)) return jj % 3 == 0 ? jj / 3 + 1 : jj / 3;
+        return NC - 1;
+    }
 };
 
 template <int NC, int L, int NACC>
@@ -150,7 +168,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
     float *s_bias = reinterpret_cast<float *>(smem + SL.bias);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
     const uint32_t rank = cluster_ctarank();
-    const int KI = p.KI, KO = p.KO, H = p.H;
+    const int KI = p.KI, KO = p.KO;
     constexpr uint32_t nops = S::NOPS;
     const uint32_t smem_base = smem_u32(smem);
     const uint32_t bars_addr = smem_base + SL.bars;
@@ -168,7 +186,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
         fence_mbar_init();
     }
     if (warp == W_ISSUE) tmem_alloc_cg2(&s_tmem_base, 512);
-    for (int i = threadIdx.x; i < 3 * H + KO + 4; i += NTHREADS) s_bias[i] = p.bias[i];
+    for (int i = threadIdx.x; i < KO + 4; i += NTHREADS) s_bias[i] = p.bias[i];
     for (int i = threadIdx.x; i < (int)(p.res_bytes / 16); i += NTHREADS)
         reinterpret_cast<uint4 *>(smem + SL.res)[i] = reinterpret_cast<const uint4 *>(p.resimg + (size_t)rank * p.res_bytes)[i];
     fence_proxy_async();                                  // resident tiles are read by the tensor core (async proxy)
@@ -238,6 +256,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             const uint32_t slots_lo = (smem_base + SL.slots) >> 4, slot_step = p.slot_bytes >> 4;
             // descriptor words: lo = addr/16 | (lbo/16) << 16, hi = sbo/16 | version 1 << 14 | layout << 29
             const uint32_t lo_noswz = (128u >> 4) << 16, hi_noswz = (((uint32_t)(KI / 8) * 128u) >> 4) | (1u << 14);
+            const uint32_t hi_noswz16 = (256u >> 4) | (1u << 14);          // one K-step wide tile (the layer-2 bias rows)
             const uint32_t lo_sw128 = (16u >> 4) << 16, hi_sw128 = (1024u >> 4) | (1u << 14) | (2u << 29);
             const uint32_t id128 = idesc_f16(256, CN), id16 = idesc_f16(256, 16), id0 = idesc_f16(256, 0);
             const uint32_t nslots = (uint32_t)p.nslots;
@@ -245,10 +264,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             uint32_t slot = 0, wpar = 0, slot_lo = slots_lo;
             uint32_t ph = 0;                             // parity of the next phase to wait for, one bit per barrier id
 #ifdef TC_PROF
-            long long pw_wait = 0, pw_wf = 0, pw_tot = clock64();
+            long long pw_wait = 0, pw_wf = 0, pw_tot = clock64(), pw_cls[4] = {0, 0, 0, 0};
+            int pw_site = 0;                             // 0 = A0FULL, 1 = prewait (accumulator / A1 chunk), 2 = consumer EDONE, 3 = D3EMPTY
 #endif
-#define WAIT(id) do { PROF_T0(); mbar_spin(BAR_ADDR(id), (ph >> (id)) & 1u); ph ^= 1u << (id); tc_fence_after(); PROF_ADD(pw_wait); } while (0)
-#define SLOT_ACQUIRE(w) do { if ((w) & SUB_NEW) { PROF_T0(); mbar_spin(BAR_ADDR(BAR_WFULL + slot), wpar); tc_fence_after(); PROF_ADD(pw_wf); } } while (0)
+#define WAIT(id) do { PROF_T0(); if (!TESTMODE) mbar_spin(BAR_ADDR(id), (ph >> (id)) & 1u); ph ^= 1u << (id); tc_fence_after(); PROF_ADD(pw_wait); PROF_ADD(pw_cls[pw_site]); } while (0)
+#define SLOT_ACQUIRE(w) do { if ((w) & SUB_NEW) { PROF_T0(); if (TESTMODE < 2) mbar_spin(BAR_ADDR(BAR_WFULL + slot), wpar); tc_fence_after(); PROF_ADD(pw_wf); } } while (0)
 #define SLOT_RELEASE(w) do { if ((w) & SUB_END) { mma_commit_cg2(BAR_ADDR(BAR_WEMPTY + slot)); slot_lo += slot_step; \
                              if (++slot == nslots) { slot = 0; wpar ^= 1u; slot_lo = slots_lo; } } } while (0)
             for (long long ti = 0; ti < ntl; ++ti) {
@@ -257,13 +277,13 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                 uint32_t si = 0;
                 asm volatile("" : "+r"(si));
                 uint32_t w = p.sub[si];                      // current table word; the next one is always loaded one step ahead
-                WAIT(BAR_A0FULL);
+                PROF_SITE(0); WAIT(BAR_A0FULL);
                 // consumer of tile-local op jc (jc is a compile-time constant after unrolling)
                 auto consume = [&](const int jc) {
                     const int type = S::type(jc);
                     if (type == T_L1S) return;
-                    WAIT(BAR_EDONE + jc % NACC);
-                    if (jc == S::FIRST_INPLACE) WAIT(BAR_D3EMPTY);              // first write into D3 of this tile
+                    PROF_SITE(2); WAIT(BAR_EDONE + jc % NACC);
+                    if (jc == S::FIRST_INPLACE) { PROF_SITE(3); WAIT(BAR_D3EMPTY); }              // first write into D3 of this tile
                     const uint32_t a_t = tmem + (uint32_t)(jc % NACC) * CN;
                     if (type == T_P) {                                          // resident P2 tile of this chunk, N = 16
                         const uint32_t b_lo = (res_lo + (uint32_t)S::chunk(jc) * (2048u >> 4)) | lo_sw128;
@@ -289,13 +309,22 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                     uint32_t jj = (uint32_t)j;
                     asm volatile("" : "+r"(jj));
                     const uint32_t pw = p.prewait[jj];      // pending chunk epilogues this op depends on (accumulator reuse, A1 chunks)
+                    PROF_SITE(1);
                     if (pw & 1u) WAIT(BAR_EDONE + 0);
                     if (NACC > 1 && (pw & 2u)) WAIT(BAR_EDONE + 1);
                     if (NACC > 2 && (pw & 4u)) WAIT(BAR_EDONE + 2);
                     const uint32_t d = tmem + (uint32_t)acc * CN;
                     if (type == T_L2) {
                         const uint32_t nb = p.nblk[jj - (uint32_t)(j - c)];
-                        uint32_t accum = 0;
+                        {   // D = [1 1 x'..] . [b2_hi b2_lo 0..]^T: the bias, and the overwrite of the accumulator
+                            const uint32_t wn = p.sub[++si];
+                            SLOT_ACQUIRE(w);
+                            mma_ts_cg2(d, tm_a0, (slot_lo + (w & SUB_OFF_MASK)) | lo_noswz, hi_noswz16, id128, 0u);
+                            SLOT_RELEASE(w);
+                            w = wn;
+                        }
+                        if (j == S::NOPS - 1) mma_commit_cg2(BAR_ADDR(BAR_A0FREE));            // last reader of A0 in a two-layer tile
+                        const uint32_t accum = 1u;
 #pragma unroll 1
                         for (uint32_t b = 0; b < nb; ++b) {
                             const uint32_t wn = p.sub[++si];
@@ -308,11 +337,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                                 mma_ss_cg2(d, a_lo + 2, hi_sw128, b_lo + 2, hi_sw128, id128, 1u);
                                 mma_ss_cg2(d, a_lo + 4, hi_sw128, b_lo + 4, hi_sw128, id128, 1u);
                                 mma_ss_cg2(d, a_lo + 6, hi_sw128, b_lo + 6, hi_sw128, id128, 1u);
-                                accum = 1u;
                             } else {
 #pragma unroll
                                 for (uint32_t ks = 0; ks < 4; ++ks)
-                                    if ((kmask >> ks) & 1u) { mma_ss_cg2(d, a_lo + 2 * ks, hi_sw128, b_lo + 2 * ks, hi_sw128, id128, accum); accum = 1u; }
+                                    if ((kmask >> ks) & 1u) mma_ss_cg2(d, a_lo + 2 * ks, hi_sw128, b_lo + 2 * ks, hi_sw128, id128, accum);
                             }
                             SLOT_RELEASE(w);
                             w = wn;
@@ -333,7 +361,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                         w = wn;
                     }
                     mma_commit_cg2(BAR_ADDR(BAR_FULL + acc));
-                    if (j == S::LAST_A0) mma_commit_cg2(BAR_ADDR(BAR_A0FREE));                 // A0 may be rebuilt for the next tile
+                    if (L == 1 && j == S::LAST_A0) mma_commit_cg2(BAR_ADDR(BAR_A0FREE));       // A0 may be rebuilt for the next tile
                     if (L == 2 && j == S::NOPS - 1) mma_commit_cg2(BAR_ADDR(BAR_A1FREE));      // A1 may be rewritten by the next tile
                     if (j >= S::LAG) consume(j - S::LAG);
                 }
@@ -342,7 +370,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                 mma_commit_cg2(BAR_ADDR(BAR_D3FULL));
             }
 #ifdef TC_PROF
-            if (p.prof) { long long *pr = p.prof + (size_t)blockIdx.x * 32; pr[0] = clock64() - pw_tot; pr[1] = pw_wait; pr[3] = pw_wf; pr[5] = ntl; }
+            if (p.prof) { long long *pr = p.prof + (size_t)blockIdx.x * 32; pr[0] = clock64() - pw_tot; pr[1] = pw_wait; pr[3] = pw_wf; pr[5] = ntl; pr[28] = pw_cls[0]; pr[29] = pw_cls[1]; pr[30] = pw_cls[2]; pr[31] = pw_cls[3]; }
 #endif
 #undef WAIT
 #undef SLOT_ACQUIRE
@@ -351,39 +379,39 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
         __syncwarp();
     } else if (warp >= W_EPI) {
         // =========================== chunk epilogue groups: ops alternate between the two groups ===========================
-        const uint32_t grp = (uint32_t)(warp - W_EPI) >> 2;
+        const uint32_t grp = (uint32_t)(warp - W_EPI) >> 2;          // = the accumulator this group serves (groups >= NACC idle)
         const uint32_t row = (uint32_t)((warp & 3) * 32 + lane);
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;     // TMEM lane quadrant of this warp
         const uint32_t a1_row = smem_base + SL.a1 + (row >> 3) * 1024u + (row & 7u) * 128u, sw = row & 7u;
         uint32_t fb = 0;                                   // bit a: parity of accumulator a's first FULL phase of this tile
-        long long pe_wait = 0, pe_a1 = 0, pe_tot = clock64(), pe_fence = 0, pe_arr = 0;
-        (void)pe_wait; (void)pe_a1; (void)pe_tot; (void)pe_fence; (void)pe_arr;
-        for (long long ti = 0; ti < ntl; ++ti, fb ^= p.cntmask)
-        for (uint32_t j = grp; j < nops; j += 2) {
+        long long pe_wait = 0, pe_a1 = 0, pe_tot = clock64(), pe_fence = 0, pe_arr = 0, pe_ld = 0;
+        (void)pe_wait; (void)pe_a1; (void)pe_tot; (void)pe_fence; (void)pe_arr; (void)pe_ld;
+        if (grp < (uint32_t)NACC && !TESTMODE)
+        for (long long ti = 0; ti < ntl; ++ti, fb ^= p.cntmask) {
+        bool a1_waited = false;
+        for (uint32_t j = grp, q = 0; j < nops; j += NACC, ++q) {
             const uint32_t type = p.optype[j], c = p.opchunk[j];
-            const uint32_t q = (NACC == 2) ? (j >> 1) : ((NACC == 3) ? ((j * 11u) >> 5) : j), acc = j - q * NACC;   // j / NACC, j % NACC (j < 32)
+            const uint32_t acc = grp;
             { PROF_T0(); mbar_wait(&bars[BAR_FULL + acc], ((fb >> acc) ^ q) & 1u); PROF_ADD(pe_wait); }
             tc_fence_after();
-            if (L == 2 && ti > 0 && j == grp) {            // once per tile: the previous tile's layer-2 MMAs have read A1
+            // before this group's first write into A1: the previous tile's layer-2 MMAs have read it.  (Only groups that
+            // write A1 wait, at a layer-1 op: by the time a layer-2 accumulator is full the barrier may already be a phase
+            // further, and a parity wait two phases behind blocks.)
+            if (L == 2 && ti > 0 && type == T_L1S && !a1_waited) {
                 PROF_T0(); mbar_wait(&bars[BAR_A1FREE], (uint32_t)(ti - 1) & 1u); PROF_ADD(pe_a1);
+                a1_waited = true;
             }
             const uint32_t d_addr = tmem + lane_base + acc * CN;
-            const float *bias = s_bias + (type == T_P ? 0 : (type == T_L2 ? 2 * H : H)) + c * CN;
             uint32_t va[32], vb[32];
             tmem_ld32p(d_addr, va);
 #pragma unroll
             for (int pc = 0; pc < 4; ++pc) {
                 uint32_t *v = (pc & 1) ? vb : va;
-                tmem_wait_ld();
+                { PROF_T0(); tmem_wait_ld(); PROF_ADD(pe_ld); }
                 if (pc < 3) tmem_ld32p(d_addr + 32 * (pc + 1), (pc & 1) ? va : vb);     // next piece in flight
-                const float4 *bp = reinterpret_cast<const float4 *>(bias + 32 * pc);
-                uint32_t w[16];
+                uint32_t w[16];                                // the bias is already in the accumulator (constant input columns)
 #pragma unroll
-                for (int j4 = 0; j4 < 8; ++j4) {
-                    const float4 bb = bp[j4];
-                    w[2 * j4] = cvt_relu_f16x2(__uint_as_float(v[4 * j4]) + bb.x, __uint_as_float(v[4 * j4 + 1]) + bb.y);
-                    w[2 * j4 + 1] = cvt_relu_f16x2(__uint_as_float(v[4 * j4 + 2]) + bb.z, __uint_as_float(v[4 * j4 + 3]) + bb.w);
-                }
+                for (int j2 = 0; j2 < 16; ++j2) w[j2] = cvt_relu_f16x2(__uint_as_float(v[2 * j2]), __uint_as_float(v[2 * j2 + 1]));
                 if (type == T_L1S) {
                     // 32 hidden units = 64 B of this row: four 16-byte pieces of K-block 2c + pc/2, 128B swizzle
                     const uint32_t kb_addr = a1_row + (2 * c + (uint32_t)(pc >> 1)) * 16384u;
@@ -404,8 +432,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             if (lane == 0) mbar_arrive_leader(BAR_ADDR(BAR_EDONE + acc), rank);
             __syncwarp(); PROF_ADD(pe_arr); }
         }
+        }
 #ifdef TC_PROF
-        if (p.prof && lane == 0 && (warp == W_EPI || warp == W_EPI + 4)) { long long *pr = p.prof + (size_t)blockIdx.x * 32 + (warp == W_EPI ? 6 : 11); pr[0] = clock64() - pe_tot; pr[1] = pe_wait; pr[2] = pe_a1; pr[3] = pe_fence; pr[4] = pe_arr; }
+        if (p.prof && lane == 0 && (warp & 3) == 0) { long long *pr = p.prof + (size_t)blockIdx.x * 32 + (grp == 0 ? 6 : (grp == 1 ? 11 : 23)); pr[0] = clock64() - pe_tot; pr[1] = pe_wait; pr[2] = pe_ld; pr[3] = pe_fence; pr[4] = pe_arr; }
 #endif
     } else {
         // =========================== tile warps: A0 of the next tile, contraction, final epilogue ===========================
@@ -413,7 +442,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
         const int row = q * 32 + lane;
         const uint32_t lane_base = (uint32_t)(q * 32) << 16;
         const uint32_t d3_addr = tmem + lane_base + p.tm_d3, a0_addr = tmem + lane_base + p.tm_a0;
-        const float *s_b3 = s_bias + 3 * H, *s_c2 = s_bias + 3 * H + KO;
+        const float *s_b3 = s_bias, *s_c2 = s_bias + KO;
         const uint32_t zero16[16] = {0};
 
         struct RowState { long long sb, i; ulonglong2 xp, xq; float2 b0; };
@@ -426,7 +455,10 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             } else { r.i = p.B; r.xp = make_ulonglong2(0, 0); r.xq = r.xp; r.b0 = make_float2(0.f, 0.f); }
         };
         // (a2) A0: +-1 fp16, one row per thread = one TMEM lane, 16 inputs = 8 columns per K-step
-        auto build_a0 = [&](ulonglong2 zp) {
+        // K index 0 and 1 are the constant +1 columns that carry the hidden-layer biases (hi + lo fp16 parts); position d
+        // of the configuration sits at K index d + 2
+        auto build_a0 = [&](ulonglong2 zq) {
+            const ulonglong2 zp = make_ulonglong2((zq.x << 2) | 3ull, (zq.y << 2) | (zq.x >> 62));
             for (int kc = 0; kc < KI / 16; ++kc) {
                 const uint32_t bits = (uint32_t)(shr128(zp, kc * 16) & 0xFFFFull);
                 uint32_t w[8];
@@ -467,7 +499,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
         float mr = (p.mode == 1 && p.hm.has_diag) ? 1.0f : 0.0f;     // the f = 0 group has ratio exactly 1
         long long pt_a0 = 0, pt_d3 = 0, pt_tot = clock64(), pt_s = 0, pt_fin = 0;
         (void)pt_a0; (void)pt_d3; (void)pt_tot; (void)pt_s; (void)pt_fin;
-        if (ntl > 0) {
+        if (ntl > 0 && !TESTMODE) {
             const long long t = 2 * q_lo + rank;
             const bool valid = t < ntiles;
             load_row(t / Gnd, valid, cur);
@@ -476,7 +508,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             clamp_of(zp, fm, inval);
             build_a0(zp);
         }
-        for (long long ti = 0; ti < ntl; ++ti) {
+        for (long long ti = 0; ti < (TESTMODE ? 0 : ntl); ++ti) {
             const long long t = 2 * (q_lo + ti) + rank;
             const bool valid = t < ntiles;
             const long long g = p.g_begin + (t % Gnd);
@@ -655,7 +687,7 @@ struct TcShape { int KI, KO, NC, nacc, nslots; uint32_t slot; };
 static bool tc_shape(const nqs_made *M, TcShape *out) {
     if ((M->L != 1 && M->L != 2) || M->h % CN != 0 || M->h < CN || M->h > CN * MAX_NC) return false;
     TcShape s;
-    s.KI = round16(M->n); s.KO = round16(M->n + 4); s.NC = M->h / CN;
+    s.KI = round16(M->n + 2); s.KO = round16(M->n + 4); s.NC = M->h / CN;      // + 2: the constant bias columns
     if (s.KI > 128 || s.KO > 144) return false;
     // TMEM: nacc accumulators of CN columns, D3 (KO), A0 (KI/2)
     s.nacc = 3;
@@ -668,8 +700,10 @@ static bool tc_shape(const nqs_made *M, TcShape *out) {
     const uint32_t fixed = smem_layout(M->h, s.KO, M->L, 0, 0).total;
     if (fixed + 2 * need > budget) return false;
     const uint32_t ring = budget - fixed;
-    int ns = 4;                                                                // few, large fills: every ring hand-over costs the issuer a poll
-    while (ns > 2 && (ring / ns) / 1024 * 1024 < 2 * need) --ns;
+    // Two large slots (plain double buffering).  Measured: a bulk copy costs its issuing warp ~590 cycles whatever its size
+    // (2 KB .. 64 KB), and every hand-over costs the MMA issuer ~220 cycles, so fewer and larger fills win: 2 x 40 KB ran
+    // 4 % faster than 4 x 20 KB and 16 % faster than 8 x 10 KB on the 76-qubit workload.
+    int ns = 2;
     uint32_t slot = (ring / ns) / 1024 * 1024;
     if (slot < need) return false;
     if (slot > 0x1FFFu * 16u) slot = 0x1FFFu * 16u / 1024 * 1024;
@@ -707,17 +741,21 @@ int tc_pack_upload(const nqs_made *M) {
 
     // ---- the per-tile op list (must match the issuer / epilogue loops of eloc_tc_kernel) ----
     int nops = 0;
+    auto push_op = [&](uint8_t t, int c) {
+        P->optype[nops] = t; P->opchunk[nops] = (uint8_t)c;
+        if (t != T_L2) P->last_a0_op = nops;
+        if (t == T_L2) P->last_l2_op = nops;
+        ++nops;
+    };
     if (L == 2) {
-        for (int c = 0; c < NC; ++c) { P->optype[nops] = T_L1S; P->opchunk[nops++] = (uint8_t)c; }
+        push_op(T_L1S, 0);
         for (int c = 0; c < NC; ++c) {
-            P->optype[nops] = T_P; P->opchunk[nops] = (uint8_t)c; P->last_a0_op = nops++;
-            P->optype[nops] = T_L2; P->opchunk[nops] = (uint8_t)c; P->last_l2_op = nops++;
+            if (c + 1 < NC) push_op(T_L1S, c + 1);
+            push_op(T_P, c);
+            push_op(T_L2, c);
         }
     } else {
-        for (int c = 0; c < NC; ++c) {
-            P->optype[nops] = T_L1I; P->opchunk[nops++] = (uint8_t)c;
-            P->optype[nops] = T_P; P->opchunk[nops] = (uint8_t)c; P->last_a0_op = nops++;
-        }
+        for (int c = 0; c < NC; ++c) { push_op(T_L1I, c); push_op(T_P, c); }
     }
     P->nops = nops;
 
@@ -755,10 +793,15 @@ int tc_pack_upload(const nqs_made *M) {
         for (int r = 0; r < 2; ++r)
             for (int rr = 0; rr < HALF; ++rr) {
                 const int j = c * CN + r * HALF + rr;
+                const float bj = phase ? M->c1[j] : M->bias[0][j];
+                const float bj_hi = __half2float(__float2half_rn(bj));
                 for (int k = 0; k < KI; ++k) {
-                    float v = 0.f;
-                    if (phase) { if (k < n - 2) v = M->p1[(size_t)j * (n - 2) + k]; }
-                    else if (k < n) v = W1[(size_t)j * n + k];
+                    float v = 0.f;                              // K index 0, 1: bias (hi, lo) against the constant +1 inputs
+                    const int d = k - 2;
+                    if (k == 0) v = bj_hi;
+                    else if (k == 1) v = bj - bj_hi;
+                    else if (phase) { if (d < n - 2) v = M->p1[(size_t)j * (n - 2) + d]; }
+                    else if (d < n) v = W1[(size_t)j * n + d];
                     put(img[r], base + noswz_offset(rr, k, KI), v);
                     if (v != 0.0f && k / 16 + 1 > nk) nk = k / 16 + 1;
                 }
@@ -776,6 +819,17 @@ int tc_pack_upload(const nqs_made *M) {
     // layer-2 chunk c2: k-blocks of 64 with any non-zero weight, and inside a block only the non-zero K-steps
     auto l2_chunk = [&](int c2) {
         const std::vector<float> &W2 = M->wm[1];
+        {   // bias rows of the chunk, one K-step wide: K index 0, 1 = b2 (hi, lo), the rest 0 (A operand = A0's first K-step)
+            const uint32_t base = stream_alloc(HALF * 16 * 2, 0);
+            for (int r = 0; r < 2; ++r)
+                for (int rr = 0; rr < HALF; ++rr) {
+                    const float bj = M->bias[1][c2 * CN + r * HALF + rr];
+                    const float bj_hi = __half2float(__float2half_rn(bj));
+                    put(img[r], base + noswz_offset(rr, 0, 16), bj_hi);
+                    put(img[r], base + noswz_offset(rr, 1, 16), bj - bj_hi);
+                }
+            P->mma_issued += CN;
+        }
         int nb = 0, need = 0;
         for (int kb = 0; kb < H / 64; ++kb) {
             uint32_t kmask = 0;
@@ -783,8 +837,7 @@ int tc_pack_upload(const nqs_made *M) {
                 for (int k = 0; k < 64; ++k)
                     if (W2[(size_t)(c2 * CN + r) * H + kb * 64 + k] != 0.0f) kmask |= 1u << (k / 16);
             P->mma_dense += 4 * CN;
-            if (!kmask && !(nb == 0 && kb == H / 64 - 1)) continue;      // exact: an all-zero block adds 0
-            if (!kmask) kmask = 1;                                       // nothing at all: still overwrite the accumulator
+            if (!kmask) continue;                                        // exact: an all-zero block adds 0
             const uint32_t base = stream_alloc(w2_bytes, (uint32_t)kb | (kmask << 4));
             for (int r = 0; r < 2; ++r)
                 for (int rr = 0; rr < HALF; ++rr)
@@ -835,14 +888,18 @@ int tc_pack_upload(const nqs_made *M) {
     if (L == 2) P->l2need[NC - 1] = (uint8_t)(NC - 1);          // every layer-1 epilogue is waited for inside its own tile
     {
         int pending[3] = {-1, -1, -1};
+        int l1s_op[MAX_NC] = {0};
+        for (int j = 0; j < nops; ++j) if (P->optype[j] == T_L1S) l1s_op[P->opchunk[j]] = j;
         auto consumed = [&](int j) { if (P->optype[j] != T_L1S && pending[j % sh.nacc] == j) pending[j % sh.nacc] = -1; };
         for (int j = 0; j < nops; ++j) {
             const int a = j % sh.nacc;
             uint8_t pw = 0;
             if (pending[a] >= 0) { pw |= (uint8_t)(1u << a); pending[a] = -1; }
             if (P->optype[j] == T_L2)
-                for (int cn = 0; cn <= P->l2need[P->opchunk[j]]; ++cn)
-                    if (pending[cn % sh.nacc] == cn) { pw |= (uint8_t)(1u << (cn % sh.nacc)); pending[cn % sh.nacc] = -1; }
+                for (int cn = 0; cn <= P->l2need[P->opchunk[j]]; ++cn) {
+                    const int jo = l1s_op[cn], ao = jo % sh.nacc;
+                    if (pending[ao] == jo) { pw |= (uint8_t)(1u << ao); pending[ao] = -1; }
+                }
             P->prewait[j] = pw;
             pending[a] = j;
             if (j >= lag) consumed(j - lag);
@@ -861,11 +918,10 @@ int tc_pack_upload(const nqs_made *M) {
     memcpy(P->sub, sub.data(), sub.size() * 4);
     P->img_stride = (uint32_t)((img[0].size() + 255) & ~(size_t)255);
 
-    // biases: [c1 | b1 | b2 | b3 (KO) | c2]
-    std::vector<float> bias((size_t)3 * H + KO + 4, 0.f);
-    for (int j = 0; j < H; ++j) { bias[j] = M->c1[j]; bias[H + j] = M->bias[0][j]; if (L == 2) bias[2 * H + j] = M->bias[1][j]; }
-    for (int d = 0; d < n; ++d) bias[3 * H + d] = M->bias[L][d];
-    for (int o = 0; o < 4; ++o) bias[3 * H + KO + o] = M->c2[o];
+    // biases left to the final epilogue: [b3 (KO) | c2]
+    std::vector<float> bias((size_t)KO + 4, 0.f);
+    for (int d = 0; d < n; ++d) bias[d] = M->bias[L][d];
+    for (int o = 0; o < 4; ++o) bias[KO + o] = M->c2[o];
 
     std::vector<uint8_t> wboth((size_t)2 * P->img_stride, 0), rboth((size_t)2 * P->res_bytes, 0);
     for (int r = 0; r < 2; ++r) {
@@ -946,6 +1002,10 @@ extern "C" void nqs_tc_prof_buffer(long long *dev_buf) { g_tc_prof = dev_buf; }
 
 template <int NC, int L, int NACC>
 static int launch_inst(const TcParams &p, int grid, uint32_t smem_bytes, cudaStream_t st) {
+    using S = Sched<NC, L, NACC>;
+    if (p.nops != S::NOPS) return NQS_EUNSUPPORTED;
+    for (int j = 0; j < S::NOPS; ++j)                        // the host-packed op list must be the compiled schedule
+        if (p.optype[j] != S::type(j) || p.opchunk[j] != S::chunk(j)) return NQS_EUNSUPPORTED;
     // the attribute is per device and per kernel; setting it is a cheap host call, so no process-wide cache
     if (cudaFuncSetAttribute(eloc_tc_kernel<NC, L, NACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes) != cudaSuccess) {
         cudaGetLastError();
@@ -958,6 +1018,7 @@ static int launch_inst(const TcParams &p, int grid, uint32_t smem_bytes, cudaStr
 static int launch_chain(const TcPack *P, TcParams &p, long long ntiles, cudaStream_t st) {
 #ifdef TC_PROF
     p.prof = g_tc_prof;
+    p.test_mode = getenv("NQS_TC_TESTMODE") ? atoi(getenv("NQS_TC_TESTMODE")) : 0;
 #endif
     const long long npairs = (ntiles + 1) / 2;
     const long long ncl_max = P->sms / 2;
