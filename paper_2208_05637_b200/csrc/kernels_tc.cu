@@ -6,18 +6,21 @@
 //        input-layer MMAs; no shared-memory copy of the inputs exists),
 //   (a4) the MADE chain and the phase MLP as tcgen05 MMAs (fp16 operands, fp32 accumulation in TMEM), in 128-unit
 //        hidden CHUNKS that rotate through up to three 128-column TMEM accumulators:
-//          layer 1   D = A0 . W1c^T   TS  -> epilogue: +b1, ReLU, fp16 -> A1 in SHARED memory (128B-swizzled K-major)
-//          phase     D = A0 . P1c^T   TS  -> epilogue: +c1, ReLU, fp16 IN PLACE -> D3 += D . P2c^T   (TS, N = 16)
-//          layer 2   D = A1 . W2c^T   SS  -> epilogue: +b2, ReLU, fp16 IN PLACE -> D3 += D . W3c^T   (TS)
-//        (one hidden layer: layer 1 is rewritten in place and feeds W3 directly).  All-zero K-steps of the masked
-//        weights are never issued (exact: they contribute 0),
+//          layer 1   D = A0 . W1c^T   TS  -> epilogue: ReLU, fp16 -> A1 in SHARED memory (128B-swizzled K-major)
+//          phase     D = A0 . P1c^T   TS  -> epilogue: ReLU, fp16 IN PLACE -> D3 += D . P2c^T   (TS, N = 16)
+//          layer 2   D = A1 . W2c^T   SS  -> epilogue: ReLU, fp16 IN PLACE -> D3 += D . W3c^T   (TS)
+//        (one hidden layer: layer 1 is rewritten in place and feeds W3 directly).  The hidden-layer BIASES are part of
+//        the MMAs: A0 carries two constant +1 columns and every weight image two bias columns (fp16 hi + lo parts);
+//        layer 2 gets its bias from a one-K-step MMA on A0's constant columns, which also overwrites the accumulator.
+//        The chunk epilogue is therefore tcgen05.ld -> cvt.rn.relu.f16x2 -> store, nothing else (the F2FP pipe, 16
+//        lanes/clk/SM, is what bounds it).  All-zero K-steps of the masked weights are never issued (exact),
 //   (a3) the Pauli contraction S[i,g] over the group's terms (popcount parity, (-i)^r folded into c),
 //   (a5) ratio = exp(dlog|psi|) cis(dphi), E_i += S * ratio, kept in registers per sample.
-// Warp roles (14 warps per CTA): 12 = weight producers (TMA 1-D bulk copies of this CTA's half of the weight image into
-// a ring of large slots); 13 = in the leader CTA the MMA issuer (ONE elect.sync thread issues every tcgen05.mma /
+// Warp roles (14 warps per CTA): 12 = weight producer (TMA 1-D bulk copies of this CTA's half of the weight image into
+// a ring of two large slots); 13 = in the leader CTA the MMA issuer (ONE elect.sync thread issues every tcgen05.mma /
 // commit of the pair; commits are multicast to the barriers of both CTAs), in the peer CTA a forwarder that tells the
-// leader when the peer's half of a ring slot has landed; 4-7 / 8-11 = two chunk-epilogue groups (ops alternate);
-// 0-3 = tile warps (A0 of the NEXT tile, contraction, final epilogue).  DESIGN.md sections 6-7.
+// leader when the peer's half of a ring slot has landed; 4-7 / 8-11 = two chunk-epilogue groups, each serving one
+// 64-column half of every op; 0-3 = tile warps (A0 of the NEXT tile, contraction, final epilogue).  DESIGN.md 6-7.
 // PAPER.md:122-134 (Alg. 1), :84-96 (architecture, Eq. 8-10), :152-158 (Eq. 15-16).
 #include <cstdlib>
 #include <cstring>
@@ -33,7 +36,7 @@ namespace {
 constexpr int TILE_M = 128;
 constexpr int CN = 128;                  // hidden-unit chunk = accumulator columns = MMA N of the pair
 constexpr int HALF = CN / 2;             // weight rows per CTA and chunk
-constexpr int NTHREADS = 576;
+constexpr int NTHREADS = 448;
 constexpr int MAX_NC = 4;                // hidden <= 512
 constexpr int MAX_SLOTS = 8;
 constexpr int NPROD = 4;                 // producer lanes (bulk-copy issuers), never more than slots
@@ -42,7 +45,7 @@ constexpr int MAX_OPS = 3 * MAX_NC;
 // warps, and every sub-partition hosts epilogue warps (a warp reaches only TMEM lane quadrant id % 4): the one thread
 // that issues all MMAs therefore lives in the highest warp id of its sub-partition, or it only gets the issue slots
 // the epilogue warps leave over.
-constexpr int W_EPI = 4, W_PROD = 16, W_ISSUE = 17;      // warps 0-3: tile warps, 4-15: three chunk-epilogue groups
+constexpr int W_EPI = 4, W_PROD = 12, W_ISSUE = 13;      // warps 0-3: tile warps, 4-11: two chunk-epilogue groups (column halves)
 
 enum : uint8_t { T_L1S = 0, T_L1I = 1, T_P = 2, T_L2 = 3 };   // layer 1 -> smem A1 | layer 1 in place | phase hidden | layer 2
 
@@ -111,7 +114,6 @@ struct TcParams {
 #ifdef TC_PROF
 #define PROF_T0() const long long _t0 = clock64()
 #define PROF_ADD(v) (v) += clock64() - _t0
-#define PROF_STALL(sp) do { if (sp) { pw_stall += clock64() - _t0; ++pw_nstall; } ++pw_npoll; } while (0)
 #define PROF_SITE(x) pw_site = (x)
 #define TESTMODE (p.test_mode)
 #else
@@ -119,7 +121,6 @@ struct TcParams {
 #define TESTMODE 0
 #define PROF_T0() do {} while (0)
 #define PROF_ADD(v) do {} while (0)
-#define PROF_STALL(sp) do { (void)(sp); } while (0)
 #endif
 
 __device__ __forceinline__ unsigned long long shr128(ulonglong2 a, int s) {      // low 64 bits of a >> s, 0 <= s < 128
@@ -178,7 +179,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
     if (threadIdx.x == 0) {
         mbar_init(&bars[BAR_A0FULL], 8); mbar_init(&bars[BAR_A0FREE], 1); mbar_init(&bars[BAR_A1FREE], 1);
         mbar_init(&bars[BAR_D3FULL], 1); mbar_init(&bars[BAR_D3EMPTY], 8);
-        for (int a = 0; a < 3; ++a) { mbar_init(&bars[BAR_FULL + a], 1); mbar_init(&bars[BAR_EDONE + a], 8); }
+        for (int a = 0; a < 3; ++a) { mbar_init(&bars[BAR_FULL + a], 1); mbar_init(&bars[BAR_EDONE + a], 16); }   // 8 epilogue warps x 2 CTAs
         for (int s = 0; s < p.nslots; ++s) {
             mbar_init(&bars[BAR_WFULL + s], rank == 0 ? 2 : 1);      // leader: own producer + the peer's forwarder
             mbar_init(&bars[BAR_WEMPTY + s], 1);
@@ -289,7 +290,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                         const uint32_t b_lo = (res_lo + (uint32_t)S::chunk(jc) * (2048u >> 4)) | lo_sw128;
 #pragma unroll
                         for (uint32_t ks = 0; ks < 8; ++ks)
-                            mma_ts_cg2(tm_ph, a_t + 8 * ks, b_lo + (ks >> 2) * (1024u >> 4) + 2 * (ks & 3), hi_sw128, id16, 1u);
+                            mma_ts_cg2(tm_ph, a_t + 32 * (ks >> 1) + 8 * (ks & 1), b_lo + (ks >> 2) * (1024u >> 4) + 2 * (ks & 3), hi_sw128, id16, 1u);
                     } else {                                                    // streamed layer-3 tile
                         const uint32_t wn = p.sub[++si];
                         SLOT_ACQUIRE(w);
@@ -298,7 +299,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                         const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_sw128, idesc = id0 | ((N >> 3) << 17);
 #pragma unroll
                         for (uint32_t ks = 0; ks < 8; ++ks)
-                            mma_ts_cg2(tm_d3 + nlo, a_t + 8 * ks, b_lo + (ks >> 2) * kb_step + 2 * (ks & 3), hi_sw128, idesc, 1u);
+                            mma_ts_cg2(tm_d3 + nlo, a_t + 32 * (ks >> 1) + 8 * (ks & 1), b_lo + (ks >> 2) * kb_step + 2 * (ks & 3), hi_sw128, idesc, 1u);
                         SLOT_RELEASE(w);
                         w = wn;
                     }
@@ -379,51 +380,60 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
         __syncwarp();
     } else if (warp >= W_EPI) {
         // =========================== chunk epilogue groups: ops alternate between the two groups ===========================
-        const uint32_t grp = (uint32_t)(warp - W_EPI) >> 2;          // = the accumulator this group serves (groups >= NACC idle)
+        // Every op is served by BOTH groups, each taking one half of the accumulator's columns (two 32-column pieces), so
+        // that the hand-over round trip commit -> epilogue -> arrive is half as long.  An in-place op keeps each piece's
+        // fp16 result inside the piece's own columns [32 pc, 32 pc + 16): no piece ever writes what another still reads.
+        const uint32_t grp = (uint32_t)(warp - W_EPI) >> 2;
         const uint32_t row = (uint32_t)((warp & 3) * 32 + lane);
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;     // TMEM lane quadrant of this warp
         const uint32_t a1_row = smem_base + SL.a1 + (row >> 3) * 1024u + (row & 7u) * 128u, sw = row & 7u;
         uint32_t fb = 0;                                   // bit a: parity of accumulator a's first FULL phase of this tile
-        long long pe_wait = 0, pe_a1 = 0, pe_tot = clock64(), pe_fence = 0, pe_arr = 0, pe_ld = 0;
-        (void)pe_wait; (void)pe_a1; (void)pe_tot; (void)pe_fence; (void)pe_arr; (void)pe_ld;
-        if (grp < (uint32_t)NACC && !TESTMODE)
+        long long pe_wait = 0, pe_a1 = 0, pe_tot = clock64(), pe_fence = 0, pe_arr = 0, pe_ld = 0, pe_ldi = 0, pe_cvt = 0;
+        (void)pe_wait; (void)pe_a1; (void)pe_tot; (void)pe_fence; (void)pe_arr; (void)pe_ld; (void)pe_ldi; (void)pe_cvt;
+        if (!TESTMODE)
         for (long long ti = 0; ti < ntl; ++ti, fb ^= p.cntmask) {
         bool a1_waited = false;
-        for (uint32_t j = grp, q = 0; j < nops; j += NACC, ++q) {
+        uint32_t acc = 0, q = 0;                           // j % NACC, j / NACC
+        for (uint32_t j = 0; j < nops; ++j) {
             const uint32_t type = p.optype[j], c = p.opchunk[j];
-            const uint32_t acc = grp;
             { PROF_T0(); mbar_wait(&bars[BAR_FULL + acc], ((fb >> acc) ^ q) & 1u); PROF_ADD(pe_wait); }
             tc_fence_after();
-            // before this group's first write into A1: the previous tile's layer-2 MMAs have read it.  (Only groups that
-            // write A1 wait, at a layer-1 op: by the time a layer-2 accumulator is full the barrier may already be a phase
-            // further, and a parity wait two phases behind blocks.)
+            // before the first write into A1: the previous tile's layer-2 MMAs have read it
             if (L == 2 && ti > 0 && type == T_L1S && !a1_waited) {
                 PROF_T0(); mbar_wait(&bars[BAR_A1FREE], (uint32_t)(ti - 1) & 1u); PROF_ADD(pe_a1);
                 a1_waited = true;
             }
-            const uint32_t d_addr = tmem + lane_base + acc * CN;
+            const uint32_t d_addr = tmem + lane_base + acc * CN + 64u * grp;
             uint32_t va[32], vb[32];
+            { PROF_T0();
             tmem_ld32p(d_addr, va);
+            tmem_ld32p(d_addr + 32, vb);
+            PROF_ADD(pe_ldi); }
+            { PROF_T0(); tmem_wait_ld(); PROF_ADD(pe_ld); }
+#ifdef TC_PROF
+            const long long _tc0 = clock64();
+#endif
 #pragma unroll
-            for (int pc = 0; pc < 4; ++pc) {
-                uint32_t *v = (pc & 1) ? vb : va;
-                { PROF_T0(); tmem_wait_ld(); PROF_ADD(pe_ld); }
-                if (pc < 3) tmem_ld32p(d_addr + 32 * (pc + 1), (pc & 1) ? va : vb);     // next piece in flight
+            for (int pp = 0; pp < 2; ++pp) {
+                const uint32_t *v = pp ? vb : va;
                 uint32_t w[16];                                // the bias is already in the accumulator (constant input columns)
 #pragma unroll
                 for (int j2 = 0; j2 < 16; ++j2) w[j2] = cvt_relu_f16x2(__uint_as_float(v[2 * j2]), __uint_as_float(v[2 * j2 + 1]));
                 if (type == T_L1S) {
-                    // 32 hidden units = 64 B of this row: four 16-byte pieces of K-block 2c + pc/2, 128B swizzle
-                    const uint32_t kb_addr = a1_row + (2 * c + (uint32_t)(pc >> 1)) * 16384u;
+                    // this group's 64 hidden units are K-block 2c + grp of A1; 32 units = four 16-byte pieces, 128B swizzle
+                    const uint32_t kb_addr = a1_row + (2 * c + grp) * 16384u;
 #pragma unroll
                     for (uint32_t i = 0; i < 4; ++i) {
-                        const uint32_t jj = (uint32_t)(pc & 1) * 4 + i;
+                        const uint32_t jj = (uint32_t)pp * 4 + i;
                         st_shared_v4(kb_addr + ((jj ^ sw) << 4), w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
                     }
                 } else {
-                    tmem_st16p(d_addr + 16 * pc, w);          // in place: columns [16 pc, 16 pc + 16) were read by piece pc / 2 <= pc
+                    tmem_st16p(d_addr + 32 * pp, w);          // in place, inside the piece's own columns
                 }
             }
+#ifdef TC_PROF
+            pe_cvt += clock64() - _tc0;
+#endif
             { PROF_T0();
             if (type == T_L1S) fence_proxy_async(); else tmem_wait_st();
             tc_fence_before();
@@ -431,10 +441,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             { PROF_T0();
             if (lane == 0) mbar_arrive_leader(BAR_ADDR(BAR_EDONE + acc), rank);
             __syncwarp(); PROF_ADD(pe_arr); }
+            if (++acc == (uint32_t)NACC) { acc = 0; ++q; }
         }
         }
 #ifdef TC_PROF
-        if (p.prof && lane == 0 && (warp & 3) == 0) { long long *pr = p.prof + (size_t)blockIdx.x * 32 + (grp == 0 ? 6 : (grp == 1 ? 11 : 23)); pr[0] = clock64() - pe_tot; pr[1] = pe_wait; pr[2] = pe_ld; pr[3] = pe_fence; pr[4] = pe_arr; }
+        if (p.prof && lane == 0 && (warp & 3) == 0) { long long *pr = p.prof + (size_t)blockIdx.x * 32 + (grp == 0 ? 6 : 11); pr[0] = clock64() - pe_tot; pr[1] = pe_wait; pr[2] = pe_ld; pr[3] = pe_fence; pr[4] = pe_arr; long long *pa = p.prof + (size_t)blockIdx.x * 32 + (grp == 0 ? 23 : 25); pa[0] = pe_ldi; pa[1] = pe_cvt; }
 #endif
     } else {
         // =========================== tile warps: A0 of the next tile, contraction, final epilogue ===========================
