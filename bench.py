@@ -95,21 +95,64 @@ def build_inputs(cfg, need_samples):
     return w, (x, z, c), params, samples, counts
 
 
-def time_oracle(w, ham, params, samples, n_samples):
-    """The oracle as it stands (fp64 numpy, memoised mode) on the host cores; returns (pairs/s, seconds, threads)."""
+def time_oracle(w, ham, params, samples, n_samples, one_thread=False):
+    """The oracle as it stands (fp64 numpy, memoised mode) on the host cores; returns (pairs/s, seconds, threads).
+    one_thread=True pins the BLAS pool the oracle's matmuls run on to a single thread (the oracle is
+    timed on all cores and on one)."""
+    import contextlib
     from paper_2208_05637_b200 import workloads as wl
     from oracle import eloc as oeloc
     x, z, c = ham
     codes = wl.masks_to_codes(x, z, w.n_qubits)
+    limit = contextlib.nullcontext()
     try:
-        from threadpoolctl import threadpool_info
+        from threadpoolctl import threadpool_info, threadpool_limits
         threads = max([p.get("num_threads", 1) for p in threadpool_info()] or [1])
+        if one_thread:
+            limit, threads = threadpool_limits(limits=1), 1
     except Exception:
         threads = os.cpu_count()
-    t0 = time.perf_counter()
-    oeloc.local_energy(codes, c, params, samples[:n_samples], memo=True)
-    dt = time.perf_counter() - t0
+    with limit:
+        t0 = time.perf_counter()
+        oeloc.local_energy(codes, c, params, samples[:n_samples], memo=True)
+        dt = time.perf_counter() - t0
     return n_samples * len(c) / dt, dt, threads
+
+
+# DRAM bytes (read + write) of ONE full-size eloc_tc_kernel launch (cfg 5, 8,192 samples x all groups), from the
+# `ncu --set full` capture summarised in profiles/r2_final_summary.md.  A constant of that capture, not measured live.
+NCU_DRAM_BYTES_PER_LAUNCH = {5: None}
+
+
+def time_contraction(nqs, torch, H, xs, stream, clocks_mhz):
+    """Standalone Pauli contraction (a3, nqs_pauli_contract) of one mini-batch against ALL groups, in group chunks
+    that reuse one output buffer (S is never materialised whole: B x G x 8 bytes would be 38 GB at cfg 5).
+    ALU roofline: 148 SM x 128 INT/FP32 lanes x SM clock; 7 lane-operations per (sample, term) pair for n <= 128
+    (2 AND + 2 POPC + parity add/select + 2 sign-injected FP32 adds)."""
+    B, G, K = xs.shape[0], H.G, H.K
+    chunk = max(1, min(G, (256 << 20) // (B * 8)))
+    out = torch.empty((chunk, B, 2), dtype=torch.float32, device=xs.device)
+    L = nqs.lib()
+
+    def sweep():
+        for g0 in range(0, G, chunk):
+            g1 = min(G, g0 + chunk)
+            rc = L.nqs_pauli_contract(H._h, xs.data_ptr(), B, g0, g1, out.data_ptr(), stream.cuda_stream)
+            assert rc == 0, rc
+    sweep()
+    torch.cuda.synchronize()
+    e0, e1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+    e0.record(stream)
+    sweep()
+    e1.record(stream)
+    torch.cuda.synchronize()
+    ms = e0.elapsed_time(e1)
+    pairs_s = B * K / (ms / 1e3)
+    peak = 148 * 128 * clocks_mhz * 1e6
+    return {"value": pairs_s, "unit": "pairs/s", "ms": ms, "launches": (G + chunk - 1) // chunk,
+            "lane_ops_per_pair": 7, "alu_peak_lane_ops_per_s": peak, "alu_frac": 7 * pairs_s / peak,
+            "hbm_write_gbs": B * G * 8 / (ms / 1e3) / 1e9,
+            "note": "standalone nqs_pauli_contract over all groups; S chunks are written to HBM (the fused path keeps them in registers)"}
 
 
 def main():
@@ -122,6 +165,7 @@ def main():
     ap.add_argument("--cfg", type=int, default=5)
     ap.add_argument("--oracle-samples", type=int, default=0, help="samples for the cpu_baseline leg (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-contraction", action="store_true", help="skip the standalone contraction figure")
     ap.add_argument("--mb-samples", type=int, default=0,
                     help="profiling aid: samples per step instead of the configured mini-batch (labelled in config)")
     args = ap.parse_args()
@@ -131,7 +175,7 @@ def main():
     local_rank = int(os.environ.get("LOCAL_RANK", "0"))
     from paper_2208_05637_b200 import workloads as wl
     w = wl.WORKLOADS[args.cfg]
-    n_oracle = args.oracle_samples or {1: 256, 2: 64, 3: 16, 4: 2, 5: 1}[args.cfg]
+    n_oracle = args.oracle_samples or {1: 256, 2: 64, 3: 16, 4: 4, 5: 2}[args.cfg]
     workload_name = (f"cfg{args.cfg}: {w.n_qubits} qubits, h={w.hidden}, one {args.mb_samples or w.minibatch}-sample "
                      f"mini-batch x all unique-flip groups per step" + (" [REDUCED mini-batch: profiling run]" if args.mb_samples else ""))
 
@@ -263,11 +307,24 @@ def main():
                  "algorithmic_flops_per_eval": flops_eval, "evals_per_launch": evals_per_launch,
                  "kernel_share_of_step": chain_ms / total_ms})
 
-    cpu_baseline = None
+    roof["traffic"] = NCU_DRAM_BYTES_PER_LAUNCH.get(args.cfg) if (used_tc and not args.mb_samples) else None
+    if used_tc:
+        issued, dense = M.tc_flops()
+        roof["issued_flops_per_eval"] = issued                # what the kernel sends to the tensor cores (overhead included)
+        roof["issued_over_algorithmic"] = issued / flops_eval
+
+    contraction = None
+    if not args.no_contraction:
+        contraction = time_contraction(nqs, torch, H, xs_all[:mb], stream, clocks["sm_mhz"] or peaks["sm_max_mhz"])
+
+    cpu_baseline = cpu_baseline_1 = None
     if not args.no_cpu_baseline:
         v, dt, threads = time_oracle(wq, ham, params, samples, n_oracle)
         cpu_baseline = {"value": v, "unit": UNIT, "cores": threads, "kind": "oracle", "seconds": dt,
                         "sample": f"{n_oracle} of {mb} samples of one mini-batch x all {K} terms (memoised oracle mode)"}
+        v1, dt1, _ = time_oracle(wq, ham, params, samples[n_oracle:], 1, one_thread=True)
+        cpu_baseline_1 = {"value": v1, "unit": UNIT, "cores": 1, "kind": "oracle", "seconds": dt1,
+                          "sample": f"1 of {mb} samples x all {K} terms, BLAS pool limited to one thread"}
 
     line = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
             "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
@@ -275,7 +332,8 @@ def main():
             "config": {"workload": workload_name, "n_qubits": wq.n_qubits, "n_terms": K, "n_groups": G,
                        "minibatch": mb, "hidden": wq.hidden, "path": "tc" if used_tc else "simt",
                        "l2": "flushed between timed steps (256 MiB write)", "parallelism": f"dp{world} over mini-batches"},
-            "psi_evals_per_s": evals_per_s, "roofline": roof, "cpu_baseline": cpu_baseline,
+            "psi_evals_per_s": evals_per_s, "roofline": roof, "contraction": contraction,
+            "cpu_baseline": cpu_baseline, "cpu_baseline_1thread": cpu_baseline_1,
             "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": mb * 16 + mb * 8,
                     "d2h_bytes_per_step": mb * 8 + 5 * 8},
             "gpu_launches": int(launches), "clocks": clocks}

@@ -52,10 +52,11 @@ enum nqs_status {
  *  NQS_PATH_SIMT : fp32 FFMA on CUDA cores, every layer (reference-quality, any shape).
  *  NQS_PATH_TC   : tcgen05 tensor cores driven by CTA pairs (cta_group::2), fp16 operands / fp32 accumulation in
  *                  TMEM, fused gather of x xor f into the operand tile and log|psi| / phase / ratio / E_loc in the
- *                  epilogue.  Needs n_hidden_layers in {1, 2} and hidden a multiple of 128 in [128, 512]; every
- *                  n_qubits in [3, 128] fits (two 128-column accumulators + round16(n+4) output columns +
- *                  round16(n)/2 input columns <= 512 TMEM columns; three accumulators when n <= 76).  Other shapes
- *                  return NQS_EUNSUPPORTED.
+ *                  epilogue.  Needs n_hidden_layers in {1, 2}, hidden a multiple of 128 in [128, 512] and
+ *                  n_qubits in [3, 126]: the operand tile carries two constant columns for the hidden-layer biases,
+ *                  so round16(n+2) <= 128 input columns; TMEM holds two 128-column accumulators + round16(n+4)
+ *                  output columns + round16(n+2)/2 input columns <= 512 (three accumulators when n <= 76).  Other
+ *                  shapes (n = 127, 128 included) return NQS_EUNSUPPORTED; NQS_PATH_AUTO then takes NQS_PATH_SIMT.
  *  NQS_PATH_AUTO : TC when the shape supports it and hidden >= 384 (where single-pass fp16 operands keep
  *                  |dE_loc| several times below 1e-5 sum|c| on the chemistry workloads),
  *                  else SIMT.
@@ -141,6 +142,12 @@ void nqs_made_free(nqs_made_t *made);
 /* Which kernels `path` resolves to for this model: NQS_PATH_SIMT or NQS_PATH_TC, or a negative status
  * (NQS_EUNSUPPORTED when NQS_PATH_TC is forced on an unsupported shape).  Host only. */
 int nqs_made_path(const nqs_made_t *made, int path);
+
+/* Bookkeeping for the roofline report: multiply-add flops per psi evaluation that
+ * NQS_PATH_TC ISSUES to the tensor cores (masked-zero K-steps skipped, padding and the bias K-steps included) and
+ * the flops of the same chain with nothing skipped.  Needs a device (the weight images are packed on first use);
+ * NQS_EUNSUPPORTED when the shape has no tensor-core path.  Host only, no kernel launch. */
+int nqs_made_tc_flops(const nqs_made_t *made, int64_t *issued_per_eval, int64_t *dense_per_eval);
 
 /* ---- (a4) MADE forward: Eq. 10 ---------------------------------------------------------
  * configs_dev : device uint64 [B][2]; bits >= n_qubits must be zero.

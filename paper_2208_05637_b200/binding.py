@@ -44,6 +44,7 @@ def lib():
         L.nqs_made_export_masked.argtypes = [c_void_p, c_int, c_void_p]
         L.nqs_made_free.argtypes = [c_void_p]
         L.nqs_made_path.argtypes = [c_void_p, c_int]
+        L.nqs_made_tc_flops.argtypes = [c_void_p, ctypes.POINTER(c_int64), ctypes.POINTER(c_int64)]
         L.nqs_made_free.restype = None
         L.nqs_made_logpsi.argtypes = [c_void_p, c_void_p, c_int64, c_void_p, c_int, c_void_p]
         L.nqs_pauli_contract.argtypes = [c_void_p, c_void_p, c_int64, c_int64, c_int64, c_void_p, c_void_p]
@@ -147,6 +148,12 @@ class Made:
         k = c_int64()
         _chk(lib().nqs_made_num_params(self._h, k), "nqs_made_num_params")
         return k.value
+
+    def tc_flops(self):
+        """(issued, dense) tensor-core flops per psi evaluation of NQS_PATH_TC (nqs_made_tc_flops)."""
+        a, b = c_int64(), c_int64()
+        _chk(lib().nqs_made_tc_flops(self._h, a, b), "nqs_made_tc_flops")
+        return a.value, b.value
 
     def last_chain_kernel_ms(self):
         ms, k = ctypes.c_float(), c_int()

@@ -119,6 +119,24 @@ int nqs_made_upload(const nqs_made *M) {
     if ((rc = up(t, &d.p2t))) return rc;
     if ((rc = up(M->c1, &d.c1))) return rc;
     if ((rc = up(M->c2, &d.c2))) return rc;
+    {   // kend arrays (see MadeDev)
+        auto kend_of = [&](const std::vector<float> &W, int rows, int cols, const int32_t **dst) -> int {
+            std::vector<int32_t> ke((size_t)rows, 0);
+            for (int j = 0; j < rows; ++j)
+                for (int k = cols - 1; k >= 0; --k)
+                    if (W[(size_t)j * cols + k] != 0.0f) { ke[j] = k + 1; break; }
+            void *p = nullptr;
+            const int r = upload(ke.data(), ke.size(), &p);
+            if (r) return r;
+            M->d_allocs.push_back(p);
+            *dst = (const int32_t *)p;
+            return NQS_OK;
+        };
+        d.kend2 = nullptr;
+        if ((rc = kend_of(M->wm[0], h, n, &d.kend1))) return rc;
+        if (L == 2 && (rc = kend_of(M->wm[1], h, h, &d.kend2))) return rc;
+        if ((rc = kend_of(M->wm[L], n, h, &d.kend3))) return rc;
+    }
     if (tc_supported(M) && (rc = tc_pack_upload(M))) return rc;
     M->on_device = true;
     return NQS_OK;
@@ -164,6 +182,18 @@ extern "C" int nqs_made_path(const nqs_made_t *M, int path) {
     int use_tc = 0;
     const int rc = resolve_path(M, path, &use_tc);
     return rc ? rc : (use_tc ? NQS_PATH_TC : NQS_PATH_SIMT);
+}
+
+extern "C" int nqs_made_tc_flops(const nqs_made_t *M, int64_t *issued_per_eval, int64_t *dense_per_eval) {
+    if (!M || !issued_per_eval || !dense_per_eval) return NQS_EINVAL;
+    if (!tc_supported(M)) return NQS_EUNSUPPORTED;
+    const int rc = nqs_made_upload(M);
+    if (rc) return rc;
+    long long issued = 0, dense = 0;
+    tc_mma_counts(M, &issued, &dense);             // in units of one K-step (16) x one output column, per row
+    *issued_per_eval = 32 * issued;
+    *dense_per_eval = 32 * dense;
+    return NQS_OK;
 }
 
 extern "C" int nqs_made_logpsi(const nqs_made_t *M, const uint64_t *configs_dev, int64_t B, float *out_dev,

@@ -18,10 +18,11 @@ __device__ __forceinline__ int bit128(ulonglong2 a, int q) {
 __device__ __forceinline__ float log_sigmoid(float t) { return fminf(t, 0.0f) - log1pf(expf(-fabsf(t))); }
 
 // out[j][r] = act(b[j] + sum_k Wt[k][j] * in[k][r]),  in/out are smem tiles [.][TR]; Wt is [K][ldw] global.
-// Work item = (output j, group of RPT rows); items are strided over the CTA.
+// Work item = (output j, group of RPT rows); items are strided over the CTA.  kend (or NULL): output j has no non-zero
+// weight at k >= kend[j] (masked layers), so the sum stops there — exact, the skipped terms are w = 0.
 template <int RPT, bool RELU>
 __device__ __forceinline__ void layer_fwd(const float *__restrict__ Wt, int ldw, const float *__restrict__ bias,
-                                          int K, int N, const float *in, float *out) {
+                                          int K, int N, const float *in, float *out, const int32_t *__restrict__ kend = nullptr) {
     constexpr int RG = TR / RPT;
     for (int item = threadIdx.x; item < N * RG; item += NT) {
         const int j = item % N, rg = item / N;
@@ -30,8 +31,9 @@ __device__ __forceinline__ void layer_fwd(const float *__restrict__ Wt, int ldw,
 #pragma unroll
         for (int r = 0; r < RPT; ++r) acc[r] = b;
         const float *inp = in + rg * RPT;
+        const int kstop = kend ? min(K, __ldg(kend + j)) : K;
 #pragma unroll 4
-        for (int k = 0; k < K; ++k) {
+        for (int k = 0; k < kstop; ++k) {
             const float w = __ldg(Wt + (size_t)k * ldw + j);
             if constexpr (RPT >= 4) {
 #pragma unroll
@@ -101,15 +103,15 @@ __device__ void forward_tile(const MadeDev &m, const Smem &s) {
         s.bad[r] = valid ? 0.0f : 1.0f;
     }
     __syncthreads();
-    layer_fwd<TR, true>(m.w1t, h, m.b1, n, h, s.U, s.X);
+    layer_fwd<TR, true>(m.w1t, h, m.b1, n, h, s.U, s.X, m.kend1);
     __syncthreads();
     const float *hid = s.X;
     if (m.L == 2) {
-        layer_fwd<TR, true>(m.w2t, h, m.b2, h, h, s.X, s.Y);
+        layer_fwd<TR, true>(m.w2t, h, m.b2, h, h, s.X, s.Y, m.kend2);
         __syncthreads();
         hid = s.Y;
     }
-    layer_fwd<4, false>(m.w3t, m.npad, m.b3, h, n, hid, s.A);
+    layer_fwd<4, false>(m.w3t, m.npad, m.b3, h, n, hid, s.A, m.kend3);
     float *ph = (m.L == 2) ? s.X : s.Y;                 // a free [h][TR] buffer
     __syncthreads();                                     // (L==2: X no longer read by layer 2)
     layer_fwd<TR, true>(m.p1t, h, m.c1, n, h, s.U, ph);
@@ -379,7 +381,7 @@ int launch_contract(const HamDev &hm, const ulonglong2 *x, long long B, long lon
                     cudaStream_t st) {
     if (B <= 0 || g1 <= g0) return NQS_OK;
     const long long nb = (B + CT_THREADS - 1) / CT_THREADS;
-    long long gs = (2ll * num_sms() + nb - 1) / nb;
+    long long gs = (8ll * num_sms() + nb - 1) / nb;           // ~8 resident CTAs (32 warps) per SM: the term loop is latency-bound below that
     if (gs > g1 - g0) gs = g1 - g0;
     if (gs < 1) gs = 1;
     if (gs > 65535) gs = 65535;

@@ -32,6 +32,9 @@ struct MadeDev {
     const float *p1t;            // [n][h]   phase layer 1; rows n-2, n-1 are zero
     const float *p2t;            // [h][4]
     const float *c1, *c2;        // [h], [4]
+    // exact work avoidance on the masked layers: output j of a layer needs inputs k < kend[j] only (1 + the last
+    // non-zero masked weight of its row; for sorted degrees the masks are prefixes), the rest multiply exact zeros
+    const int32_t *kend1, *kend2, *kend3;   // [h], [h] (NULL when L == 1), [n]
     // Hamming-weight constraint (Eq. 14; n_up < 0 = off): conditionals clamped to 0 / 1 contribute
     // log 1 = 0 to log|psi|; strings that violate Eq. 12 have psi = 0
     int n_up, n_down;

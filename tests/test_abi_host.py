@@ -134,14 +134,21 @@ def test_compute_entry_points_fail_loudly_without_gpu():
 
 def test_tensor_core_path_shape_limits():
     """include/nqs.h: NQS_PATH_TC takes n_hidden_layers in {1, 2}, hidden a multiple of 128 in [128, 512] and every
-    n_qubits in [3, 128]; everything else is NQS_EUNSUPPORTED (host-only query, no GPU needed)."""
+    n_qubits in [3, 126] (two operand columns carry the biases: round16(n + 2) <= 128); everything else is
+    NQS_EUNSUPPORTED and NQS_PATH_AUTO falls to the fp32 path (host-only query, no GPU needed)."""
     from paper_2208_05637_b200 import workloads as wl
-    for n in (3, 4, 16, 17, 64, 76, 77, 80, 96, 112, 127, 128):
+    for n in (3, 4, 14, 15, 16, 17, 64, 76, 77, 80, 96, 112, 126):
         for h in (128, 256, 384, 512):
             for L in (1, 2):
                 M = nqs.made_create(wl.make_made_params(n, h, 1, n_hidden_layers=L))
                 assert M.resolved_path(nqs.PATH_TC) == nqs.PATH_TC, (n, h, L)
                 assert M.resolved_path(nqs.PATH_AUTO) == (nqs.PATH_TC if h >= 384 else nqs.PATH_SIMT)
+    for n in (127, 128):
+        M = nqs.made_create(wl.make_made_params(n, 512, 1))
+        with pytest.raises(nqs.NqsError) as ei:
+            M.resolved_path(nqs.PATH_TC)
+        assert ei.value.status == -6
+        assert M.resolved_path(nqs.PATH_AUTO) == nqs.PATH_SIMT
     for n, h in ((20, 64), (20, 192), (20, 640), (20, 32)):
         M = nqs.made_create(wl.make_made_params(n, h, 1))
         with pytest.raises(nqs.NqsError) as ei:

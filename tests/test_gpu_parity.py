@@ -66,7 +66,9 @@ def _paths(M, min_hidden_tc=384):
                                          (76, 512, 2, "reverse"), (13, 48, 1, "random"), (128, 64, 2, "random"),
                                          (65, 16, 2, "reverse"), (3, 8, 1, "identity"),
                                          # tensor-core shape limits: one hidden layer (the paper's own architecture,
-                                         # PAPER.md:84), n = 3 / 77 (two accumulators) / 96 / 112 / 128, odd chunk counts
+                                         # PAPER.md:84), n = 3 / 77 (two accumulators) / 96 / 112 / 126 (the largest n
+                                         # the tensor-core path takes; 127 and 128 run on the fp32 path), odd chunk counts
+                                         (126, 512, 2, "random"), (125, 384, 1, "reverse"), (127, 256, 2, "reverse"),
                                          (30, 128, 1, "identity"), (52, 512, 1, "reverse"), (76, 384, 1, "random"),
                                          (3, 128, 2, "identity"), (77, 512, 2, "reverse"), (96, 512, 2, "random"),
                                          (112, 512, 2, "reverse"), (128, 512, 2, "random"), (128, 384, 1, "reverse")])
