@@ -119,9 +119,10 @@ def time_oracle(w, ham, params, samples, n_samples, one_thread=False):
     return n_samples * len(c) / dt, dt, threads
 
 
-# DRAM bytes (read + write) of ONE full-size eloc_tc_kernel launch (cfg 5, 8,192 samples x all groups), from the
-# `ncu --set full` capture summarised in profiles/r2_final_summary.md.  A constant of that capture, not measured live.
-NCU_DRAM_BYTES_PER_LAUNCH = {5: None}
+# DRAM bytes (read + write) of ONE eloc_tc_kernel launch from the `ncu --set full` capture summarised in
+# profiles/r2_final_summary.md, keyed by (cfg, samples per launch).  A constant of that capture, not measured live: the
+# full-size launch (8,192 samples, 2.4 s x ~45 replay passes) did not finish under ncu, the 2,048-sample launch did.
+NCU_DRAM_BYTES_PER_LAUNCH = {(5, 2048): 345632000 + 7343616}
 
 
 def time_contraction(nqs, torch, H, xs, stream, clocks_mhz):
@@ -307,7 +308,11 @@ def main():
                  "algorithmic_flops_per_eval": flops_eval, "evals_per_launch": evals_per_launch,
                  "kernel_share_of_step": chain_ms / total_ms})
 
-    roof["traffic"] = NCU_DRAM_BYTES_PER_LAUNCH.get(args.cfg) if (used_tc and not args.mb_samples) else None
+    roof["traffic"] = NCU_DRAM_BYTES_PER_LAUNCH.get((args.cfg, mb)) if used_tc else None
+    if used_tc and roof["traffic"] is None and (args.cfg, 2048) in NCU_DRAM_BYTES_PER_LAUNCH:
+        roof["traffic_reduced_launch"] = {"bytes": NCU_DRAM_BYTES_PER_LAUNCH[(args.cfg, 2048)], "samples": 2048,
+                                          "note": "ncu capture of a 2,048-sample launch (the full-size launch does not finish "
+                                                  "under ncu); algorithmic bytes = the term tensors once, 79 MB"}
     if used_tc:
         issued, dense = M.tc_flops()
         roof["issued_flops_per_eval"] = issued                # what the kernel sends to the tensor cores (overhead included)
