@@ -173,7 +173,7 @@ extern "C" void nqs_made_free(nqs_made_t *M) {
 static int resolve_path(const nqs_made *M, int path, int *use_tc) {
     if (path == NQS_PATH_SIMT) { *use_tc = 0; return NQS_OK; }
     if (path == NQS_PATH_TC) { if (!tc_supported(M)) return NQS_EUNSUPPORTED; *use_tc = 1; return NQS_OK; }
-    if (path == NQS_PATH_AUTO) { *use_tc = (tc_supported(M) && M->h >= 384) ? 1 : 0; return NQS_OK; }
+    if (path == NQS_PATH_AUTO) { *use_tc = tc_supported(M) ? 1 : 0; return NQS_OK; }
     return NQS_EINVAL;
 }
 

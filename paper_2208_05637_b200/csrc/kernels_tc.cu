@@ -55,19 +55,21 @@ enum { BAR_A0FULL = 0, BAR_A0FREE = 1, BAR_A1FREE = 2, BAR_D3FULL = 3, BAR_D3EMP
        BAR_WFULL = 11, BAR_WEMPTY = 11 + MAX_SLOTS, BAR_COUNT = 11 + 2 * MAX_SLOTS };
 
 // Streamed weight sub-tiles: one 32-bit word each, in consumption order (kernel parameter space -> uniform loads).
-constexpr int MAX_SUB = 2 * MAX_NC + MAX_NC * (1 + 2 * MAX_NC) + MAX_NC;   // W1 + P1 + (b2 rows + W2 blocks) + W3
+constexpr int MAX_SUB = 2 * MAX_NC + MAX_NC * (1 + 2 * MAX_NC) + MAX_NC;   // W1 + P1 + (b2 rows + W2 blocks) + W3 (split mode, NC <= 2: fewer)
 constexpr uint32_t SUB_OFF_MASK = 0x1FFFu;                   // [0:13)  byte offset inside the slot / 16
 constexpr uint32_t SUB_NEW = 1u << 13;                       // first sub-tile of a ring fill: wait for the fill
 constexpr uint32_t SUB_END = 1u << 14;                       // last sub-tile of a ring fill: release the slot
+constexpr uint32_t SUB_ACC = 1u << 15;                       // input sub-tile: accumulate onto the accumulator (the lo-part pass)
 constexpr int SUB_AUX_SHIFT = 16;                            // [16:24) input: K-steps; W2: k-block | K-step mask << 4; W3: n_lo / 16
 
 struct SmemLayout { uint32_t a1, res, bias, bars, slots, total; };
 
-__host__ __device__ inline SmemLayout smem_layout(int H, int KO, int L, uint32_t slot_bytes, int nslots) {
+__host__ __device__ inline SmemLayout smem_layout(int H, int KO, int L, uint32_t slot_bytes, int nslots, int split) {
     SmemLayout S;
     uint32_t off = 0;
-    S.a1 = off; if (L == 2) off += (uint32_t)(H / 64) * 16384u;      // fp16 layer-1 activations, [H/64] K-blocks of 128 rows x 128 B
-    S.res = off; off += (uint32_t)(H / 64) * 1024u;                  // resident P2 tiles: 8 rows x 64 K per K-block (this CTA's half)
+    const uint32_t parts = split ? 2u : 1u;                          // split precision: hi and lo fp16 parts of everything
+    S.a1 = off; if (L == 2) off += parts * (uint32_t)(H / 64) * 16384u;   // fp16 layer-1 activations, K-blocks of 128 rows x 128 B (hi blocks, then lo)
+    S.res = off; off += parts * (uint32_t)(H / 64) * 1024u;          // resident P2 tiles: 8 rows x 64 K per K-block (this CTA's half)
     S.bias = off; off += (uint32_t)(KO + 4) * 4;                 // b3 | c2 (hidden-layer biases ride in the weight images)
     off = (off + 15) & ~15u;
     S.bars = off; off += BAR_COUNT * 8;
@@ -78,7 +80,7 @@ __host__ __device__ inline SmemLayout smem_layout(int H, int KO, int L, uint32_t
 }
 
 struct TcParams {
-    int n, H, NC, KI, KO, L, nacc, nops;
+    int n, H, NC, KI, KO, L, nacc, nops, split;
     int last_a0_op, last_l2_op;
     uint32_t tm_d3, tm_a0;               // TMEM columns: accumulator a at a * CN, D3 at tm_d3, A0 at tm_a0
     const uint8_t *wimg; uint32_t img_stride;     // streamed weight image of cluster rank r at wimg + r * img_stride
@@ -159,12 +161,12 @@ struct Sched {
     }
 };
 
-template <int NC, int L, int NACC>
+template <int NC, int L, int NACC, bool SPLIT>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_constant__ TcParams p) {
     using S = Sched<NC, L, NACC>;
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t s_tmem_base;
-    const SmemLayout SL = smem_layout(p.H, p.KO, p.L, p.slot_bytes, p.nslots);
+    const SmemLayout SL = smem_layout(p.H, p.KO, p.L, p.slot_bytes, p.nslots, SPLIT ? 1 : 0);
     uint64_t *bars = reinterpret_cast<uint64_t *>(smem + SL.bars);
     float *s_bias = reinterpret_cast<float *>(smem + SL.bias);
     const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
@@ -286,11 +288,19 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                     PROF_SITE(2); WAIT(BAR_EDONE + jc % NACC);
                     if (jc == S::FIRST_INPLACE) { PROF_SITE(3); WAIT(BAR_D3EMPTY); }              // first write into D3 of this tile
                     const uint32_t a_t = tmem + (uint32_t)(jc % NACC) * CN;
+                    // split precision: the epilogue left fp16 hi parts in columns [32 pc, 32 pc + 16) and lo parts in
+                    // [32 pc + 16, 32 pc + 32) of every 32-column piece; D3 += Ahi.Bhi + Alo.Bhi + Ahi.Blo
                     if (type == T_P) {                                          // resident P2 tile of this chunk, N = 16
-                        const uint32_t b_lo = (res_lo + (uint32_t)S::chunk(jc) * (2048u >> 4)) | lo_sw128;
+                        const uint32_t b_lo = (res_lo + (uint32_t)S::chunk(jc) * ((SPLIT ? 4096u : 2048u) >> 4)) | lo_sw128;
 #pragma unroll
-                        for (uint32_t ks = 0; ks < 8; ++ks)
-                            mma_ts_cg2(tm_ph, a_t + 32 * (ks >> 1) + 8 * (ks & 1), b_lo + (ks >> 2) * (1024u >> 4) + 2 * (ks & 3), hi_sw128, id16, 1u);
+                        for (uint32_t ks = 0; ks < 8; ++ks) {
+                            const uint32_t a_k = a_t + 32 * (ks >> 1) + 8 * (ks & 1), b_k = b_lo + (ks >> 2) * (1024u >> 4) + 2 * (ks & 3);
+                            mma_ts_cg2(tm_ph, a_k, b_k, hi_sw128, id16, 1u);
+                            if (SPLIT) {
+                                mma_ts_cg2(tm_ph, a_k + 16, b_k, hi_sw128, id16, 1u);
+                                mma_ts_cg2(tm_ph, a_k, b_k + (2048u >> 4), hi_sw128, id16, 1u);
+                            }
+                        }
                     } else {                                                    // streamed layer-3 tile
                         const uint32_t wn = p.sub[++si];
                         SLOT_ACQUIRE(w);
@@ -298,8 +308,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                         const uint32_t N = (uint32_t)KO - nlo, kb_step = (N >> 1) * (128u >> 4);
                         const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_sw128, idesc = id0 | ((N >> 3) << 17);
 #pragma unroll
-                        for (uint32_t ks = 0; ks < 8; ++ks)
-                            mma_ts_cg2(tm_d3 + nlo, a_t + 32 * (ks >> 1) + 8 * (ks & 1), b_lo + (ks >> 2) * kb_step + 2 * (ks & 3), hi_sw128, idesc, 1u);
+                        for (uint32_t ks = 0; ks < 8; ++ks) {
+                            const uint32_t a_k = a_t + 32 * (ks >> 1) + 8 * (ks & 1), b_k = b_lo + (ks >> 2) * kb_step + 2 * (ks & 3);
+                            mma_ts_cg2(tm_d3 + nlo, a_k, b_k, hi_sw128, idesc, 1u);
+                            if (SPLIT) {
+                                mma_ts_cg2(tm_d3 + nlo, a_k + 16, b_k, hi_sw128, idesc, 1u);
+                                mma_ts_cg2(tm_d3 + nlo, a_k, b_k + 2 * kb_step, hi_sw128, idesc, 1u);      // lo-part tile: N * 128 bytes on
+                            }
+                        }
                         SLOT_RELEASE(w);
                         w = wn;
                     }
@@ -347,19 +363,23 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                             w = wn;
                         }
                     } else {
-                        // input layers (layer 1 / phase hidden): A = A0 in TMEM, B = this chunk's rows, K-step prefix
-                        const uint32_t wn = p.sub[++si];
-                        SLOT_ACQUIRE(w);
-                        const uint32_t nk = (w >> SUB_AUX_SHIFT) & 0xFFu;
-                        const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_noswz;
-                        mma_ts_cg2(d, tm_a0, b_lo, hi_noswz, id128, 0u);
-                        // nested so that the common exit is one taken branch (KI <= 128 -> at most 8 K-steps)
+                        // input layers (layer 1 / phase hidden): A = A0 in TMEM (exact +-1), B = this chunk's rows, K-step
+                        // prefix; split precision: a second pass over the same A with the lo parts of the weights
+#pragma unroll
+                        for (int part = 0; part < (SPLIT ? 2 : 1); ++part) {
+                            const uint32_t wn = p.sub[++si];
+                            SLOT_ACQUIRE(w);
+                            const uint32_t nk = (w >> SUB_AUX_SHIFT) & 0xFFu;
+                            const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_noswz;
+                            mma_ts_cg2(d, tm_a0, b_lo, hi_noswz, id128, (uint32_t)part);
+                            // nested so that the common exit is one taken branch (KI <= 128 -> at most 8 K-steps)
 #define KSTEP(k) mma_ts_cg2(d, tm_a0 + 8u * (k), b_lo + 16u * (k), hi_noswz, id128, 1u)
-                        if (nk > 1) { KSTEP(1); if (nk > 2) { KSTEP(2); if (nk > 3) { KSTEP(3); if (nk > 4) { KSTEP(4);
-                        if (nk > 5) { KSTEP(5); if (nk > 6) { KSTEP(6); if (nk > 7) { KSTEP(7); } } } } } } }
+                            if (nk > 1) { KSTEP(1); if (nk > 2) { KSTEP(2); if (nk > 3) { KSTEP(3); if (nk > 4) { KSTEP(4);
+                            if (nk > 5) { KSTEP(5); if (nk > 6) { KSTEP(6); if (nk > 7) { KSTEP(7); } } } } } } }
 #undef KSTEP
-                        SLOT_RELEASE(w);
-                        w = wn;
+                            SLOT_RELEASE(w);
+                            w = wn;
+                        }
                     }
                     mma_commit_cg2(BAR_ADDR(BAR_FULL + acc));
                     if (L == 1 && j == S::LAST_A0) mma_commit_cg2(BAR_ADDR(BAR_A0FREE));       // A0 may be rebuilt for the next tile
@@ -416,9 +436,16 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
 #pragma unroll
             for (int pp = 0; pp < 2; ++pp) {
                 const uint32_t *v = pp ? vb : va;
-                uint32_t w[16];                                // the bias is already in the accumulator (constant input columns)
+                uint32_t w[16], wl[16];                        // the bias is already in the accumulator (constant input columns)
 #pragma unroll
-                for (int j2 = 0; j2 < 16; ++j2) w[j2] = cvt_relu_f16x2(__uint_as_float(v[2 * j2]), __uint_as_float(v[2 * j2 + 1]));
+                for (int j2 = 0; j2 < 16; ++j2) {
+                    const float x0 = __uint_as_float(v[2 * j2]), x1 = __uint_as_float(v[2 * j2 + 1]);
+                    w[j2] = cvt_relu_f16x2(x0, x1);
+                    if (SPLIT) {                               // lo part: what the fp16 rounding of relu(x) lost, again as fp16
+                        const float2 hf = __half22float2(*reinterpret_cast<const __half2 *>(&w[j2]));
+                        wl[j2] = cvt_f16x2(fmaxf(x0, 0.0f) - hf.x, fmaxf(x1, 0.0f) - hf.y);
+                    }
+                }
                 if (type == T_L1S) {
                     // this group's 64 hidden units are K-block 2c + grp of A1; 32 units = four 16-byte pieces, 128B swizzle
                     const uint32_t kb_addr = a1_row + (2 * c + grp) * 16384u;
@@ -426,9 +453,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                     for (uint32_t i = 0; i < 4; ++i) {
                         const uint32_t jj = (uint32_t)pp * 4 + i;
                         st_shared_v4(kb_addr + ((jj ^ sw) << 4), w[4 * i], w[4 * i + 1], w[4 * i + 2], w[4 * i + 3]);
+                        if (SPLIT) st_shared_v4(kb_addr + (uint32_t)(p.H / 64) * 16384u + ((jj ^ sw) << 4), wl[4 * i], wl[4 * i + 1], wl[4 * i + 2], wl[4 * i + 3]);
                     }
                 } else {
                     tmem_st16p(d_addr + 32 * pp, w);          // in place, inside the piece's own columns
+                    if (SPLIT) tmem_st16p(d_addr + 32 * pp + 16, wl);
                 }
             }
 #ifdef TC_PROF
@@ -678,7 +707,7 @@ __global__ void diag_init_kernel(HamDev hm, const ulonglong2 *__restrict__ x, lo
 
 // ------------------------------------------------------------------------------------------------------------
 struct TcPack {
-    int KI = 0, KO = 0, NC = 0, nacc = 0, nops = 0, nsub = 0, nfills = 0, nslots = 0, last_a0_op = -1, last_l2_op = -1;
+    int KI = 0, KO = 0, NC = 0, nacc = 0, nops = 0, nsub = 0, nfills = 0, nslots = 0, last_a0_op = -1, last_l2_op = -1, split = 0;
     uint32_t slot_bytes = 0, res_bytes = 0, img_stride = 0, tm_d3 = 0, tm_a0 = 0;
     void *d_wimg = nullptr, *d_fills = nullptr, *d_res = nullptr, *d_bias = nullptr;
     void *d_fpos = nullptr; size_t fpos_cap = 0;
@@ -693,12 +722,15 @@ struct TcPack {
 
 static inline int round16(int v) { return (v + 15) / 16 * 16; }
 
-struct TcShape { int KI, KO, NC, nacc, nslots; uint32_t slot; };
+struct TcShape { int KI, KO, NC, nacc, nslots, split; uint32_t slot; };
 
 static bool tc_shape(const nqs_made *M, TcShape *out) {
     if ((M->L != 1 && M->L != 2) || M->h % CN != 0 || M->h < CN || M->h > CN * MAX_NC) return false;
     TcShape s;
     s.KI = round16(M->n + 2); s.KO = round16(M->n + 4); s.NC = M->h / CN;      // + 2: the constant bias columns
+    // Split precision (every fp16 operand as hi + lo, three MMA passes: hi.hi + lo.hi + hi.lo) where single-pass fp16 misses
+    // the 1e-5 sum|c| bound (hidden < 384); the hi/lo activations need twice the A1 width, <= 512
+    s.split = (M->h <= 256) ? 1 : 0;
     if (s.KI > 128 || s.KO > 144) return false;
     // TMEM: nacc accumulators of CN columns, D3 (KO), A0 (KI/2)
     s.nacc = 3;
@@ -706,9 +738,9 @@ static bool tc_shape(const nqs_made *M, TcShape *out) {
     if (s.nacc * CN + s.KO + s.KI / 2 > 512) return false;
     uint32_t need = (uint32_t)HALF * s.KI * 2;                                 // input sub-tile (64 rows x KI)
     if ((uint32_t)HALF * 128 > need) need = HALF * 128;                        // layer-2 sub-tile (64 x 64)
-    if ((uint32_t)s.KO * 128 > need) need = (uint32_t)s.KO * 128;              // layer-3 tile (KO/2 rows x 128 K)
+    if ((uint32_t)s.KO * 128 * (1 + s.split) > need) need = (uint32_t)s.KO * 128 * (1 + s.split);   // layer-3 tile (KO/2 rows x 128 K; hi + lo)
     const uint32_t budget = 227 * 1024 - 1024;
-    const uint32_t fixed = smem_layout(M->h, s.KO, M->L, 0, 0).total;
+    const uint32_t fixed = smem_layout(M->h, s.KO, M->L, 0, 0, s.split).total;
     if (fixed + 2 * need > budget) return false;
     const uint32_t ring = budget - fixed;
     // Two large slots (plain double buffering).  Measured: a bulk copy costs its issuing warp ~590 cycles whatever its size
@@ -743,9 +775,10 @@ int tc_pack_upload(const nqs_made *M) {
     TcPack *P = new (std::nothrow) TcPack();
     if (!P) return NQS_ENOMEM;
     const int n = M->n, H = M->h, NC = sh.NC, KI = sh.KI, KO = sh.KO, L = M->L;
-    P->KI = KI; P->KO = KO; P->NC = NC; P->nacc = sh.nacc; P->slot_bytes = sh.slot; P->nslots = sh.nslots;
+    P->KI = KI; P->KO = KO; P->NC = NC; P->nacc = sh.nacc; P->slot_bytes = sh.slot; P->nslots = sh.nslots; P->split = sh.split;
+    const int SP = sh.split;
     P->tm_d3 = (uint32_t)sh.nacc * CN; P->tm_a0 = P->tm_d3 + (uint32_t)KO;
-    P->L = smem_layout(H, KO, L, sh.slot, sh.nslots);
+    P->L = smem_layout(H, KO, L, sh.slot, sh.nslots, sh.split);
     const uint32_t slot = sh.slot;
     const uint32_t in_bytes = (uint32_t)HALF * KI * 2, w2_bytes = HALF * 128;
     const std::vector<float> &W1 = M->wm[0], &W3 = M->wm[L];
@@ -771,10 +804,12 @@ int tc_pack_upload(const nqs_made *M) {
     P->nops = nops;
 
     std::vector<uint8_t> img[2], res[2];
-    res[0].assign((size_t)(H / 64) * 1024, 0); res[1] = res[0];
+    res[0].assign((size_t)(1 + SP) * (H / 64) * 1024, 0); res[1] = res[0];
     std::vector<uint2> fills;
     std::vector<uint32_t> sub;
     auto put = [](std::vector<uint8_t> &buf, size_t off, float v) { __half hv = __float2half_rn(v); memcpy(&buf[off], &hv, 2); };
+    // part 0: the fp16 rounding of v (all there is in single-pass mode); part 1: the fp16 rounding of what part 0 lost
+    auto part_of = [](float v, int part) { const float hi = __half2float(__float2half_rn(v)); return part == 0 ? hi : v - hi; };
 
     // ---- streamed sub-tiles are appended to the open ring fill (<= slot bytes, in consumption order) ----
     uint32_t fill_start = 0, fill_bytes = 0;
@@ -799,33 +834,38 @@ int tc_pack_upload(const nqs_made *M) {
     // input-layer chunk c (layer 1 or phase hidden): rank r holds units 128 c + 64 r .. + 63.  Masked layer-1 columns
     // are the high ones for sorted degrees; in general the issued K-steps are the prefix up to the last non-zero one.
     auto input_chunk = [&](int c, bool phase) {
-        const uint32_t base = stream_alloc(in_bytes, 0);
-        int nk = 1;                                             // the accumulator must be overwritten even if all zero
-        for (int r = 0; r < 2; ++r)
-            for (int rr = 0; rr < HALF; ++rr) {
-                const int j = c * CN + r * HALF + rr;
-                const float bj = phase ? M->c1[j] : M->bias[0][j];
-                const float bj_hi = __half2float(__float2half_rn(bj));
-                for (int k = 0; k < KI; ++k) {
-                    float v = 0.f;                              // K index 0, 1: bias (hi, lo) against the constant +1 inputs
-                    const int d = k - 2;
-                    if (k == 0) v = bj_hi;
-                    else if (k == 1) v = bj - bj_hi;
-                    else if (phase) { if (d < n - 2) v = M->p1[(size_t)j * (n - 2) + d]; }
-                    else if (d < n) v = W1[(size_t)j * n + d];
-                    put(img[r], base + noswz_offset(rr, k, KI), v);
-                    if (v != 0.0f && k / 16 + 1 > nk) nk = k / 16 + 1;
+        for (int part = 0; part <= SP; ++part) {
+            const uint32_t base = stream_alloc(in_bytes, 0);
+            int nk = 1;                                         // the accumulator must be overwritten even if all zero
+            for (int r = 0; r < 2; ++r)
+                for (int rr = 0; rr < HALF; ++rr) {
+                    const int j = c * CN + r * HALF + rr;
+                    const float bj = phase ? M->c1[j] : M->bias[0][j];
+                    const float bj_hi = __half2float(__float2half_rn(bj));
+                    for (int k = 0; k < KI; ++k) {
+                        float v = 0.f;                          // K index 0, 1: bias (hi, lo) against the constant +1 inputs
+                        const int d = k - 2;
+                        if (k == 0) v = part == 0 ? bj_hi : 0.f;
+                        else if (k == 1) v = part == 0 ? bj - bj_hi : 0.f;
+                        else if (phase) { if (d < n - 2) v = part_of(M->p1[(size_t)j * (n - 2) + d], part); }
+                        else if (d < n) v = part_of(W1[(size_t)j * n + d], part);
+                        put(img[r], base + noswz_offset(rr, k, KI), v);
+                        if (v != 0.0f && k / 16 + 1 > nk) nk = k / 16 + 1;
+                    }
                 }
-            }
-        sub.back() |= (uint32_t)nk << SUB_AUX_SHIFT;
-        P->mma_issued += (long long)nk * CN; P->mma_dense += (long long)(KI / 16) * CN;
+            sub.back() |= ((uint32_t)nk << SUB_AUX_SHIFT) | (part ? SUB_ACC : 0u);
+            P->mma_issued += (long long)nk * CN;
+        }
+        P->mma_dense += (long long)(KI / 16) * CN;
     };
     // resident P2 tile of phase chunk c: rows 12..15 of the 16-row tile hold the 4 phase outputs -> rank 1, rows 4..7
     auto phase_out_tile = [&](int c) {
-        for (int o = 0; o < 4; ++o)
-            for (int k = 0; k < CN; ++k)
-                put(res[1], (size_t)c * 2048 + (size_t)(k / 64) * 1024 + sw128_offset(4 + o, k % 64), M->p2[(size_t)o * H + c * CN + k]);
-        P->mma_issued += 8 * 16; P->mma_dense += 8 * 16;
+        for (int part = 0; part <= SP; ++part)
+            for (int o = 0; o < 4; ++o)
+                for (int k = 0; k < CN; ++k)
+                    put(res[1], (size_t)(c * (1 + SP) + part) * 2048 + (size_t)(k / 64) * 1024 + sw128_offset(4 + o, k % 64),
+                        part_of(M->p2[(size_t)o * H + c * CN + k], part));
+        P->mma_issued += (1 + 2 * SP) * 8 * 16; P->mma_dense += 8 * 16;
     };
     // layer-2 chunk c2: k-blocks of 64 with any non-zero weight, and inside a block only the non-zero K-steps
     auto l2_chunk = [&](int c2) {
@@ -849,14 +889,20 @@ int tc_pack_upload(const nqs_made *M) {
                     if (W2[(size_t)(c2 * CN + r) * H + kb * 64 + k] != 0.0f) kmask |= 1u << (k / 16);
             P->mma_dense += 4 * CN;
             if (!kmask) continue;                                        // exact: an all-zero block adds 0
-            const uint32_t base = stream_alloc(w2_bytes, (uint32_t)kb | (kmask << 4));
-            for (int r = 0; r < 2; ++r)
-                for (int rr = 0; rr < HALF; ++rr)
-                    for (int k = 0; k < 64; ++k)
-                        put(img[r], base + sw128_offset(rr, k), W2[(size_t)(c2 * CN + r * HALF + rr) * H + kb * 64 + k]);
-            P->mma_issued += (long long)__builtin_popcount(kmask) * CN;
+            // single pass: A1[kb] . W2^T.  Split: A1hi[kb] . W2hi^T + A1lo[kb] . W2hi^T + A1hi[kb] . W2lo^T — three
+            // streamed blocks (A k-block, weight part); the lo activations live H/64 k-blocks after the hi ones
+            const int npass = SP ? 3 : 1;
+            for (int ps = 0; ps < npass; ++ps) {
+                const int a_kb = kb + (ps == 1 ? H / 64 : 0), wpart = ps == 2 ? 1 : 0;
+                const uint32_t base = stream_alloc(w2_bytes, (uint32_t)a_kb | (kmask << 4));
+                for (int r = 0; r < 2; ++r)
+                    for (int rr = 0; rr < HALF; ++rr)
+                        for (int k = 0; k < 64; ++k)
+                            put(img[r], base + sw128_offset(rr, k), part_of(W2[(size_t)(c2 * CN + r * HALF + rr) * H + kb * 64 + k], wpart));
+                P->mma_issued += (long long)__builtin_popcount(kmask) * CN;
+                ++nb;
+            }
             need = kb / 2;
-            ++nb;
         }
         P->nblk[c2] = (uint8_t)nb; P->l2need[c2] = (uint8_t)need;
     };
@@ -869,15 +915,18 @@ int tc_pack_upload(const nqs_made *M) {
                 if (W3[(size_t)d * H + c * CN + k] != 0.0f && d < row_lo) row_lo = d;
         const int n_lo = row_lo >= KO ? KO - 16 : (row_lo / 16) * 16;
         const int N = KO - n_lo, Nh = N / 2;
-        const uint32_t base = stream_alloc((uint32_t)2 * Nh * 128, (uint32_t)(n_lo / 16));
-        for (int r = 0; r < 2; ++r)
-            for (int rr = 0; rr < Nh; ++rr) {
-                const int d = n_lo + r * Nh + rr;
-                if (d >= n) continue;
-                for (int k = 0; k < CN; ++k)
-                    put(img[r], base + (size_t)(k / 64) * Nh * 128 + sw128_offset(rr, k % 64), W3[(size_t)d * H + c * CN + k]);
-            }
-        P->mma_issued += (long long)8 * N; P->mma_dense += (long long)8 * KO;
+        const uint32_t tile_bytes = (uint32_t)2 * Nh * 128;                   // split: the lo-part tile follows the hi-part tile
+        const uint32_t base = stream_alloc(tile_bytes * (1 + SP), (uint32_t)(n_lo / 16));
+        for (int part = 0; part <= SP; ++part)
+            for (int r = 0; r < 2; ++r)
+                for (int rr = 0; rr < Nh; ++rr) {
+                    const int d = n_lo + r * Nh + rr;
+                    if (d >= n) continue;
+                    for (int k = 0; k < CN; ++k)
+                        put(img[r], base + part * tile_bytes + (size_t)(k / 64) * Nh * 128 + sw128_offset(rr, k % 64),
+                            part_of(W3[(size_t)d * H + c * CN + k], part));
+                }
+        P->mma_issued += (long long)(1 + 2 * SP) * 8 * N; P->mma_dense += (long long)8 * KO;
     };
     auto emit_op = [&](int j) {
         const int c = P->opchunk[j];
@@ -973,7 +1022,7 @@ void tc_mma_counts(const nqs_made *M, long long *issued, long long *dense) {
 
 static void fill_common(const nqs_made *M, TcParams &p) {
     const TcPack *P = M->tc;
-    p.n = M->n; p.H = M->h; p.NC = P->NC; p.KI = P->KI; p.KO = P->KO; p.L = M->L; p.nacc = P->nacc; p.nops = P->nops;
+    p.n = M->n; p.H = M->h; p.NC = P->NC; p.KI = P->KI; p.KO = P->KO; p.L = M->L; p.nacc = P->nacc; p.nops = P->nops; p.split = P->split;
     p.last_a0_op = P->last_a0_op; p.last_l2_op = P->last_l2_op;
     p.tm_d3 = P->tm_d3; p.tm_a0 = P->tm_a0;
     p.wimg = (const uint8_t *)P->d_wimg; p.img_stride = P->img_stride;
@@ -1011,18 +1060,18 @@ long long *g_tc_prof = nullptr;   // [148][16], set by the profiling harness thr
 extern "C" void nqs_tc_prof_buffer(long long *dev_buf) { g_tc_prof = dev_buf; }
 #endif
 
-template <int NC, int L, int NACC>
+template <int NC, int L, int NACC, bool SPLIT>
 static int launch_inst(const TcParams &p, int grid, uint32_t smem_bytes, cudaStream_t st) {
     using S = Sched<NC, L, NACC>;
     if (p.nops != S::NOPS) return NQS_EUNSUPPORTED;
     for (int j = 0; j < S::NOPS; ++j)                        // the host-packed op list must be the compiled schedule
         if (p.optype[j] != S::type(j) || p.opchunk[j] != S::chunk(j)) return NQS_EUNSUPPORTED;
     // the attribute is per device and per kernel; setting it is a cheap host call, so no process-wide cache
-    if (cudaFuncSetAttribute(eloc_tc_kernel<NC, L, NACC>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes) != cudaSuccess) {
+    if (cudaFuncSetAttribute(eloc_tc_kernel<NC, L, NACC, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes) != cudaSuccess) {
         cudaGetLastError();
         return NQS_ECUDA;
     }
-    eloc_tc_kernel<NC, L, NACC><<<grid, NTHREADS, smem_bytes, st>>>(p);
+    eloc_tc_kernel<NC, L, NACC, SPLIT><<<grid, NTHREADS, smem_bytes, st>>>(p);
     return NQS_OK;
 }
 
@@ -1035,12 +1084,14 @@ static int launch_chain(const TcPack *P, TcParams &p, long long ntiles, cudaStre
     const long long ncl_max = P->sms / 2;
     const int grid = 2 * (int)(npairs < ncl_max ? npairs : ncl_max);
     int rc = NQS_EUNSUPPORTED;
-#define TC_CASE(NC_, L_, NA_) case (NC_ * 16 + L_ * 4 + NA_): rc = launch_inst<NC_, L_, NA_>(p, grid, P->L.total, st); break;
+    // hidden <= 256 runs in split precision (tc_shape), wider nets in a single fp16 pass
+#define TC_CASE(NC_, L_, NA_, SP_) case (NC_ * 16 + L_ * 4 + NA_): rc = launch_inst<NC_, L_, NA_, SP_>(p, grid, P->L.total, st); break;
+    if ((p.split != 0) != (p.NC <= 2)) return NQS_EUNSUPPORTED;
     switch (p.NC * 16 + p.L * 4 + p.nacc) {
-        TC_CASE(1, 1, 2) TC_CASE(2, 1, 2) TC_CASE(3, 1, 2) TC_CASE(4, 1, 2)
-        TC_CASE(1, 2, 2) TC_CASE(2, 2, 2) TC_CASE(3, 2, 2) TC_CASE(4, 2, 2)
-        TC_CASE(1, 1, 3) TC_CASE(2, 1, 3) TC_CASE(3, 1, 3) TC_CASE(4, 1, 3)
-        TC_CASE(1, 2, 3) TC_CASE(2, 2, 3) TC_CASE(3, 2, 3) TC_CASE(4, 2, 3)
+        TC_CASE(1, 1, 2, true) TC_CASE(2, 1, 2, true) TC_CASE(3, 1, 2, false) TC_CASE(4, 1, 2, false)
+        TC_CASE(1, 2, 2, true) TC_CASE(2, 2, 2, true) TC_CASE(3, 2, 2, false) TC_CASE(4, 2, 2, false)
+        TC_CASE(1, 1, 3, true) TC_CASE(2, 1, 3, true) TC_CASE(3, 1, 3, false) TC_CASE(4, 1, 3, false)
+        TC_CASE(1, 2, 3, true) TC_CASE(2, 2, 3, true) TC_CASE(3, 2, 3, false) TC_CASE(4, 2, 3, false)
         default: break;
     }
 #undef TC_CASE

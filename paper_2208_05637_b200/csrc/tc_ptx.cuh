@@ -163,6 +163,13 @@ __device__ __forceinline__ uint32_t cvt_relu_f16x2(float lo, float hi) {
     return r;
 }
 
+// round-to-nearest fp16 pack without the ReLU (the lo parts of split-precision operands may be negative)
+__device__ __forceinline__ uint32_t cvt_f16x2(float lo, float hi) {
+    uint32_t r;
+    asm("cvt.rn.f16x2.f32 %0, %1, %2;\n" : "=r"(r) : "f"(hi), "f"(lo));
+    return r;
+}
+
 // MUFU approximations with flush-to-zero (no denormal fix-up code around them)
 __device__ __forceinline__ float ex2_ftz(float x) { float y; asm("ex2.approx.ftz.f32 %0, %1;\n" : "=f"(y) : "f"(x)); return y; }
 __device__ __forceinline__ float lg2_ftz(float x) { float y; asm("lg2.approx.ftz.f32 %0, %1;\n" : "=f"(y) : "f"(x)); return y; }

@@ -142,7 +142,7 @@ def test_tensor_core_path_shape_limits():
             for L in (1, 2):
                 M = nqs.made_create(wl.make_made_params(n, h, 1, n_hidden_layers=L))
                 assert M.resolved_path(nqs.PATH_TC) == nqs.PATH_TC, (n, h, L)
-                assert M.resolved_path(nqs.PATH_AUTO) == (nqs.PATH_TC if h >= 384 else nqs.PATH_SIMT)
+                assert M.resolved_path(nqs.PATH_AUTO) == nqs.PATH_TC
     for n in (127, 128):
         M = nqs.made_create(wl.make_made_params(n, 512, 1))
         with pytest.raises(nqs.NqsError) as ei:
