@@ -49,7 +49,7 @@ enum nqs_status {
 };
 
 /* Which kernels evaluate the MADE chain.  Both are CUDA; neither touches the CPU.
- *  NQS_PATH_SIMT : fp32 FFMA on CUDA cores, every layer (reference-quality, any shape).
+ *  NQS_PATH_SIMT : fp32 FFMA on CUDA cores, every layer (any shape; the parity reference for the tensor-core path).
  *  NQS_PATH_TC   : tcgen05 tensor cores driven by CTA pairs (cta_group::2), fp16 operands / fp32 accumulation in
  *                  TMEM, fused gather of x xor f into the operand tile and log|psi| / phase / ratio / E_loc in the
  *                  epilogue.  Needs n_hidden_layers in {1, 2}, hidden a multiple of 128 in [128, 512] and
@@ -57,9 +57,11 @@ enum nqs_status {
  *                  so round16(n+2) <= 128 input columns; TMEM holds two 128-column accumulators + round16(n+4)
  *                  output columns + round16(n+2)/2 input columns <= 512 (three accumulators when n <= 76).  Other
  *                  shapes (n = 127, 128 included) return NQS_EUNSUPPORTED; NQS_PATH_AUTO then takes NQS_PATH_SIMT.
- *  NQS_PATH_AUTO : TC when the shape supports it and hidden >= 384 (where single-pass fp16 operands keep
- *                  |dE_loc| several times below 1e-5 sum|c| on the chemistry workloads),
- *                  else SIMT.
+ *                  Precision: hidden >= 384 runs one fp16 pass (|dE_loc| 0.1-0.2 x 1e-5 sum|c| on the chemistry
+ *                  workloads); hidden <= 256 runs in SPLIT precision — every fp16 operand as hi + lo parts, three MMA
+ *                  passes (hi.hi + lo.hi + hi.lo) — because a single fp16 pass misses the bound there (2 x); split
+ *                  results are as accurate as the fp32 path (0.03 x the bound) at 3 x the tensor work.
+ *  NQS_PATH_AUTO : TC when the shape supports it, else SIMT.
  * A handle (nqs_made_t / nqs_ham_t) owns device scratch that its compute calls reuse: use one handle from one
  * host thread and one CUDA stream at a time, on the device that was current when it was first used (other
  * devices: NQS_EINVAL). */
