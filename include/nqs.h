@@ -45,20 +45,21 @@ enum nqs_status {
     NQS_ENOMEM       = -3,   /* host or device allocation failed                                                 */
     NQS_ECUDA        = -4,   /* a CUDA runtime call or kernel launch failed (no device, ...)                      */
     NQS_EARCH        = -5,   /* device is not compute capability 10.x (the kernels are sm_100a only)             */
-    NQS_EUNSUPPORTED = -6    /* the requested path cannot run this shape (e.g. NQS_PATH_TC on hidden % 128 != 0)  */
+    NQS_EUNSUPPORTED = -6    /* the requested path cannot run this shape (e.g. NQS_PATH_TC on hidden > 512)       */
 };
 
 /* Which kernels evaluate the MADE chain.  Both are CUDA; neither touches the CPU.
  *  NQS_PATH_SIMT : fp32 FFMA on CUDA cores, every layer (any shape; the parity reference for the tensor-core path).
  *  NQS_PATH_TC   : tcgen05 tensor cores driven by CTA pairs (cta_group::2), fp16 operands / fp32 accumulation in
  *                  TMEM, fused gather of x xor f into the operand tile and log|psi| / phase / ratio / E_loc in the
- *                  epilogue.  Needs n_hidden_layers in {1, 2}, hidden a multiple of 128 in [128, 512] and
+ *                  epilogue.  Needs n_hidden_layers in {1, 2}, hidden in [1, 512] (padded inside the library to a
+ *                  multiple of 128 with zero-weight units: the padded network is the same function, exactly) and
  *                  n_qubits in [3, 126]: the operand tile carries two constant columns for the hidden-layer biases,
  *                  so round16(n+2) <= 128 input columns; TMEM holds two 128-column accumulators + round16(n+4)
  *                  output columns + round16(n+2)/2 input columns <= 512 (three accumulators when n <= 76).  Other
  *                  shapes (n = 127, 128 included) return NQS_EUNSUPPORTED; NQS_PATH_AUTO then takes NQS_PATH_SIMT.
- *                  Precision: hidden >= 384 runs one fp16 pass (|dE_loc| 0.1-0.2 x 1e-5 sum|c| on the chemistry
- *                  workloads); hidden <= 256 runs in SPLIT precision — every fp16 operand as hi + lo parts, three MMA
+ *                  Precision: hidden (padded) >= 384 runs one fp16 pass (|dE_loc| 0.1-0.2 x 1e-5 sum|c| on the chemistry
+ *                  workloads); hidden (padded) <= 256 runs in SPLIT precision — every fp16 operand as hi + lo parts, three MMA
  *                  passes (hi.hi + lo.hi + hi.lo) — because a single fp16 pass misses the bound there (2 x); split
  *                  results are as accurate as the fp32 path (0.03 x the bound) at 3 x the tensor work.
  *  NQS_PATH_AUTO : TC when the shape supports it, else SIMT.
@@ -184,7 +185,10 @@ int nqs_local_energy(const nqs_ham_t *ham, const nqs_made_t *made, const uint64_
 
 /* Same computation with HOST buffers: copies samples/counts host->device, runs nqs_local_energy on an
  * internal stream, copies eloc device->host and synchronises.  samples_host uint64 [B][2], counts_host
- * int64 [B] or NULL, eloc_out_host float [B][2], stats_out_host double [5] or NULL. */
+ * int64 [B] or NULL, eloc_out_host float [B][2], stats_out_host double [5] or NULL.  A sample with a bit >= n_qubits set,
+ * or a Hamiltonian and a model of different n_qubits: NQS_EINVAL (checked on the host before anything is launched; the
+ * device-pointer entry points take "bits >= n_qubits are zero" as a precondition — checking it there would force a
+ * synchronisation). */
 int nqs_local_energy_host(const nqs_ham_t *ham, const nqs_made_t *made, const uint64_t *samples_host,
                           const int64_t *counts_host, int64_t B, int64_t minibatch, int path,
                           float *eloc_out_host, double *stats_out_host);

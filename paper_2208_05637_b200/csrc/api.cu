@@ -298,6 +298,13 @@ extern "C" int nqs_local_energy_host(const nqs_ham_t *H, const nqs_made_t *M, co
     if (!H || !M || B < 0) return NQS_EINVAL;
     if (B == 0) return nqs_local_energy(H, M, nullptr, nullptr, 0, minibatch, path, nullptr, stats_out_host, nullptr);
     if (!samples_host || !eloc_out_host) return NQS_EINVAL;
+    {   // bits >= n_qubits must be zero (include/nqs.h): checked here, where the samples are host memory
+        const int n = M->n;
+        const uint64_t lo_bad = n >= 64 ? 0ull : ~0ull << n, hi_bad = n >= 128 ? 0ull : (n <= 64 ? ~0ull : ~0ull << (n - 64));
+        for (int64_t i = 0; i < B; ++i)
+            if ((samples_host[2 * i] & lo_bad) | (samples_host[2 * i + 1] & hi_bad)) return NQS_EINVAL;
+        if (H->n != n) return NQS_EINVAL;
+    }
     int rc = nqs_check_device();
     if (rc) return rc;
     void *d_x = nullptr, *d_c = nullptr, *d_e = nullptr;

@@ -707,7 +707,7 @@ __global__ void diag_init_kernel(HamDev hm, const ulonglong2 *__restrict__ x, lo
 
 // ------------------------------------------------------------------------------------------------------------
 struct TcPack {
-    int KI = 0, KO = 0, NC = 0, nacc = 0, nops = 0, nsub = 0, nfills = 0, nslots = 0, last_a0_op = -1, last_l2_op = -1, split = 0;
+    int KI = 0, KO = 0, NC = 0, nacc = 0, nops = 0, nsub = 0, nfills = 0, nslots = 0, last_a0_op = -1, last_l2_op = -1, split = 0, Hp = 0;
     uint32_t slot_bytes = 0, res_bytes = 0, img_stride = 0, tm_d3 = 0, tm_a0 = 0;
     void *d_wimg = nullptr, *d_fills = nullptr, *d_res = nullptr, *d_bias = nullptr;
     void *d_fpos = nullptr; size_t fpos_cap = 0;
@@ -722,15 +722,18 @@ struct TcPack {
 
 static inline int round16(int v) { return (v + 15) / 16 * 16; }
 
-struct TcShape { int KI, KO, NC, nacc, nslots, split; uint32_t slot; };
+struct TcShape { int KI, KO, NC, nacc, nslots, split, Hp; uint32_t slot; };
 
 static bool tc_shape(const nqs_made *M, TcShape *out) {
-    if ((M->L != 1 && M->L != 2) || M->h % CN != 0 || M->h < CN || M->h > CN * MAX_NC) return false;
+    if ((M->L != 1 && M->L != 2) || M->h < 1 || M->h > CN * MAX_NC) return false;
     TcShape s;
-    s.KI = round16(M->n + 2); s.KO = round16(M->n + 4); s.NC = M->h / CN;      // + 2: the constant bias columns
+    // the hidden width is padded to a multiple of 128 with units whose weights and biases are zero: relu(0) = 0 feeds
+    // zero weights, so the padded network computes exactly the same function
+    s.Hp = (M->h + CN - 1) / CN * CN;
+    s.KI = round16(M->n + 2); s.KO = round16(M->n + 4); s.NC = s.Hp / CN;      // + 2: the constant bias columns
     // Split precision (every fp16 operand as hi + lo, three MMA passes: hi.hi + lo.hi + hi.lo) where single-pass fp16 misses
     // the 1e-5 sum|c| bound (hidden < 384); the hi/lo activations need twice the A1 width, <= 512
-    s.split = (M->h <= 256) ? 1 : 0;
+    s.split = (s.Hp <= 256) ? 1 : 0;
     if (s.KI > 128 || s.KO > 144) return false;
     // TMEM: nacc accumulators of CN columns, D3 (KO), A0 (KI/2)
     s.nacc = 3;
@@ -740,7 +743,7 @@ static bool tc_shape(const nqs_made *M, TcShape *out) {
     if ((uint32_t)HALF * 128 > need) need = HALF * 128;                        // layer-2 sub-tile (64 x 64)
     if ((uint32_t)s.KO * 128 * (1 + s.split) > need) need = (uint32_t)s.KO * 128 * (1 + s.split);   // layer-3 tile (KO/2 rows x 128 K; hi + lo)
     const uint32_t budget = 227 * 1024 - 1024;
-    const uint32_t fixed = smem_layout(M->h, s.KO, M->L, 0, 0, s.split).total;
+    const uint32_t fixed = smem_layout(s.Hp, s.KO, M->L, 0, 0, s.split).total;
     if (fixed + 2 * need > budget) return false;
     const uint32_t ring = budget - fixed;
     // Two large slots (plain double buffering).  Measured: a bulk copy costs its issuing warp ~590 cycles whatever its size
@@ -774,14 +777,23 @@ int tc_pack_upload(const nqs_made *M) {
     if (!tc_shape(M, &sh)) return NQS_EUNSUPPORTED;
     TcPack *P = new (std::nothrow) TcPack();
     if (!P) return NQS_ENOMEM;
-    const int n = M->n, H = M->h, NC = sh.NC, KI = sh.KI, KO = sh.KO, L = M->L;
+    const int n = M->n, h = M->h, H = sh.Hp, NC = sh.NC, KI = sh.KI, KO = sh.KO, L = M->L;       // H: padded width
+    P->Hp = H;
     P->KI = KI; P->KO = KO; P->NC = NC; P->nacc = sh.nacc; P->slot_bytes = sh.slot; P->nslots = sh.nslots; P->split = sh.split;
     const int SP = sh.split;
     P->tm_d3 = (uint32_t)sh.nacc * CN; P->tm_a0 = P->tm_d3 + (uint32_t)KO;
     P->L = smem_layout(H, KO, L, sh.slot, sh.nslots, sh.split);
     const uint32_t slot = sh.slot;
     const uint32_t in_bytes = (uint32_t)HALF * KI * 2, w2_bytes = HALF * 128;
-    const std::vector<float> &W1 = M->wm[0], &W3 = M->wm[L];
+    const std::vector<float> &W1v = M->wm[0], &W3v = M->wm[L];
+    auto w1 = [&](int j, int d) { return j < h ? W1v[(size_t)j * n + d] : 0.f; };
+    auto p1 = [&](int j, int d) { return j < h ? M->p1[(size_t)j * (n - 2) + d] : 0.f; };
+    auto w2 = [&](int j, int k) { return (j < h && k < h) ? M->wm[1][(size_t)j * h + k] : 0.f; };
+    auto w3 = [&](int d, int k) { return k < h ? W3v[(size_t)d * h + k] : 0.f; };
+    auto p2 = [&](int o, int k) { return k < h ? M->p2[(size_t)o * h + k] : 0.f; };
+    auto b1 = [&](int j) { return j < h ? M->bias[0][j] : 0.f; };
+    auto c1 = [&](int j) { return j < h ? M->c1[j] : 0.f; };
+    auto b2 = [&](int j) { return j < h ? M->bias[1][j] : 0.f; };
 
     // ---- the per-tile op list (must match the issuer / epilogue loops of eloc_tc_kernel) ----
     int nops = 0;
@@ -840,15 +852,15 @@ int tc_pack_upload(const nqs_made *M) {
             for (int r = 0; r < 2; ++r)
                 for (int rr = 0; rr < HALF; ++rr) {
                     const int j = c * CN + r * HALF + rr;
-                    const float bj = phase ? M->c1[j] : M->bias[0][j];
+                    const float bj = phase ? c1(j) : b1(j);
                     const float bj_hi = __half2float(__float2half_rn(bj));
                     for (int k = 0; k < KI; ++k) {
                         float v = 0.f;                          // K index 0, 1: bias (hi, lo) against the constant +1 inputs
                         const int d = k - 2;
                         if (k == 0) v = part == 0 ? bj_hi : 0.f;
                         else if (k == 1) v = part == 0 ? bj - bj_hi : 0.f;
-                        else if (phase) { if (d < n - 2) v = part_of(M->p1[(size_t)j * (n - 2) + d], part); }
-                        else if (d < n) v = part_of(W1[(size_t)j * n + d], part);
+                        else if (phase) { if (d < n - 2) v = part_of(p1(j, d), part); }
+                        else if (d < n) v = part_of(w1(j, d), part);
                         put(img[r], base + noswz_offset(rr, k, KI), v);
                         if (v != 0.0f && k / 16 + 1 > nk) nk = k / 16 + 1;
                     }
@@ -864,17 +876,16 @@ int tc_pack_upload(const nqs_made *M) {
             for (int o = 0; o < 4; ++o)
                 for (int k = 0; k < CN; ++k)
                     put(res[1], (size_t)(c * (1 + SP) + part) * 2048 + (size_t)(k / 64) * 1024 + sw128_offset(4 + o, k % 64),
-                        part_of(M->p2[(size_t)o * H + c * CN + k], part));
+                        part_of(p2(o, c * CN + k), part));
         P->mma_issued += (1 + 2 * SP) * 8 * 16; P->mma_dense += 8 * 16;
     };
     // layer-2 chunk c2: k-blocks of 64 with any non-zero weight, and inside a block only the non-zero K-steps
     auto l2_chunk = [&](int c2) {
-        const std::vector<float> &W2 = M->wm[1];
         {   // bias rows of the chunk, one K-step wide: K index 0, 1 = b2 (hi, lo), the rest 0 (A operand = A0's first K-step)
             const uint32_t base = stream_alloc(HALF * 16 * 2, 0);
             for (int r = 0; r < 2; ++r)
                 for (int rr = 0; rr < HALF; ++rr) {
-                    const float bj = M->bias[1][c2 * CN + r * HALF + rr];
+                    const float bj = b2(c2 * CN + r * HALF + rr);
                     const float bj_hi = __half2float(__float2half_rn(bj));
                     put(img[r], base + noswz_offset(rr, 0, 16), bj_hi);
                     put(img[r], base + noswz_offset(rr, 1, 16), bj - bj_hi);
@@ -886,7 +897,7 @@ int tc_pack_upload(const nqs_made *M) {
             uint32_t kmask = 0;
             for (int r = 0; r < CN; ++r)
                 for (int k = 0; k < 64; ++k)
-                    if (W2[(size_t)(c2 * CN + r) * H + kb * 64 + k] != 0.0f) kmask |= 1u << (k / 16);
+                    if (w2(c2 * CN + r, kb * 64 + k) != 0.0f) kmask |= 1u << (k / 16);
             P->mma_dense += 4 * CN;
             if (!kmask) continue;                                        // exact: an all-zero block adds 0
             // single pass: A1[kb] . W2^T.  Split: A1hi[kb] . W2hi^T + A1lo[kb] . W2hi^T + A1hi[kb] . W2lo^T — three
@@ -898,7 +909,7 @@ int tc_pack_upload(const nqs_made *M) {
                 for (int r = 0; r < 2; ++r)
                     for (int rr = 0; rr < HALF; ++rr)
                         for (int k = 0; k < 64; ++k)
-                            put(img[r], base + sw128_offset(rr, k), part_of(W2[(size_t)(c2 * CN + r * HALF + rr) * H + kb * 64 + k], wpart));
+                            put(img[r], base + sw128_offset(rr, k), part_of(w2(c2 * CN + r * HALF + rr, kb * 64 + k), wpart));
                 P->mma_issued += (long long)__builtin_popcount(kmask) * CN;
                 ++nb;
             }
@@ -912,7 +923,7 @@ int tc_pack_upload(const nqs_made *M) {
         int row_lo = KO;
         for (int d = 0; d < n; ++d)
             for (int k = 0; k < CN; ++k)
-                if (W3[(size_t)d * H + c * CN + k] != 0.0f && d < row_lo) row_lo = d;
+                if (w3(d, c * CN + k) != 0.0f && d < row_lo) row_lo = d;
         const int n_lo = row_lo >= KO ? KO - 16 : (row_lo / 16) * 16;
         const int N = KO - n_lo, Nh = N / 2;
         const uint32_t tile_bytes = (uint32_t)2 * Nh * 128;                   // split: the lo-part tile follows the hi-part tile
@@ -924,7 +935,7 @@ int tc_pack_upload(const nqs_made *M) {
                     if (d >= n) continue;
                     for (int k = 0; k < CN; ++k)
                         put(img[r], base + part * tile_bytes + (size_t)(k / 64) * Nh * 128 + sw128_offset(rr, k % 64),
-                            part_of(W3[(size_t)d * H + c * CN + k], part));
+                            part_of(w3(d, c * CN + k), part));
                 }
         P->mma_issued += (long long)(1 + 2 * SP) * 8 * N; P->mma_dense += (long long)8 * KO;
     };
@@ -1022,7 +1033,7 @@ void tc_mma_counts(const nqs_made *M, long long *issued, long long *dense) {
 
 static void fill_common(const nqs_made *M, TcParams &p) {
     const TcPack *P = M->tc;
-    p.n = M->n; p.H = M->h; p.NC = P->NC; p.KI = P->KI; p.KO = P->KO; p.L = M->L; p.nacc = P->nacc; p.nops = P->nops; p.split = P->split;
+    p.n = M->n; p.H = P->Hp; p.NC = P->NC; p.KI = P->KI; p.KO = P->KO; p.L = M->L; p.nacc = P->nacc; p.nops = P->nops; p.split = P->split;
     p.last_a0_op = P->last_a0_op; p.last_l2_op = P->last_l2_op;
     p.tm_d3 = P->tm_d3; p.tm_a0 = P->tm_a0;
     p.wimg = (const uint8_t *)P->d_wimg; p.img_stride = P->img_stride;

@@ -132,8 +132,26 @@ def test_compute_entry_points_fail_loudly_without_gpu():
     assert e.value.status in (-4, -5)
 
 
+def test_host_entry_point_rejects_bits_above_n_qubits():
+    """include/nqs.h: a sample with a bit >= n_qubits set is NQS_EINVAL; nqs_local_energy_host checks it on the host,
+    before any device work (so the check runs here without a GPU)."""
+    w, (x, z, c), params, samples, counts = wl.make_workload(1, batch=4)
+    H = nqs.ham_compile_packed(w.n_qubits, x, z, c)
+    M = nqs.made_create(params)
+    bad = samples.copy()
+    bad[2, 0] |= np.uint64(1) << np.uint64(w.n_qubits)
+    with pytest.raises(nqs.NqsError) as e:
+        nqs.local_energy_host(H, M, bad, counts)
+    assert e.value.status == -1
+    bad = samples.copy()
+    bad[1, 1] = 1
+    with pytest.raises(nqs.NqsError) as e:
+        nqs.local_energy_host(H, M, bad, counts)
+    assert e.value.status == -1
+
+
 def test_tensor_core_path_shape_limits():
-    """include/nqs.h: NQS_PATH_TC takes n_hidden_layers in {1, 2}, hidden a multiple of 128 in [128, 512] and every
+    """include/nqs.h: NQS_PATH_TC takes n_hidden_layers in {1, 2}, hidden in [1, 512] and every
     n_qubits in [3, 126] (two operand columns carry the biases: round16(n + 2) <= 128); everything else is
     NQS_EUNSUPPORTED and NQS_PATH_AUTO falls to the fp32 path (host-only query, no GPU needed)."""
     from paper_2208_05637_b200 import workloads as wl
@@ -149,7 +167,10 @@ def test_tensor_core_path_shape_limits():
             M.resolved_path(nqs.PATH_TC)
         assert ei.value.status == -6
         assert M.resolved_path(nqs.PATH_AUTO) == nqs.PATH_SIMT
-    for n, h in ((20, 64), (20, 192), (20, 640), (20, 32)):
+    for n, h in ((20, 64), (20, 192), (8, 32), (20, 1), (20, 500)):                 # padded to a multiple of 128 inside
+        M = nqs.made_create(wl.make_made_params(n, h, 1))
+        assert M.resolved_path(nqs.PATH_TC) == nqs.PATH_TC and M.resolved_path(nqs.PATH_AUTO) == nqs.PATH_TC
+    for n, h in ((20, 640), (20, 513), (20, 1024)):
         M = nqs.made_create(wl.make_made_params(n, h, 1))
         with pytest.raises(nqs.NqsError) as ei:
             M.resolved_path(nqs.PATH_TC)
