@@ -285,13 +285,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                 auto consume = [&](const int jc) {
                     const int type = S::type(jc);
                     if (type == T_L1S) return;
-                    PROF_SITE(2); WAIT(BAR_EDONE + jc % NACC);
-                    if (jc == S::FIRST_INPLACE) { PROF_SITE(3); WAIT(BAR_D3EMPTY); }              // first write into D3 of this tile
+                    // every address is computed and the weight slot acquired BEFORE the wait for the chunk epilogue, so
+                    // that the first MMA leaves right behind the poll (an idle pipe costs ~100 cycles to restart)
                     const uint32_t a_t = tmem + (uint32_t)(jc % NACC) * CN;
                     // split precision: the epilogue left fp16 hi parts in columns [32 pc, 32 pc + 16) and lo parts in
                     // [32 pc + 16, 32 pc + 32) of every 32-column piece; D3 += Ahi.Bhi + Alo.Bhi + Ahi.Blo
                     if (type == T_P) {                                          // resident P2 tile of this chunk, N = 16
                         const uint32_t b_lo = (res_lo + (uint32_t)S::chunk(jc) * ((SPLIT ? 4096u : 2048u) >> 4)) | lo_sw128;
+                        PROF_SITE(2); WAIT(BAR_EDONE + jc % NACC);
+                        if (jc == S::FIRST_INPLACE) { PROF_SITE(3); WAIT(BAR_D3EMPTY); }          // first write into D3 of this tile
 #pragma unroll
                         for (uint32_t ks = 0; ks < 8; ++ks) {
                             const uint32_t a_k = a_t + 32 * (ks >> 1) + 8 * (ks & 1), b_k = b_lo + (ks >> 2) * (1024u >> 4) + 2 * (ks & 3);
@@ -303,10 +305,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                         }
                     } else {                                                    // streamed layer-3 tile
                         const uint32_t wn = p.sub[++si];
-                        SLOT_ACQUIRE(w);
                         const uint32_t nlo = ((w >> SUB_AUX_SHIFT) & 0xFFu) * 16;      // output rows below n_lo receive exactly 0
                         const uint32_t N = (uint32_t)KO - nlo, kb_step = (N >> 1) * (128u >> 4);
                         const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_sw128, idesc = id0 | ((N >> 3) << 17);
+                        SLOT_ACQUIRE(w);
+                        PROF_SITE(2); WAIT(BAR_EDONE + jc % NACC);
+                        if (jc == S::FIRST_INPLACE) { PROF_SITE(3); WAIT(BAR_D3EMPTY); }          // first write into D3 of this tile
 #pragma unroll
                         for (uint32_t ks = 0; ks < 8; ++ks) {
                             const uint32_t a_k = a_t + 32 * (ks >> 1) + 8 * (ks & 1), b_k = b_lo + (ks >> 2) * kb_step + 2 * (ks & 3);
