@@ -164,6 +164,10 @@ extern "C" void nqs_made_free(nqs_made_t *M) {
     if (!M) return;
     for (void *p : M->d_allocs) cudaFree(p);
     if (M->ws) cudaFree(M->ws);
+    if (M->hx) cudaFree(M->hx);
+    if (M->hc) cudaFree(M->hc);
+    if (M->he) cudaFree(M->he);
+    if (M->h_stream) cudaStreamDestroy(M->h_stream);
     for (cudaEvent_t e : M->ev) cudaEventDestroy(e);
     tc_pack_free(M);
     grad_pack_free(M);
@@ -307,12 +311,26 @@ extern "C" int nqs_local_energy_host(const nqs_ham_t *H, const nqs_made_t *M, co
     }
     int rc = nqs_check_device();
     if (rc) return rc;
-    void *d_x = nullptr, *d_c = nullptr, *d_e = nullptr;
-    cudaStream_t st = nullptr;
-    auto cleanup = [&]() { if (d_x) cudaFree(d_x); if (d_c) cudaFree(d_c); if (d_e) cudaFree(d_e); if (st) cudaStreamDestroy(st); };
-    if (cudaStreamCreateWithFlags(&st, cudaStreamNonBlocking) != cudaSuccess) { cleanup(); return NQS_ECUDA; }
-    if (cudaMalloc(&d_x, 16 * (size_t)B) != cudaSuccess || cudaMalloc(&d_e, 8 * (size_t)B) != cudaSuccess ||
-        (counts_host && cudaMalloc(&d_c, 8 * (size_t)B) != cudaSuccess)) { cudaGetLastError(); cleanup(); return NQS_ENOMEM; }
+    // staging buffers and the stream live in the model handle and are reused (a handle serves one call at a time)
+    if (!M->h_stream && cudaStreamCreateWithFlags(&M->h_stream, cudaStreamNonBlocking) != cudaSuccess) { cudaGetLastError(); return NQS_ECUDA; }
+    if (M->h_rows < (size_t)B) {
+        if (M->hx) cudaFree(M->hx);
+        if (M->hc) cudaFree(M->hc);
+        if (M->he) cudaFree(M->he);
+        M->hx = M->hc = M->he = nullptr; M->h_rows = 0;
+        if (cudaMalloc(&M->hx, 16 * (size_t)B) != cudaSuccess || cudaMalloc(&M->he, 8 * (size_t)B) != cudaSuccess ||
+            cudaMalloc(&M->hc, 8 * (size_t)B) != cudaSuccess) {
+            cudaGetLastError();
+            if (M->hx) cudaFree(M->hx);
+            if (M->hc) cudaFree(M->hc);
+            if (M->he) cudaFree(M->he);
+            M->hx = M->hc = M->he = nullptr;
+            return NQS_ENOMEM;
+        }
+        M->h_rows = (size_t)B;
+    }
+    cudaStream_t st = M->h_stream;
+    void *d_x = M->hx, *d_c = counts_host ? M->hc : nullptr, *d_e = M->he;
     rc = NQS_ECUDA;
     if (cudaMemcpyAsync(d_x, samples_host, 16 * (size_t)B, cudaMemcpyHostToDevice, st) == cudaSuccess &&
         (!counts_host || cudaMemcpyAsync(d_c, counts_host, 8 * (size_t)B, cudaMemcpyHostToDevice, st) == cudaSuccess)) {
@@ -323,7 +341,7 @@ extern "C" int nqs_local_energy_host(const nqs_ham_t *H, const nqs_made_t *M, co
                 cudaStreamSynchronize(st) != cudaSuccess) rc = NQS_ECUDA;
         }
     }
-    cleanup();
+    if (rc == NQS_ECUDA) cudaGetLastError();
     return rc;
 }
 

@@ -9,7 +9,6 @@ namespace {
 constexpr int TR = 16;     // rows (configurations) per CTA tile
 constexpr int NT = 256;    // threads per CTA
 
-__device__ __forceinline__ int popc128(ulonglong2 a) { return __popcll(a.x) + __popcll(a.y); }
 __device__ __forceinline__ int bit128(ulonglong2 a, int q) {
     return (int)(((q < 64 ? a.x : a.y) >> (q & 63)) & 1ull);
 }
@@ -229,9 +228,9 @@ __global__ void __launch_bounds__(NT) eloc_simt_kernel(HamDev hm, MadeDev m, con
             for (uint32_t t = hm.offsets[g]; t < t1; ++t) {
                 const ulonglong2 zy = hm.zy[t];
                 const float2 c = hm.cph[t];
-                const bool neg = (popc128(make_ulonglong2(xr.x & zy.x, xr.y & zy.y)) & 1) != 0;
-                S.x += neg ? -c.x : c.x;
-                S.y += neg ? -c.y : c.y;
+                const float2 cs = nqs_signed(c, nqs_parity_sign(xr, zy));
+                S.x += cs.x;
+                S.y += cs.y;
             }
             // (a5) ratio = exp(dlog|psi|) * cis(dphi); E += S * ratio
             float rr = 1.0f, ri = 0.0f;
@@ -266,9 +265,12 @@ __global__ void reduce_partials_kernel(const float2 *__restrict__ partial, int n
     eloc[i] = e;
 }
 
-// (a3) standalone.  CTA = 128 samples (one per thread) x a range of groups; term tiles are staged through
-// shared memory with cp.async (double-buffered) and every staged term is reused by the 128 samples.
+// (a3) standalone.  CTA = 256 samples (two per thread: every staged term is loaded once for both) x a range of groups;
+// term tiles are staged through shared memory with cp.async (double-buffered) and every staged term is reused by the
+// 256 samples.  Per (sample, term) pair: 4 LOP3 (AND + XOR fold), 1 POPC, 1 shift, 2 LOP3 (sign), 2 FADD.
 constexpr int CT_THREADS = 128;
+constexpr int CT_SPT = 2;                 // samples per thread
+constexpr int CT_ROWS = CT_THREADS * CT_SPT;
 constexpr int CT_TILE = 512;
 
 __device__ __forceinline__ void cp_async16(void *dst, const void *src) {
@@ -286,8 +288,8 @@ __global__ void __launch_bounds__(CT_THREADS) contract_kernel(HamDev hm, const u
     const long long ng = g1 - g0;
     const long long ga = g0 + ng * blockIdx.y / gsplit, gb = g0 + ng * (blockIdx.y + 1) / gsplit;
     if (ga >= gb) return;
-    const long long i = (long long)blockIdx.x * CT_THREADS + threadIdx.x;
-    const ulonglong2 xr = (i < B) ? x[i] : make_ulonglong2(0, 0);
+    const long long i0 = (long long)blockIdx.x * CT_ROWS + threadIdx.x, i1 = i0 + CT_THREADS;     // coalesced stores per half
+    const ulonglong2 xa = (i0 < B) ? x[i0] : make_ulonglong2(0, 0), xb = (i1 < B) ? x[i1] : make_ulonglong2(0, 0);
     const uint32_t t_begin = hm.offsets[ga], t_end = hm.offsets[gb];
     auto stage = [&](int buf, uint32_t t0) {
         for (int k = threadIdx.x; k < CT_TILE; k += CT_THREADS) {
@@ -298,7 +300,7 @@ __global__ void __launch_bounds__(CT_THREADS) contract_kernel(HamDev hm, const u
     };
     long long g = ga;
     uint32_t next_off = hm.offsets[g + 1];
-    float2 S = make_float2(0.f, 0.f);
+    float2 Sa = make_float2(0.f, 0.f), Sb = Sa;
     int buf = 0;
     stage(0, t_begin);
     for (uint32_t t0 = t_begin; t0 < t_end; t0 += CT_TILE, buf ^= 1) {
@@ -308,19 +310,23 @@ __global__ void __launch_bounds__(CT_THREADS) contract_kernel(HamDev hm, const u
         const int cnt = min((uint32_t)CT_TILE, t_end - t0);
         for (int k = 0; k < cnt; ++k) {
             while (t0 + k == next_off) {                               // uniform across the CTA
-                if (i < B) S_out[(size_t)(g - g0) * B + i] = S;
-                S = make_float2(0.f, 0.f);
+                float2 *row = S_out + (size_t)(g - g0) * B;
+                if (i0 < B) row[i0] = Sa;
+                if (i1 < B) row[i1] = Sb;
+                Sa = Sb = make_float2(0.f, 0.f);
                 ++g; next_off = hm.offsets[g + 1];
             }
             const ulonglong2 zy = s_zy[buf][k];
             const float2 c = s_c[buf][k];
-            const bool neg = (popc128(make_ulonglong2(xr.x & zy.x, xr.y & zy.y)) & 1) != 0;
-            S.x += neg ? -c.x : c.x;
-            S.y += neg ? -c.y : c.y;
+            const float2 ca = nqs_signed(c, nqs_parity_sign(xa, zy)), cb = nqs_signed(c, nqs_parity_sign(xb, zy));
+            Sa.x += ca.x; Sa.y += ca.y;
+            Sb.x += cb.x; Sb.y += cb.y;
         }
         __syncthreads();
     }
-    if (i < B) S_out[(size_t)(g - g0) * B + i] = S;
+    float2 *row = S_out + (size_t)(g - g0) * B;
+    if (i0 < B) row[i0] = Sa;
+    if (i1 < B) row[i1] = Sb;
 }
 
 // (a6) count-weighted statistics in fp64, one CTA, fixed summation order.
@@ -380,7 +386,7 @@ int launch_cond_simt(const MadeDev &m, const ulonglong2 *cfg, long long E, int d
 int launch_contract(const HamDev &hm, const ulonglong2 *x, long long B, long long g0, long long g1, float2 *S,
                     cudaStream_t st) {
     if (B <= 0 || g1 <= g0) return NQS_OK;
-    const long long nb = (B + CT_THREADS - 1) / CT_THREADS;
+    const long long nb = (B + CT_ROWS - 1) / CT_ROWS;
     long long gs = (8ll * num_sms() + nb - 1) / nb;           // ~8 resident CTAs (32 warps) per SM: the term loop is latency-bound below that
     if (gs > g1 - g0) gs = g1 - g0;
     if (gs < 1) gs = 1;

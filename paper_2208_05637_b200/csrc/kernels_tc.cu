@@ -576,9 +576,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                 for (uint32_t tt = __ldg(&p.hm.offsets[g]); tt < t1; ++tt) {
                     const ulonglong2 zy = __ldg(&p.hm.zy[tt]);
                     const float2 c = __ldg(&p.hm.cph[tt]);
-                    const bool neg = ((__popcll(cur.xq.x & zy.x) + __popcll(cur.xq.y & zy.y)) & 1) != 0;
-                    S.x += neg ? -c.x : c.x;
-                    S.y += neg ? -c.y : c.y;
+                    const float2 cs = nqs_signed(c, nqs_parity_sign(cur.xq, zy));
+                    S.x += cs.x;
+                    S.y += cs.y;
                 }
             }
 #ifdef TC_PROF
@@ -699,9 +699,9 @@ __global__ void diag_init_kernel(HamDev hm, const ulonglong2 *__restrict__ x, lo
         for (uint32_t t = hm.offsets[0]; t < t1; ++t) {
             const ulonglong2 zy = __ldg(&hm.zy[t]);
             const float2 c = __ldg(&hm.cph[t]);
-            const bool neg = ((__popcll(xr.x & zy.x) + __popcll(xr.y & zy.y)) & 1) != 0;
-            S.x += neg ? -c.x : c.x;
-            S.y += neg ? -c.y : c.y;
+            const float2 cs = nqs_signed(c, nqs_parity_sign(xr, zy));
+            S.x += cs.x;
+            S.y += cs.y;
         }
     }
     eloc[i] = S;

@@ -42,6 +42,18 @@ struct MadeDev {
 };
 
 #ifdef __CUDACC__
+// Sign bit of (-1)^{popcount(x & s)} (Eq. 16) as a float sign mask: 0x80000000 if the parity is odd.
+// parity(a) ^ parity(b) = parity(a ^ b), so the four 32-bit words are AND-ed with the mask, XOR-folded (LOP3) and ONE
+// popcount decides (POPC is a quarter-rate pipe; the straightforward form needs four).
+__device__ __forceinline__ uint32_t nqs_parity_sign(ulonglong2 x, ulonglong2 s) {
+    const unsigned long long f = (x.x & s.x) ^ (x.y & s.y);
+    return (uint32_t)__popc((uint32_t)f ^ (uint32_t)(f >> 32)) << 31;
+}
+// c * (-1)^{parity}: flip the sign bits of (Re, Im)
+__device__ __forceinline__ float2 nqs_signed(float2 c, uint32_t sign) {
+    return make_float2(__uint_as_float(__float_as_uint(c.x) ^ sign), __uint_as_float(__float_as_uint(c.y) ^ sign));
+}
+
 // Positions whose conditional Eq. 14 clamps, for one configuration zp given in POSITION order (reading A13: at a
 // position of spin s with c spin-s bits set before it and m spin-s positions left, forced to 0 if c = n_s, to 1 if
 // n_s - c = m).  *valid = the string respects every clamp (equivalently satisfies Eq. 12).
@@ -101,6 +113,10 @@ struct nqs_made {
     // workspace (grown on demand, reused across calls)
     mutable void  *ws = nullptr;
     mutable size_t ws_bytes = 0;
+    // staging buffers and stream of nqs_local_energy_host (grown on demand, reused across calls)
+    mutable void *hx = nullptr, *hc = nullptr, *he = nullptr;
+    mutable size_t h_rows = 0;
+    mutable cudaStream_t h_stream = nullptr;
     // timing of the chain kernel (nqs_last_chain_kernel_ms)
     mutable std::vector<cudaEvent_t> ev;        // pairs (start, stop)
     mutable int ev_used = 0;
