@@ -80,7 +80,7 @@ __host__ __device__ inline SmemLayout smem_layout(int H, int KO, int L, uint32_t
 }
 
 struct TcParams {
-    int n, H, NC, KI, KO, L, nacc, nops, split;
+    int n, H, NC, KI, KO, L, nacc, nops, split, seq;
     int last_a0_op, last_l2_op;
     uint32_t tm_d3, tm_a0;               // TMEM columns: accumulator a at a * CN, D3 at tm_d3, A0 at tm_a0
     const uint8_t *wimg; uint32_t img_stride;     // streamed weight image of cluster rank r at wimg + r * img_stride
@@ -138,15 +138,18 @@ __device__ __forceinline__ unsigned long long shr128(ulonglong2 a, int s) {     
 // chunk c (in place) / phase chunk c alternating.  Op j runs in accumulator j % NACC, whose epilogue group (warps
 // W_EPI + 4 a ..) handles every op of that accumulator; the consumer of an in-place op is issued LAG = NACC - 1 ops
 // later, just before the accumulator's next producer.
-template <int NC, int L, int NACC>
+template <int NC, int L, int NACC, bool SEQ>
 struct Sched {
     static constexpr int NOPS = (L == 2) ? 3 * NC : 2 * NC;
     static constexpr int LAG = NACC - 1;
-    static constexpr int FIRST_INPLACE = (L == 2) ? (NC > 1 ? 2 : 1) : 0;
+    static constexpr int FIRST_INPLACE = (L == 2) ? (SEQ ? NC : (NC > 1 ? 2 : 1)) : 0;
     static constexpr int LAST_A0 = (L == 2) ? NOPS - 2 : NOPS - 1;
-    // two hidden layers: L1S 0 | (L1S c+1, P c, L2 c) for c < NC-1 | P NC-1, L2 NC-1
+    // two hidden layers, interleaved (layer-2 chunk c reads layer-1 chunks <= c only — the sorted-degree masks):
+    //     L1S 0 | (L1S c+1, P c, L2 c) for c < NC-1 | P NC-1, L2 NC-1
+    // two hidden layers, SEQ (any masks: some layer-2 chunk reads a later layer-1 chunk): every L1S first, then (P c, L2 c)
     __host__ __device__ static constexpr int type(int j) {
         if (L != 2) return (j & 1) ? (int)T_P : (int)T_L1I;
+        if (SEQ) return j < NC ? (int)T_L1S : (((j - NC) & 1) ? (int)T_L2 : (int)T_P);
         if (j == 0) return (int)T_L1S;
         const int jj = j - 1;
         if (jj < 3 * (NC - 1)) return jj % 3 == 0 ? (int)T_L1S : (jj % 3 == 1 ? (int)T_P : (int)T_L2);
@@ -154,6 +157,7 @@ struct Sched {
     }
     __host__ __device__ static constexpr int chunk(int j) {
         if (L != 2) return j / 2;
+        if (SEQ) return j < NC ? j : (j - NC) / 2;
         if (j == 0) return 0;
         const int jj = j - 1;
         if (jj < 3 * (NC - 1)) return jj % 3 == 0 ? jj / 3 + 1 : jj / 3;
@@ -161,9 +165,9 @@ struct Sched {
     }
 };
 
-template <int NC, int L, int NACC, bool SPLIT>
+template <int NC, int L, int NACC, bool SPLIT, bool SEQ>
 __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc_kernel(const __grid_constant__ TcParams p) {
-    using S = Sched<NC, L, NACC>;
+    using S = Sched<NC, L, NACC, SEQ>;
     extern __shared__ __align__(1024) uint8_t smem[];
     __shared__ uint32_t s_tmem_base;
     const SmemLayout SL = smem_layout(p.H, p.KO, p.L, p.slot_bytes, p.nslots, SPLIT ? 1 : 0);
@@ -711,7 +715,7 @@ __global__ void diag_init_kernel(HamDev hm, const ulonglong2 *__restrict__ x, lo
 
 // ------------------------------------------------------------------------------------------------------------
 struct TcPack {
-    int KI = 0, KO = 0, NC = 0, nacc = 0, nops = 0, nsub = 0, nfills = 0, nslots = 0, last_a0_op = -1, last_l2_op = -1, split = 0, Hp = 0;
+    int KI = 0, KO = 0, NC = 0, nacc = 0, nops = 0, nsub = 0, nfills = 0, nslots = 0, last_a0_op = -1, last_l2_op = -1, split = 0, Hp = 0, seq = 0;
     uint32_t slot_bytes = 0, res_bytes = 0, img_stride = 0, tm_d3 = 0, tm_a0 = 0;
     void *d_wimg = nullptr, *d_fills = nullptr, *d_res = nullptr, *d_bias = nullptr;
     void *d_fpos = nullptr; size_t fpos_cap = 0;
@@ -807,7 +811,17 @@ int tc_pack_upload(const nqs_made *M) {
         if (t == T_L2) P->last_l2_op = nops;
         ++nops;
     };
-    if (L == 2) {
+    // The interleaved order issues layer-2 chunk c before the layer-1 chunks > c exist: legal only if no layer-2 chunk has
+    // a non-zero weight on a later layer-1 chunk (true for the sorted default degrees, where the masks are prefixes).
+    if (L == 2)
+        for (int c2 = 0; c2 < NC; ++c2)
+            for (int r = 0; r < CN; ++r)
+                for (int k = (c2 + 1) * CN; k < H; ++k)
+                    if (w2(c2 * CN + r, k) != 0.0f) P->seq = 1;
+    if (L == 2 && P->seq) {
+        for (int c = 0; c < NC; ++c) push_op(T_L1S, c);
+        for (int c = 0; c < NC; ++c) { push_op(T_P, c); push_op(T_L2, c); }
+    } else if (L == 2) {
         push_op(T_L1S, 0);
         for (int c = 0; c < NC; ++c) {
             if (c + 1 < NC) push_op(T_L1S, c + 1);
@@ -1037,7 +1051,7 @@ void tc_mma_counts(const nqs_made *M, long long *issued, long long *dense) {
 
 static void fill_common(const nqs_made *M, TcParams &p) {
     const TcPack *P = M->tc;
-    p.n = M->n; p.H = P->Hp; p.NC = P->NC; p.KI = P->KI; p.KO = P->KO; p.L = M->L; p.nacc = P->nacc; p.nops = P->nops; p.split = P->split;
+    p.n = M->n; p.H = P->Hp; p.NC = P->NC; p.KI = P->KI; p.KO = P->KO; p.L = M->L; p.nacc = P->nacc; p.nops = P->nops; p.split = P->split; p.seq = P->seq;
     p.last_a0_op = P->last_a0_op; p.last_l2_op = P->last_l2_op;
     p.tm_d3 = P->tm_d3; p.tm_a0 = P->tm_a0;
     p.wimg = (const uint8_t *)P->d_wimg; p.img_stride = P->img_stride;
@@ -1075,18 +1089,18 @@ long long *g_tc_prof = nullptr;   // [148][16], set by the profiling harness thr
 extern "C" void nqs_tc_prof_buffer(long long *dev_buf) { g_tc_prof = dev_buf; }
 #endif
 
-template <int NC, int L, int NACC, bool SPLIT>
+template <int NC, int L, int NACC, bool SPLIT, bool SEQ>
 static int launch_inst(const TcParams &p, int grid, uint32_t smem_bytes, cudaStream_t st) {
-    using S = Sched<NC, L, NACC>;
+    using S = Sched<NC, L, NACC, SEQ>;
     if (p.nops != S::NOPS) return NQS_EUNSUPPORTED;
     for (int j = 0; j < S::NOPS; ++j)                        // the host-packed op list must be the compiled schedule
         if (p.optype[j] != S::type(j) || p.opchunk[j] != S::chunk(j)) return NQS_EUNSUPPORTED;
     // the attribute is per device and per kernel; setting it is a cheap host call, so no process-wide cache
-    if (cudaFuncSetAttribute(eloc_tc_kernel<NC, L, NACC, SPLIT>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes) != cudaSuccess) {
+    if (cudaFuncSetAttribute(eloc_tc_kernel<NC, L, NACC, SPLIT, SEQ>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_bytes) != cudaSuccess) {
         cudaGetLastError();
         return NQS_ECUDA;
     }
-    eloc_tc_kernel<NC, L, NACC, SPLIT><<<grid, NTHREADS, smem_bytes, st>>>(p);
+    eloc_tc_kernel<NC, L, NACC, SPLIT, SEQ><<<grid, NTHREADS, smem_bytes, st>>>(p);
     return NQS_OK;
 }
 
@@ -1100,7 +1114,9 @@ static int launch_chain(const TcPack *P, TcParams &p, long long ntiles, cudaStre
     const int grid = 2 * (int)(npairs < ncl_max ? npairs : ncl_max);
     int rc = NQS_EUNSUPPORTED;
     // hidden <= 256 runs in split precision (tc_shape), wider nets in a single fp16 pass
-#define TC_CASE(NC_, L_, NA_, SP_) case (NC_ * 16 + L_ * 4 + NA_): rc = launch_inst<NC_, L_, NA_, SP_>(p, grid, P->L.total, st); break;
+#define TC_CASE(NC_, L_, NA_, SP_) case (NC_ * 16 + L_ * 4 + NA_): \
+        rc = (L_ == 2 && p.seq) ? launch_inst<NC_, L_, NA_, SP_, (L_ == 2)>(p, grid, P->L.total, st) \
+                                : launch_inst<NC_, L_, NA_, SP_, false>(p, grid, P->L.total, st); break;
     if ((p.split != 0) != (p.NC <= 2)) return NQS_EUNSUPPORTED;
     switch (p.NC * 16 + p.L * 4 + p.nacc) {
         TC_CASE(1, 1, 2, true) TC_CASE(2, 1, 2, true) TC_CASE(3, 1, 2, false) TC_CASE(4, 1, 2, false)

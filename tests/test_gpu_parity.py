@@ -88,6 +88,71 @@ def test_logpsi_parity(n, h, L, order):
     assert nqs.made_logpsi(M, torch.zeros((0, 2), dtype=torch.int64, device=DEV)).shape == (0, 2)   # B = 0
 
 
+def test_logpsi_tensor_core_vs_fp32_path_random_shapes():
+    """Fuzz over shapes the fixed lists do not name: random (n, hidden, layers, order, degrees) with hidden NOT a
+    multiple of 128 (zero-padded inside), both precisions (split for padded hidden <= 256, single pass above), two or
+    three accumulators, ragged multi-tile launches.  GPU vs GPU against the fp32 path (itself checked against the
+    oracle above), so 24 shapes cost a second; two shapes also go to the oracle."""
+    rng = np.random.default_rng(2208)
+    worst = {}
+    for it in range(24):
+        n = int(rng.integers(3, 127))
+        h = int(rng.integers(1, 513))
+        L = int(rng.integers(1, 3))
+        order = ["reverse", "identity", "random"][int(rng.integers(0, 3))]
+        p = wl.make_made_params(n, h, 5000 + it, n_hidden_layers=L, order=order)
+        if it % 3 == 0:                                          # unsorted degrees: masks are not prefixes
+            p.deg_hidden = rng.integers(1, max(2, n), size=(L, h)).astype(np.int32)
+        M = nqs.made_create(p)
+        assert M.resolved_path(nqs.PATH_TC) == nqs.PATH_TC, (n, h, L)
+        B = int(rng.integers(1, 1200))
+        cfgs = wl.pack_bits(rng.integers(0, 2, size=(B, n)).astype(np.uint8))
+        a = nqs.made_logpsi(M, _dev_u64(cfgs), path=nqs.PATH_TC).cpu().numpy().astype(np.float64)
+        b = nqs.made_logpsi(M, _dev_u64(cfgs), path=nqs.PATH_SIMT).cpu().numpy().astype(np.float64)
+        hp = (h + 127) // 128 * 128
+        tol = 4e-4 if hp <= 256 else TC_LOGPSI_TOL               # split precision: the fp32 path's own 2e-4, twice
+        err = np.abs(a - b).max()
+        worst[hp <= 256] = max(worst.get(hp <= 256, 0.0), err)
+        assert np.isfinite(a).all() and err < tol, (n, h, L, order, B, err)
+        if it in (1, 2):
+            ref = omade.logpsi(p, cfgs[:16])
+            assert np.abs(a[:16, 0] - ref.real).max() < tol and np.abs(a[:16, 1] - ref.imag).max() < tol
+    print(f"[parity] TC vs fp32 path over 24 random shapes: max|dlogpsi| split {worst.get(True, 0):.2e}, single pass {worst.get(False, 0):.2e}")
+
+
+def test_eloc_tensor_core_vs_fp32_path_random_shapes():
+    """The same fuzz through nqs_local_energy: random generic Hamiltonians (odd Y counts, with and without an f = 0
+    group) on random model shapes, several ragged sample blocks, counts; every row of the tensor-core path against the
+    fp32 path, which the oracle tests above pin.  Bound: sum|c| max|ratio| times the ratio error the log psi bound
+    allows (2 sqrt 2 tol), as in test_generic_odd_Y_no_diagonal_on_tensor_core_path."""
+    rng = np.random.default_rng(52637)
+    for it in range(10):
+        n = int(rng.integers(5, 127))
+        h = int(rng.integers(1, 513))
+        L = int(rng.integers(1, 3))
+        p = wl.make_made_params(n, h, 7000 + it, n_hidden_layers=L, order=["reverse", "random"][it & 1])
+        if it % 4 == 1:
+            p.deg_hidden = rng.integers(1, n, size=(L, h)).astype(np.int32)
+        codes, coeffs = _few_flip_pauli_list(rng, n, 120)
+        if it % 2 == 0:
+            codes[:30, 0] = np.where(codes[:30, 0] == 2, 3, 0)   # some strings without any flip: an f = 0 group exists
+            codes[:30, 1:] = np.where(np.isin(codes[:30, 1:], (1, 2)), 3, codes[:30, 1:])
+        H = nqs.ham_compile(codes, coeffs)
+        M = nqs.made_create(p)
+        B = int(rng.integers(1, 700))
+        xs = _dev_u64(wl.pack_bits(rng.integers(0, 2, size=(B, n)).astype(np.uint8)))
+        cn = torch.from_numpy(rng.integers(1, 50, size=B).astype(np.int64)).to(DEV)
+        mb = [0, 128, 200][it % 3]
+        e_tc, s_tc = nqs.local_energy(H, M, xs, cn, minibatch=mb, path=nqs.PATH_TC)
+        e_si, s_si = nqs.local_energy(H, M, xs, cn, minibatch=mb, path=nqs.PATH_SIMT)
+        d = (e_tc - e_si).cpu().numpy().astype(np.float64)
+        hp = (h + 127) // 128 * 128
+        tol = H.sum_abs_coeff * max(1.0, s_si[4]) * 2 * 2 ** 0.5 * (4e-4 if hp <= 256 else TC_LOGPSI_TOL)
+        err = np.hypot(d[:, 0], d[:, 1]).max()
+        assert torch.isfinite(e_tc).all() and err <= tol, (it, n, h, L, B, err, tol)
+        assert s_tc[0] == s_si[0] and abs(s_tc[1] - s_si[1]) <= tol * s_si[0]
+
+
 @pytest.mark.parametrize("n,h", [(20, 128), (76, 128), (40, 256), (76, 512), (100, 384)])
 def test_logpsi_tensor_core_many_tiles_per_cta(n, h):
     """Persistent-kernel paths that a few-tile launch never reaches: every CTA walks several 128-row tiles, so
