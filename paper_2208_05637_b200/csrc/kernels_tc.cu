@@ -813,10 +813,12 @@ int tc_pack_upload(const nqs_made *M) {
     };
     // The interleaved order issues layer-2 chunk c before the layer-1 chunks > c exist: legal only if no layer-2 chunk has
     // a non-zero weight on a later layer-1 chunk (true for the sorted default degrees, where the masks are prefixes).
+    // (The interleaved list has L1S c+1 ahead of L2 c, so a chunk may also read the NEXT layer-1 chunk: with sorted
+    // degrees, units on both sides of a chunk boundary can share a degree.)
     if (L == 2)
         for (int c2 = 0; c2 < NC; ++c2)
             for (int r = 0; r < CN; ++r)
-                for (int k = (c2 + 1) * CN; k < H; ++k)
+                for (int k = (c2 + 2) * CN; k < H; ++k)
                     if (w2(c2 * CN + r, k) != 0.0f) P->seq = 1;
     if (L == 2 && P->seq) {
         for (int c = 0; c < NC; ++c) push_op(T_L1S, c);
@@ -979,6 +981,10 @@ int tc_pack_upload(const nqs_made *M) {
         int pending[3] = {-1, -1, -1};
         int l1s_op[MAX_NC] = {0};
         for (int j = 0; j < nops; ++j) if (P->optype[j] == T_L1S) l1s_op[P->opchunk[j]] = j;
+        for (int j = 0; j < nops; ++j)                           // every layer-1 chunk a layer-2 op reads is issued before it
+            if (P->optype[j] == T_L2)
+                for (int cn = 0; cn <= P->l2need[P->opchunk[j]]; ++cn)
+                    if (l1s_op[cn] > j) { delete P; return NQS_EUNSUPPORTED; }
         auto consumed = [&](int j) { if (P->optype[j] != T_L1S && pending[j % sh.nacc] == j) pending[j % sh.nacc] = -1; };
         for (int j = 0; j < nops; ++j) {
             const int a = j % sh.nacc;
