@@ -122,7 +122,7 @@ def time_oracle(w, ham, params, samples, n_samples, one_thread=False):
 # DRAM bytes (read + write) of ONE eloc_tc_kernel launch from the `ncu --set full` capture summarised in
 # profiles/r2_final_summary.md, keyed by (cfg, samples per launch).  A constant of that capture, not measured live: the
 # full-size launch (8,192 samples, 2.4 s x ~45 replay passes) did not finish under ncu, the 2,048-sample launch did.
-NCU_DRAM_BYTES_PER_LAUNCH = {(5, 2048): 345632000 + 7343616}
+NCU_DRAM_BYTES_PER_LAUNCH = {(5, 2048): 326464000 + 7157248}
 
 
 def time_contraction(nqs, torch, H, xs, stream, clocks_mhz):

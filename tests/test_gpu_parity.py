@@ -120,6 +120,22 @@ def test_logpsi_tensor_core_vs_fp32_path_random_shapes():
     print(f"[parity] TC vs fp32 path over 24 random shapes: max|dlogpsi| split {worst.get(True, 0):.2e}, single pass {worst.get(False, 0):.2e}")
 
 
+def test_tc_flops_bookkeeping():
+    """nqs_made_tc_flops (the roofline report's issued / dense flops per psi evaluation): the dense figure is the
+    chain's plain MAC count on the padded shapes, the issued one lies between the algorithmic count bench.py uses
+    (423,346 at cfg 5) and the dense one in single-pass mode, and is about three times larger in
+    split-precision mode."""
+    w, _, params, _, M = workload(5)
+    issued, dense = M.tc_flops()
+    n, h = w.n_qubits, w.hidden
+    KI, KO = 80, 80                                              # round16(n + 2), round16(n + 4)
+    assert dense == 2 * (2 * KI * h + h * h + KO * h + 16 * h)   # W1 + P1 (K = KI), W2, W3 (N = KO), P2 (N = 16)
+    assert 423346 < issued < dense
+    w2, _, params2, _, M2 = workload(2)
+    i2, d2 = M2.tc_flops()
+    assert i2 > 2 * (2 * (11185 + 2816))                         # split precision issues > 2 x the algorithmic flops
+
+
 def test_eloc_tensor_core_vs_fp32_path_random_shapes():
     """The same fuzz through nqs_local_energy: random generic Hamiltonians (odd Y counts, with and without an f = 0
     group) on random model shapes, several ragged sample blocks, counts; every row of the tensor-core path against the
