@@ -367,6 +367,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                                 for (uint32_t ks = 0; ks < 4; ++ks)
                                     if ((kmask >> ks) & 1u) mma_ss_cg2(d, a_lo + 2 * ks, hi_sw128, b_lo + 2 * ks, hi_sw128, id128, accum);
                             }
+                            if (SPLIT && (w & SUB_ACC)) {       // the hi weight block serves the lo activations too (H/64 k-blocks on)
+                                const uint32_t a_l2 = a_lo + (uint32_t)(p.H / 64) * (16384u >> 4);
+#pragma unroll
+                                for (uint32_t ks = 0; ks < 4; ++ks)
+                                    if ((kmask >> ks) & 1u) mma_ss_cg2(d, a_l2 + 2 * ks, hi_sw128, b_lo + 2 * ks, hi_sw128, id128, accum);
+                            }
                             SLOT_RELEASE(w);
                             w = wn;
                         }
@@ -920,17 +926,19 @@ int tc_pack_upload(const nqs_made *M) {
                     if (w2(c2 * CN + r, kb * 64 + k) != 0.0f) kmask |= 1u << (k / 16);
             P->mma_dense += 4 * CN;
             if (!kmask) continue;                                        // exact: an all-zero block adds 0
-            // single pass: A1[kb] . W2^T.  Split: A1hi[kb] . W2hi^T + A1lo[kb] . W2hi^T + A1hi[kb] . W2lo^T — three
-            // streamed blocks (A k-block, weight part); the lo activations live H/64 k-blocks after the hi ones
-            const int npass = SP ? 3 : 1;
+            // single pass: A1[kb] . W2^T.  Split: A1hi[kb] . W2hi^T + A1lo[kb] . W2hi^T + A1hi[kb] . W2lo^T — two
+            // streamed blocks (weight parts); the lo activations live H/64 k-blocks after the hi ones
+            // (the hi weight block is streamed once and used against both activation parts: flag SUB_ACC)
+            const int npass = SP ? 2 : 1;
             for (int ps = 0; ps < npass; ++ps) {
-                const int a_kb = kb + (ps == 1 ? H / 64 : 0), wpart = ps == 2 ? 1 : 0;
+                const int a_kb = kb, wpart = ps;
                 const uint32_t base = stream_alloc(w2_bytes, (uint32_t)a_kb | (kmask << 4));
+                if (SP && ps == 0) sub.back() |= SUB_ACC;
                 for (int r = 0; r < 2; ++r)
                     for (int rr = 0; rr < HALF; ++rr)
                         for (int k = 0; k < 64; ++k)
                             put(img[r], base + sw128_offset(rr, k), part_of(w2(c2 * CN + r * HALF + rr, kb * 64 + k), wpart));
-                P->mma_issued += (long long)__builtin_popcount(kmask) * CN;
+                P->mma_issued += (long long)__builtin_popcount(kmask) * CN * ((SP && ps == 0) ? 2 : 1);
                 ++nb;
             }
             need = kb / 2;
