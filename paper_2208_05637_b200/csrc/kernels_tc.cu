@@ -81,13 +81,11 @@ __host__ __device__ inline SmemLayout smem_layout(int H, int KO, int L, uint32_t
 
 struct TcParams {
     int n, H, NC, KI, KO, L, nacc, nops, split, seq;
-    int last_a0_op, last_l2_op;
     uint32_t tm_d3, tm_a0;               // TMEM columns: accumulator a at a * CN, D3 at tm_d3, A0 at tm_a0
     const uint8_t *wimg; uint32_t img_stride;     // streamed weight image of cluster rank r at wimg + r * img_stride
     const uint2 *fills; int nfills;      // per-tile ring fills (byte offset, bytes), consumption order, same for both ranks
     uint32_t sub[MAX_SUB + 1];
     uint8_t nblk[MAX_NC];                // layer-2 k-blocks issued per output chunk
-    uint8_t l2need[MAX_NC];              // layer-2 chunk c needs A1 chunks 0 .. l2need[c]
     uint8_t optype[MAX_OPS], opchunk[MAX_OPS];
     uint8_t prewait[MAX_OPS];            // bit a: wait for the chunk epilogue pending on accumulator a before issuing op j
     uint32_t cntmask;                    // bit a: accumulator a is used an odd number of times per tile
@@ -721,7 +719,7 @@ __global__ void diag_init_kernel(HamDev hm, const ulonglong2 *__restrict__ x, lo
 
 // ------------------------------------------------------------------------------------------------------------
 struct TcPack {
-    int KI = 0, KO = 0, NC = 0, nacc = 0, nops = 0, nsub = 0, nfills = 0, nslots = 0, last_a0_op = -1, last_l2_op = -1, split = 0, Hp = 0, seq = 0;
+    int KI = 0, KO = 0, NC = 0, nacc = 0, nops = 0, nsub = 0, nfills = 0, nslots = 0, split = 0, Hp = 0, seq = 0;
     uint32_t slot_bytes = 0, res_bytes = 0, img_stride = 0, tm_d3 = 0, tm_a0 = 0;
     void *d_wimg = nullptr, *d_fills = nullptr, *d_res = nullptr, *d_bias = nullptr;
     void *d_fpos = nullptr; size_t fpos_cap = 0;
@@ -813,8 +811,6 @@ int tc_pack_upload(const nqs_made *M) {
     int nops = 0;
     auto push_op = [&](uint8_t t, int c) {
         P->optype[nops] = t; P->opchunk[nops] = (uint8_t)c;
-        if (t != T_L2) P->last_a0_op = nops;
-        if (t == T_L2) P->last_l2_op = nops;
         ++nops;
     };
     // The interleaved order issues layer-2 chunk c before the layer-1 chunks > c exist: legal only if no layer-2 chunk has
@@ -1066,11 +1062,10 @@ void tc_mma_counts(const nqs_made *M, long long *issued, long long *dense) {
 static void fill_common(const nqs_made *M, TcParams &p) {
     const TcPack *P = M->tc;
     p.n = M->n; p.H = P->Hp; p.NC = P->NC; p.KI = P->KI; p.KO = P->KO; p.L = M->L; p.nacc = P->nacc; p.nops = P->nops; p.split = P->split; p.seq = P->seq;
-    p.last_a0_op = P->last_a0_op; p.last_l2_op = P->last_l2_op;
     p.tm_d3 = P->tm_d3; p.tm_a0 = P->tm_a0;
     p.wimg = (const uint8_t *)P->d_wimg; p.img_stride = P->img_stride;
     p.fills = (const uint2 *)P->d_fills; p.nfills = P->nfills;
-    memcpy(p.sub, P->sub, sizeof(p.sub)); memcpy(p.nblk, P->nblk, sizeof(p.nblk)); memcpy(p.l2need, P->l2need, sizeof(p.l2need));
+    memcpy(p.sub, P->sub, sizeof(p.sub)); memcpy(p.nblk, P->nblk, sizeof(p.nblk));
     memcpy(p.optype, P->optype, sizeof(p.optype)); memcpy(p.opchunk, P->opchunk, sizeof(p.opchunk));
     memcpy(p.prewait, P->prewait, sizeof(p.prewait)); p.cntmask = P->cntmask;
     p.resimg = (const uint8_t *)P->d_res; p.res_bytes = P->res_bytes;
