@@ -317,6 +317,7 @@ def main():
         issued, dense = M.tc_flops()
         roof["issued_flops_per_eval"] = issued                # what the kernel sends to the tensor cores (overhead included)
         roof["issued_over_algorithmic"] = issued / flops_eval
+        roof["frac_issued"] = roof["frac"] * issued / flops_eval     # context only: MMA flops the kernel issues / the same peak
 
     contraction = None
     if not args.no_contraction:
