@@ -19,7 +19,10 @@ template <class T>
 static int upload(const T *src, size_t count, void **dst) {
     *dst = nullptr;
     if (cudaMalloc(dst, sizeof(T) * (count ? count : 1)) != cudaSuccess) { cudaGetLastError(); return NQS_ENOMEM; }
-    if (count && cudaMemcpy(*dst, src, sizeof(T) * count, cudaMemcpyHostToDevice) != cudaSuccess) return NQS_ECUDA;
+    if (count && cudaMemcpy(*dst, src, sizeof(T) * count, cudaMemcpyHostToDevice) != cudaSuccess) {
+        cudaGetLastError(); cudaFree(*dst); *dst = nullptr;
+        return NQS_ECUDA;
+    }
     return NQS_OK;
 }
 
@@ -45,12 +48,20 @@ int nqs_ham_upload(const nqs_ham *H) {
             default: cph[t] = make_float2(0.f, c); break;
         }
     }
-    if ((rc = upload(H->flips.data(), H->flips.size(), &H->d_flips))) return rc;
-    if ((rc = upload(H->offsets.data(), H->offsets.size(), &H->d_offsets))) return rc;
-    if ((rc = upload(H->zy.data(), H->zy.size(), &H->d_zy))) return rc;
-    if ((rc = upload(cph.data(), cph.size(), &H->d_cph))) return rc;
-    H->on_device = true;
-    return NQS_OK;
+    if ((rc = upload(H->flips.data(), H->flips.size(), &H->d_flips)) == NQS_OK &&
+        (rc = upload(H->offsets.data(), H->offsets.size(), &H->d_offsets)) == NQS_OK &&
+        (rc = upload(H->zy.data(), H->zy.size(), &H->d_zy)) == NQS_OK &&
+        (rc = upload(cph.data(), cph.size(), &H->d_cph)) == NQS_OK) {
+        H->on_device = true;
+        return NQS_OK;
+    }
+    // a partial upload is released: the handle stays usable for a later attempt
+    if (H->d_flips) cudaFree(H->d_flips);
+    if (H->d_offsets) cudaFree(H->d_offsets);
+    if (H->d_zy) cudaFree(H->d_zy);
+    if (H->d_cph) cudaFree(H->d_cph);
+    H->d_flips = H->d_offsets = H->d_zy = H->d_cph = nullptr;
+    return rc;
 }
 
 HamDev nqs_ham_dev(const nqs_ham *H) {
