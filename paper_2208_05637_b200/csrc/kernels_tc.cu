@@ -272,8 +272,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             long long pw_wait = 0, pw_wf = 0, pw_tot = clock64(), pw_cls[4] = {0, 0, 0, 0};
             int pw_site = 0;                             // 0 = A0FULL, 1 = prewait (accumulator / A1 chunk), 2 = consumer EDONE, 3 = D3EMPTY
 #endif
-#define WAIT(id) do { PROF_T0(); if (!TESTMODE) mbar_spin(BAR_ADDR(id), (ph >> (id)) & 1u); ph ^= 1u << (id); tc_fence_after(); PROF_ADD(pw_wait); PROF_ADD(pw_cls[pw_site]); } while (0)
-#define SLOT_ACQUIRE(w) do { if ((w) & SUB_NEW) { PROF_T0(); if (TESTMODE < 2) mbar_spin(BAR_ADDR(BAR_WFULL + slot), wpar); tc_fence_after(); PROF_ADD(pw_wf); } } while (0)
+#define WAIT(id) do { PROF_T0(); if (!(TESTMODE & 3)) mbar_spin(BAR_ADDR(id), (ph >> (id)) & 1u); ph ^= 1u << (id); tc_fence_after(); PROF_ADD(pw_wait); PROF_ADD(pw_cls[pw_site]); } while (0)
+#define SLOT_ACQUIRE(w) do { if ((w) & SUB_NEW) { PROF_T0(); if ((TESTMODE & 3) < 2) mbar_spin(BAR_ADDR(BAR_WFULL + slot), wpar); tc_fence_after(); PROF_ADD(pw_wf); } } while (0)
 #define SLOT_RELEASE(w) do { if ((w) & SUB_END) { mma_commit_cg2(BAR_ADDR(BAR_WEMPTY + slot)); slot_lo += slot_step; \
                              if (++slot == nslots) { slot = 0; wpar ^= 1u; slot_lo = slots_lo; } } } while (0)
             for (long long ti = 0; ti < ntl; ++ti) {
@@ -342,7 +342,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                         {   // D = [1 1 x'..] . [b2_hi b2_lo 0..]^T: the bias, and the overwrite of the accumulator
                             const uint32_t wn = p.sub[++si];
                             SLOT_ACQUIRE(w);
-                            mma_ts_cg2(d, tm_a0, (slot_lo + (w & SUB_OFF_MASK)) | lo_noswz, hi_noswz16, id128, 0u);
+                            if (!(TESTMODE & 4)) mma_ts_cg2(d, tm_a0, (slot_lo + (w & SUB_OFF_MASK)) | lo_noswz, hi_noswz16, id128, 0u);
                             SLOT_RELEASE(w);
                             w = wn;
                         }
@@ -422,7 +422,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
         uint32_t fb = 0;                                   // bit a: parity of accumulator a's first FULL phase of this tile
         long long pe_wait = 0, pe_a1 = 0, pe_tot = clock64(), pe_fence = 0, pe_arr = 0, pe_ld = 0, pe_ldi = 0, pe_cvt = 0;
         (void)pe_wait; (void)pe_a1; (void)pe_tot; (void)pe_fence; (void)pe_arr; (void)pe_ld; (void)pe_ldi; (void)pe_cvt;
-        if (!TESTMODE)
+        if (!(TESTMODE & 3))
         for (long long ti = 0; ti < ntl; ++ti, fb ^= p.cntmask) {
         bool a1_waited = false;
         uint32_t acc = 0, q = 0;                           // j % NACC, j / NACC
@@ -551,7 +551,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
         float mr = (p.mode == 1 && p.hm.has_diag) ? 1.0f : 0.0f;     // the f = 0 group has ratio exactly 1
         long long pt_a0 = 0, pt_d3 = 0, pt_tot = clock64(), pt_s = 0, pt_fin = 0;
         (void)pt_a0; (void)pt_d3; (void)pt_tot; (void)pt_s; (void)pt_fin;
-        if (ntl > 0 && !TESTMODE) {
+        if (ntl > 0 && !(TESTMODE & 3)) {
             const long long t = 2 * q_lo + rank;
             const bool valid = t < ntiles;
             load_row(t / Gnd, valid, cur);
@@ -560,7 +560,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             clamp_of(zp, fm, inval);
             build_a0(zp);
         }
-        for (long long ti = 0; ti < (TESTMODE ? 0 : ntl); ++ti) {
+        for (long long ti = 0; ti < ((TESTMODE & 3) ? 0 : ntl); ++ti) {
             const long long t = 2 * (q_lo + ti) + rank;
             const bool valid = t < ntiles;
             const long long g = p.g_begin + (t % Gnd);
