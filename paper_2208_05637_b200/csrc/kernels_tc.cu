@@ -299,7 +299,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
 #pragma unroll
                         for (uint32_t ks = 0; ks < 8; ++ks) {
                             const uint32_t a_k = a_t + 32 * (ks >> 1) + 8 * (ks & 1), b_k = b_lo + (ks >> 2) * (1024u >> 4) + 2 * (ks & 3);
-                            mma_ts_cg2(tm_ph, a_k, b_k, hi_sw128, id16, 1u);
+                            if (!(TESTMODE & 8)) mma_ts_cg2(tm_ph, a_k, b_k, hi_sw128, id16, 1u);
                             if (SPLIT) {
                                 mma_ts_cg2(tm_ph, a_k + 16, b_k, hi_sw128, id16, 1u);
                                 mma_ts_cg2(tm_ph, a_k, b_k + (2048u >> 4), hi_sw128, id16, 1u);
@@ -579,7 +579,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
 #ifdef TC_PROF
             const long long _ts = clock64();
 #endif
-            if (p.mode == 1 && valid && cur.i < p.B) {
+            if (p.mode == 1 && valid && cur.i < p.B && !(TESTMODE & 32)) {
                 const uint32_t t1 = __ldg(&p.hm.offsets[g + 1]);
                 for (uint32_t tt = __ldg(&p.hm.offsets[g]); tt < t1; ++tt) {
                     const ulonglong2 zy = __ldg(&p.hm.zy[tt]);
@@ -623,7 +623,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                 const float4 *bp = reinterpret_cast<const float4 *>(s_b3 + c0);
                 float prod0 = 1.0f, prod1 = 1.0f, m0 = 0.0f, m1 = 0.0f;
 #pragma unroll
-                for (int k4 = 0; k4 < 4; ++k4) {
+                for (int k4 = 0; k4 < ((TESTMODE & 16) ? 0 : 4); ++k4) {
                     const float4 bb = bp[k4];
                     const float bk[4] = {bb.x, bb.y, bb.z, bb.w};
 #pragma unroll
