@@ -222,8 +222,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             for (long long q = lane; q < total; q += nprod) {
                 const uint2 pe = __ldg(&p.fills[e]);
                 { PROF_T0(); mbar_wait(&bars[BAR_WEMPTY + slot], par); PROF_ADD(pp_wait); }
+                if (TESTMODE & 128) mbar_arrive_addr(BAR_ADDR(BAR_WFULL + slot));        // probe: no weight traffic at all
+                else {
                 mbar_arrive_expect_tx(&bars[BAR_WFULL + slot], pe.y);
                 bulk_g2s(smem + SL.slots + slot * p.slot_bytes, img + pe.x, pe.y, &bars[BAR_WFULL + slot]);
+                }
                 e += nprod; while (e >= (uint32_t)p.nfills) e -= (uint32_t)p.nfills;
                 slot += nprod; while (slot >= (uint32_t)p.nslots) { slot -= (uint32_t)p.nslots; par ^= 1u; }
             }
@@ -446,7 +449,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             const long long _tc0 = clock64();
 #endif
 #pragma unroll
-            for (int pp = 0; pp < 2; ++pp) {
+            for (int pp = 0; pp < ((TESTMODE & 64) ? 0 : 2); ++pp) {     // probe bit 64: no conversion, no store
                 const uint32_t *v = pp ? vb : va;
                 uint32_t w[16], wl[16];                        // the bias is already in the accumulator (constant input columns)
 #pragma unroll
