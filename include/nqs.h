@@ -48,7 +48,10 @@ enum nqs_status {
     NQS_EUNSUPPORTED = -6    /* the requested path cannot run this shape (e.g. NQS_PATH_TC on hidden > 512)       */
 };
 
-/* Which kernels evaluate the MADE chain.  Both are CUDA; neither touches the CPU.
+/* Which kernels evaluate the MADE chain.  Both are CUDA; neither touches the CPU.  Callers pass NQS_PATH_AUTO; the two
+ * explicit values exist for the parity tests and the benchmark (the fp32 path is the GPU-side reference of the tensor-core
+ * path and the only path for shapes the latter does not take) — there is one implementation per shape, not a dispatch
+ * between backends.
  *  NQS_PATH_SIMT : fp32 FFMA on CUDA cores, every layer (any shape; the parity reference for the tensor-core path).
  *  NQS_PATH_TC   : tcgen05 tensor cores driven by CTA pairs (cta_group::2), fp16 operands / fp32 accumulation in
  *                  TMEM, fused gather of x xor f into the operand tile and log|psi| / phase / ratio / E_loc in the
