@@ -196,6 +196,34 @@ int nqs_local_energy_host(const nqs_ham_t *ham, const nqs_made_t *made, const ui
                           const int64_t *counts_host, int64_t B, int64_t minibatch, int path,
                           float *eloc_out_host, double *stats_out_host);
 
+/* ---- (a6) statistics without any device allocation: PAPER.md:200 Eq. 17, :105 (counter) -------------------------
+ * For callers that cannot let this library call cudaMalloc: a training loop whose framework allocator (PyTorch's
+ * caching allocator, or an arena sized to the card) already owns all free device memory, so that a raw allocation
+ * here fails or starves the framework later; a loop that overlaps several streams and cannot afford the device-wide
+ * synchronisation cudaMalloc / cudaFree imply; a process held to a fixed device-memory budget (an MPS client with a
+ * memory limit, ranks sharing a MIG slice).  Every other compute entry point grows a workspace inside the model
+ * handle on first use; this one allocates nothing, ever — no cudaMalloc, cudaFree, events, streams or library calls
+ * that allocate.
+ *   eloc_dev      device float [B][2] = (Re, Im) of the local energies (the output of nqs_local_energy);
+ *   counts_dev    device int64 [B] multiplicities, or NULL = all ones;
+ *   stats_out_dev device double [4] = { sum n, sum n Re E, sum n Im E, sum n |E|^2 }, overwritten (the first four
+ *                 entries of nqs_local_energy's stats; memory the caller owns, like the inputs);
+ *   B             0 <= B <= NQS_STATS_STATIC_MAX_ROWS; more rows: NQS_ERANGE, nothing launched.  B = 0 writes zeros.
+ * Asynchronous on `cuda_stream`; fp64, fixed summation order (bit-reproducible, unlike an atomic sum).
+ * Scratch: per-CTA partial sums live in a 33 KB array that is part of the library's device image (one slot per 2048
+ * rows, 1024 slots — that is where the row limit comes from).  Every GPU the process uses with libnqs loaded keeps
+ * that array until exit.  Consequences for the caller:
+ *   - the first call made with a given device current looks the array's device address up and caches it; make that
+ *     first call during set-up, before any stream capture on that device;
+ *   - all calls on one device share the array.  The library clears the one word that must start at zero on the
+ *     call's stream, so back-to-back calls on ONE stream are fine; two calls that can overlap on the GPU (different
+ *     streams without an ordering between them) race on it and both results are undefined.
+ * Errors: NQS_EINVAL (NULL pointer, B < 0), NQS_ERANGE (B above the limit), NQS_EARCH / NQS_ECUDA (no sm_100 device,
+ * a runtime call failed), NQS_EUNSUPPORTED (device ordinal >= 64). */
+#define NQS_STATS_STATIC_MAX_ROWS 2097152   /* 2^21 = 1024 scratch slots x 2048 rows */
+int nqs_weighted_stats_static(const float *eloc_dev, const int64_t *counts_dev, int64_t B,
+                              double *stats_out_dev, void *cuda_stream);
+
 /* ---- gradient of the energy objective: PAPER.md:71 Eq. 7, :73 (baseline), :202 (accumulation) ----------
  *   grad L(theta) = Re E[(l_theta(x) - b) conj(grad_theta log f(x))],   b = E[l_theta(x)],
  * the expectation taken over the unique samples weighted by their multiplicities (:105, :200).  log f = log|psi| + i phi

@@ -52,6 +52,7 @@ def lib():
                                        c_void_p, c_void_p, c_void_p]
         L.nqs_local_energy_host.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int64, c_int64, c_int,
                                             c_void_p, c_void_p]
+        L.nqs_weighted_stats_static.argtypes = [c_void_p, c_void_p, c_int64, c_void_p, c_void_p]
         L.nqs_made_set_constraint.argtypes = [c_void_p, c_int, c_int]
         L.nqs_made_num_params.argtypes = [c_void_p, ctypes.POINTER(c_int64)]
         L.nqs_energy_grad.argtypes = [c_void_p, c_void_p, c_void_p, c_void_p, c_int64, c_int64, c_void_p, c_void_p, c_void_p, c_void_p]
@@ -242,6 +243,30 @@ def local_energy_host(ham, made, samples, counts=None, minibatch=0, path=PATH_AU
                                      B, minibatch, path, out.ctypes.data, stats.ctypes.data if want_stats else None),
          "nqs_local_energy_host")
     return out, stats
+
+
+STATS_STATIC_MAX_ROWS = 1 << 21
+
+
+def weighted_stats_static(eloc, counts, out, stream=None):
+    """nqs_weighted_stats_static: the sums of Eq. 17 for callers that cannot let the library allocate device memory
+    (a framework allocator owns the card, cudaMalloc's device-wide synchronisation is unaffordable, or the process has a
+    fixed memory budget).  Nothing is allocated here either: the caller brings every buffer.
+    eloc torch.float32 CUDA [B, 2], counts torch.int64 CUDA [B] or None, out torch.float64 CUDA [4] (overwritten with
+    sum n, sum n Re E, sum n Im E, sum n |E|^2; returned).  B <= STATS_STATIC_MAX_ROWS.  Asynchronous on the stream.
+    Calls on one device share a fixed scratch array inside the library: do not let two of them overlap on the GPU, and
+    make the first call on a device before any stream capture (include/nqs.h)."""
+    import torch
+    if not (out.is_cuda and out.dtype == torch.float64 and out.numel() >= 4 and out.is_contiguous()):
+        raise ValueError("out must be a contiguous CUDA float64 tensor of at least 4 elements")
+    if not (eloc.is_cuda and eloc.dtype == torch.float32 and eloc.is_contiguous()):
+        raise ValueError("eloc must be a contiguous CUDA float32 tensor [B, 2]")
+    if counts is not None and not (counts.is_cuda and counts.dtype == torch.int64 and counts.is_contiguous()
+                                   and counts.shape[0] == eloc.shape[0]):
+        raise ValueError("counts must be a contiguous CUDA int64 tensor [B]")
+    _chk(lib().nqs_weighted_stats_static(eloc.data_ptr(), counts.data_ptr() if counts is not None else None,
+                                         eloc.shape[0], out.data_ptr(), _stream_ptr(stream)), "nqs_weighted_stats_static")
+    return out
 
 
 def energy_grad(made, samples, counts, eloc, minibatch=0, want_baseline=True, stream=None, global_stats=None):

@@ -10,7 +10,8 @@ import sys
 HERE = os.path.dirname(os.path.abspath(__file__))
 CSRC = os.path.join(HERE, "csrc")
 LIB = os.path.join(CSRC, "libnqs.so")
-SOURCES = ["api.cu", "ham_compile.cpp", "made_pack.cpp", "kernels_simt.cu", "kernels_tc.cu", "kernels_grad.cu", "kernels_sample.cu"]
+SOURCES = ["api.cu", "ham_compile.cpp", "made_pack.cpp", "kernels_simt.cu", "kernels_tc.cu", "kernels_grad.cu", "kernels_sample.cu",
+           "stats_static.cu"]
 NVCC_FLAGS = ["-O3", "-std=c++17", "-gencode", "arch=compute_100a,code=sm_100a", "-lineinfo",
               "-Xcompiler", "-fPIC", "--expt-relaxed-constexpr"]
 
