@@ -79,11 +79,29 @@ extern "C" void nqs_ham_free(nqs_ham_t *H) {
     delete H;
 }
 
+static int made_upload_tensors(const nqs_made *M);
+
 int nqs_made_upload(const nqs_made *M) {
     if (M->on_device) return same_device(M->device);
     int rc = nqs_check_device();
     if (rc) return rc;
     cudaGetDevice(&M->device);
+    if ((rc = made_upload_tensors(M))) {
+        // a partial upload is released: the handle stays usable for a later attempt and holds nothing twice
+        for (void *p : M->d_allocs) cudaFree(p);
+        M->d_allocs.clear();
+        M->dev = MadeDev{};
+        return rc;
+    }
+    // The tensor-core pack is optional: if it cannot be built or uploaded the handle still serves NQS_PATH_SIMT,
+    // NQS_PATH_AUTO takes that path and a forced NQS_PATH_TC reports NQS_EUNSUPPORTED (include/nqs.h).
+    if (tc_supported(M) && tc_pack_upload(M) != NQS_OK) { cudaGetLastError(); M->tc_failed = true; }
+    M->on_device = true;
+    return NQS_OK;
+}
+
+static int made_upload_tensors(const nqs_made *M) {
+    int rc = NQS_OK;
     const int n = M->n, h = M->h, L = M->L, npad = M->npad;
     auto up = [&](const std::vector<float> &v, const float **dst) -> int {
         void *p = nullptr;
@@ -148,8 +166,6 @@ int nqs_made_upload(const nqs_made *M) {
         if (L == 2 && (rc = kend_of(M->wm[1], h, h, &d.kend2))) return rc;
         if ((rc = kend_of(M->wm[L], n, h, &d.kend3))) return rc;
     }
-    if (tc_supported(M) && (rc = tc_pack_upload(M))) return rc;
-    M->on_device = true;
     return NQS_OK;
 }
 
@@ -185,10 +201,13 @@ extern "C" void nqs_made_free(nqs_made_t *M) {
     delete M;
 }
 
+// The shape decides, except that a handle whose tensor-core pack failed to upload (tc_failed, known once
+// nqs_made_upload has run) is an fp32-path handle: callers resolve again after the upload.
 static int resolve_path(const nqs_made *M, int path, int *use_tc) {
+    const bool tc_ok = tc_supported(M) && !M->tc_failed;
     if (path == NQS_PATH_SIMT) { *use_tc = 0; return NQS_OK; }
-    if (path == NQS_PATH_TC) { if (!tc_supported(M)) return NQS_EUNSUPPORTED; *use_tc = 1; return NQS_OK; }
-    if (path == NQS_PATH_AUTO) { *use_tc = tc_supported(M) ? 1 : 0; return NQS_OK; }
+    if (path == NQS_PATH_TC) { if (!tc_ok) return NQS_EUNSUPPORTED; *use_tc = 1; return NQS_OK; }
+    if (path == NQS_PATH_AUTO) { *use_tc = tc_ok ? 1 : 0; return NQS_OK; }
     return NQS_EINVAL;
 }
 
@@ -204,6 +223,7 @@ extern "C" int nqs_made_tc_flops(const nqs_made_t *M, int64_t *issued_per_eval, 
     if (!tc_supported(M)) return NQS_EUNSUPPORTED;
     const int rc = nqs_made_upload(M);
     if (rc) return rc;
+    if (!M->tc) return NQS_EUNSUPPORTED;
     long long issued = 0, dense = 0;
     tc_mma_counts(M, &issued, &dense);             // in units of one K-step (16) x one output column, per row
     *issued_per_eval = 32 * issued;
@@ -219,6 +239,7 @@ extern "C" int nqs_made_logpsi(const nqs_made_t *M, const uint64_t *configs_dev,
     if (rc) return rc;
     if (B == 0) return NQS_OK;
     if ((rc = nqs_made_upload(M))) return rc;
+    if ((rc = resolve_path(M, path, &use_tc))) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     if (use_tc) return launch_logpsi_tc(M, (const ulonglong2 *)configs_dev, B, (float2 *)out_dev, st);
     return launch_logpsi_simt(M->dev, (const ulonglong2 *)configs_dev, B, (float2 *)out_dev, st);
@@ -252,6 +273,7 @@ extern "C" int nqs_local_energy(const nqs_ham_t *H, const nqs_made_t *M, const u
     if (!samples_dev || !eloc_out_dev) return NQS_EINVAL;
     if ((rc = nqs_ham_upload(H))) return rc;
     if ((rc = nqs_made_upload(M))) return rc;
+    if ((rc = resolve_path(M, path, &use_tc))) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const HamDev hm = nqs_ham_dev(H);
     const long long mb = minibatch > 0 ? minibatch : 8192;

@@ -108,6 +108,7 @@ struct nqs_made {
     mutable std::vector<void *> d_allocs;
     mutable MadeDev dev{};
     mutable TcPack *tc = nullptr;
+    mutable bool tc_failed = false;             // the tensor-core pack could not be built / uploaded: this handle runs on the fp32 path
     mutable GradPack *grad = nullptr;
     int n_up = -1, n_down = -1;                 // nqs_made_set_constraint
     // workspace (grown on demand, reused across calls)
