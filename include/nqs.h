@@ -65,7 +65,9 @@ enum nqs_status {
  *                  workloads); hidden (padded) <= 256 runs in SPLIT precision — every fp16 operand as hi + lo parts, three MMA
  *                  passes (hi.hi + lo.hi + hi.lo) — because a single fp16 pass misses the bound there (2 x); split
  *                  results are as accurate as the fp32 path (0.03 x the bound) at 3 x the tensor work.
- *  NQS_PATH_AUTO : TC when the shape supports it, else SIMT.
+ *  NQS_PATH_AUTO : TC when the shape supports it, else SIMT.  If the tensor-core weight pack of a supported shape cannot be
+ *                  built or uploaded (device memory), the handle becomes an fp32-path handle: AUTO runs SIMT, a forced
+ *                  NQS_PATH_TC returns NQS_EUNSUPPORTED, and nqs_made_path reports it from then on.
  * A handle (nqs_made_t / nqs_ham_t) owns device scratch that its compute calls reuse: use one handle from one
  * host thread and one CUDA stream at a time, on the device that was current when it was first used (other
  * devices: NQS_EINVAL). */
@@ -97,7 +99,9 @@ int nqs_ham_compile_packed(int n_qubits, int64_t n_terms, const uint64_t *fmask,
  * parser", :154; the syntax is not given -- reading A4): one term per line, the real coefficient first (plain,
  * parenthesised, or a complex literal with zero imaginary part such as "(0.5+0j)"), then either a dense word of
  * n_qubits letters from IXYZ (letter j = qubit j) or sparse factors "X0 Y3 Z12"; '[' ']' '*' ',' separate, '#'
- * comments.  Malformed lines, a qubit named twice or a non-zero imaginary part: NQS_EINVAL. */
+ * comments.  The coefficient is a plain decimal literal ("-0.25", "1.5e-3") read independently of the locale; hex
+ * literals, "nan", "inf" and literals that overflow a double are refused.  Malformed lines, a qubit named twice (an
+ * explicit I counts as naming it) or a non-zero imaginary part: NQS_EINVAL. */
 int nqs_ham_compile_text(int n_qubits, const char *text, nqs_ham_t **out);
 
 /* K = merged term count, G = number of unique flips, sum_abs_coeff = sum_t |c_t| (fp64, merged, the

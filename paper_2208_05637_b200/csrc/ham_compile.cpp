@@ -2,7 +2,9 @@
 // F^{1,2} (flips) / F^{2,3} (signs), keep a buffer of unique flips and their number of occurrences.
 // Rules 1-5 are stated in include/nqs.h.
 #include <algorithm>
+#include <charconv>
 #include <cmath>
+#include <system_error>
 #include <new>
 #include <numeric>
 #include <cstdlib>
@@ -109,6 +111,17 @@ extern "C" int nqs_ham_compile_packed(int n_qubits, int64_t n_terms, const uint6
     return finish(n_qubits, terms, coeffs, out);
 }
 
+// [sign] digits [. digits] [e [sign] digits] -> finite double; *end = first character after it.
+static bool parse_decimal(const char *first, const char *last, double *value, const char **end) {
+    const char *p = first;
+    if (p < last && (*p == '+' || *p == '-')) ++p;
+    if (p >= last || !((*p >= '0' && *p <= '9') || *p == '.')) return false;          // no "nan", "inf", "x..."
+    const std::from_chars_result r = std::from_chars(*first == '+' ? first + 1 : first, last, *value, std::chars_format::general);
+    if (r.ec != std::errc() || !std::isfinite(*value)) return false;                   // overflow ("1e400") included
+    *end = r.ptr;
+    return true;
+}
+
 // Text form of a qubit Hamiltonian (PAPER.md:36 "stored in a string format", :154 "string parser"; the syntax is not
 // given, reading A4): one term per line, coefficient first, then EITHER a dense word of n_qubits letters from IXYZ
 // (letter j = qubit j) OR sparse factors "X0 Y3 Z12" (identity = nothing).  The coefficient may be written plainly
@@ -131,15 +144,22 @@ extern "C" int nqs_ham_compile_text(int n_qubits, const char *text, nqs_ham_t **
             for (char &ch : line) if (ch == '[' || ch == ']' || ch == '*' || ch == ',' || ch == '(' || ch == ')' || ch == '\t' || ch == '\r') ch = ' ';
             size_t i = line.find_first_not_of(' ');
             if (i == std::string::npos) continue;
-            char *end = nullptr;
-            const double c = strtod(line.c_str() + i, &end);
-            if (end == line.c_str() + i) return NQS_EINVAL;
+            // decimal, finite, locale-independent: std::from_chars never reads hex ("0X1 Z2" is 0 * X1 Z2 mangled,
+            // not 1.0 * Z2) and "nan" / "inf" / overflowing literals are refused so that sum|c| stays a number
+            const char *end = nullptr;
+            double c = 0.0;
+            if (!parse_decimal(line.c_str() + i, line.c_str() + line.size(), &c, &end)) return NQS_EINVAL;
             // optional imaginary part "+0j" / "-0.0j": must be zero (real coefficients)
             if (*end == '+' || *end == '-') {
-                char *e2 = nullptr;
-                const double im = strtod(end, &e2);
-                if (e2 != end && (*e2 == 'j' || *e2 == 'i')) { if (im != 0.0) return NQS_EINVAL; end = e2 + 1; }
+                const char *e2 = nullptr;
+                double im = 0.0;
+                if (parse_decimal(end, line.c_str() + line.size(), &im, &e2) && (*e2 == 'j' || *e2 == 'i')) {
+                    if (im != 0.0) return NQS_EINVAL;
+                    end = e2 + 1;
+                }
             }
+            if (*end && *end != ' ') return NQS_EINVAL;                       // the coefficient is a token of its own
+            uint64_t named[2] = {0, 0};                                       // qubits this line has named, I included
             Term t{{0, 0}, {0, 0}, (int64_t)terms.size()};
             const char *q = end;
             bool dense_seen = false;
@@ -152,7 +172,8 @@ extern "C" int nqs_ham_compile_text(int n_qubits, const char *text, nqs_ham_t **
                 auto put = [&](char letter, int j) -> bool {
                     if (j < 0 || j >= n_qubits) return false;
                     const uint64_t bit = 1ull << (j & 63);
-                    if ((t.f[j >> 6] | t.s[j >> 6]) & bit) return false;          // qubit named twice
+                    if (named[j >> 6] & bit) return false;                        // qubit named twice, in either order
+                    named[j >> 6] |= bit;
                     switch (letter) {
                         case 'I': return true;
                         case 'X': t.f[j >> 6] |= bit; return true;

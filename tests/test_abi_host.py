@@ -203,7 +203,13 @@ def test_text_loader_equals_operator_matrix_compile():
     assert (Ht.K, Ht.G) == (Hc.K, Hc.G)
     for k in a:
         assert a[k].tobytes() == b[k].tobytes(), k
-    for bad in ("0.5 XX", "0.5 X0 Y0", "(0.5+1j) X0", "abc X0", "0.5 Q1", "0.5 X99"):
+    for bad in ("0.5 XX", "0.5 X0 Y0", "(0.5+1j) X0", "abc X0", "0.5 Q1", "0.5 X99",
+                # the coefficient is a finite decimal literal: no hex ("0X1 Z2" must not read as 1.0 * Z2), nan, inf, overflow
+                "0X1 Z2", "0x1p3 Z2", "nan X0", "inf X0", "-inf X0", "1e400 X0", "0.5X0", ". X0",
+                # a qubit named twice is refused whichever factor comes first, identity included
+                "0.5 X0 I0", "0.5 I0 X0", "0.5 I3 I3"):
         with pytest.raises(nqs.NqsError):
             nqs.ham_compile_text(n, bad)
     assert nqs.ham_compile_text(n, "# nothing\n").K == 0
+    ok = nqs.ham_compile_text(n, "+1.5e-3 X0 I1 Z2\n-.25 Y4\n(2.E0-0.0j) [Z1]\n")
+    assert ok.K == 3 and abs(ok.sum_abs_coeff - (1.5e-3 + 0.25 + 2.0)) < 1e-15
