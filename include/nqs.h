@@ -247,7 +247,13 @@ int nqs_weighted_stats_static(const float *eloc_dev, const int64_t *counts_dev, 
  *   grad_out_dev device float [n_params], overwritten;
  *   baseline_out_host host double [2] = (Re b, Im b) or NULL; when non-NULL the call synchronises the stream.
  * fp32 on CUDA cores (the B sampled rows are ~1e-5 of the E_loc work), fixed reduction order: bit-reproducible.
- * B = 0 gives a zero gradient. */
+ * B = 0 gives a zero gradient.
+ * Preconditions the call cannot check without synchronising: the total count sum n is positive (0 gives NaN), and —
+ * when the handle carries a constraint — every sample satisfies Eq. 12 (the sampler produces only such rows; a
+ * violating row has psi = 0, its gradient is undefined and the value written for it is unspecified).
+ * global_stats_host[0] must be the true total over all replicas; <= 0 is NQS_EINVAL.  One row tile needs
+ * (2 npad + 3 hidden + 6) * 64 B of shared memory; that fits 227 KB for every shape nqs_made_create accepts
+ * (hidden <= 1024, n <= 128: 213 KB), and a shape that did not would get NQS_EUNSUPPORTED before anything is launched. */
 int nqs_made_num_params(const nqs_made_t *made, int64_t *n_params);
 int nqs_energy_grad(const nqs_made_t *made, const uint64_t *samples_dev, const int64_t *counts_dev,
                     const float *eloc_dev, int64_t B, int64_t minibatch, const double *global_stats_host,
@@ -267,10 +273,14 @@ int nqs_energy_grad(const nqs_made_t *made, const uint64_t *samples_dev, const i
  *     (max_unique = 0: no elimination);
  *   - n_up, n_down >= 0 switch on the Hamming-weight clamp of Eq. 14 (even qubits = up spins, odd = down, Eq. 12): at
  *     a position of spin s with c spin-s bits already set and m spin-s positions left, pi_hat(1) = 0 if c = n_s,
- *     = 1 if n_s - c = m, else the network's conditional.  n_up = n_down = -1: unconstrained.
+ *     = 1 if n_s - c = m, else the network's conditional.  n_up = n_down = -1: the constraint of the handle
+ *     (nqs_made_set_constraint), unconstrained if it has none.  A handle WITH a constraint only samples that
+ *     constraint (a different pair: NQS_EINVAL), so samples, log psi, E_loc and gradient share one pi_hat; on a handle
+ *     without one the pair clamps the sampler alone.
  * samples_out_dev : device uint64 [cap][2], counts_out_dev : device int64 [cap], cap = max_unique if 0 < max_unique <
  *   n_draws else n_draws; the first *n_unique_out_host rows are written, in buffer order (unique, bit j = qubit j).
- * Synchronous (n readbacks of the buffer size).  n_draws <= 2^30. */
+ * Synchronous (n readbacks of the buffer size); allocates and frees its buffers per call.  n_draws < 2^30
+ * (buffer indices are 32-bit; more: NQS_ERANGE). */
 int nqs_made_sample(const nqs_made_t *made, int64_t n_draws, uint64_t seed, int n_up, int n_down,
                     int64_t max_unique, uint64_t *samples_out_dev, int64_t *counts_out_dev,
                     int64_t *n_unique_out_host, void *cuda_stream);

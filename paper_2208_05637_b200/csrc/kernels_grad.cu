@@ -303,6 +303,9 @@ extern "C" int nqs_energy_grad(const nqs_made_t *M, const uint64_t *samples_dev,
     if (rc) return rc;
     if ((rc = grad_pack(M))) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
+    const size_t smem = sizeof(float) * ((size_t)(2 * M->npad + 3 * M->h + 4 + 2) * TR);
+    if (smem > 227 * 1024) return NQS_EUNSUPPORTED;                 // before anything is enqueued
+    if (global_stats_host && !(global_stats_host[0] > 0.0)) return NQS_EINVAL;
     int64_t np = 0;
     nqs_made_num_params(M, &np);
     if (cudaMemsetAsync(grad_out_dev, 0, sizeof(float) * (size_t)np, st) != cudaSuccess) return NQS_ECUDA;
@@ -331,14 +334,11 @@ extern "C" int nqs_energy_grad(const nqs_made_t *M, const uint64_t *samples_dev,
     ws.dO = (float *)w;
     double *d_stats = (double *)G->d_stats;
     if (global_stats_host) {          // data-parallel replicas: {sum n, sum n Re E, sum n Im E} over ALL ranks' samples
-        if (!(global_stats_host[0] > 0.0)) return NQS_EINVAL;
         if (cudaMemcpyAsync(d_stats, global_stats_host, 3 * sizeof(double), cudaMemcpyHostToDevice, st) != cudaSuccess) return NQS_ECUDA;
     } else {
         grad_stats_kernel<<<1, 256, 0, st>>>((const float2 *)eloc_dev, (const long long *)counts_dev, B, d_stats);
         ++g_launch_count;
     }
-    const size_t smem = sizeof(float) * ((size_t)(2 * npad + 3 * h + 4 + 2) * TR);
-    if (smem > 227 * 1024) return NQS_EUNSUPPORTED;
     if (cudaFuncSetAttribute(grad_rows_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem) != cudaSuccess) { cudaGetLastError(); return NQS_ECUDA; }
     int sms = 148, dev = 0;
     cudaGetDevice(&dev);

@@ -157,6 +157,13 @@ extern "C" int nqs_made_sample(const nqs_made_t *M, int64_t n_draws, uint64_t se
     if (n_draws > 0x7FFFFFFFll / 2) return NQS_ERANGE;            // buffer indices are 32-bit
     const int n = M->n;
     if ((n_up < 0) != (n_down < 0)) return NQS_EINVAL;
+    // One model, one distribution: when the handle carries a constraint (nqs_made_set_constraint) the samples must
+    // come from the same pi_hat that log psi, E_loc and the gradient use.  (-1, -1) takes the handle's; a different
+    // pair is a caller's mistake, not a request.
+    if (M->n_up >= 0) {
+        if (n_up < 0) { n_up = M->n_up; n_down = M->n_down; }
+        else if (n_up != M->n_up || n_down != M->n_down) return NQS_EINVAL;
+    }
     if (n_up >= 0) {                                              // Eq. 12: even qubits hold the up spins, odd qubits the down spins
         if (n_up > (n + 1) / 2 || n_down > n / 2) return NQS_EINVAL;
     }

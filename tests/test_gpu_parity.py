@@ -786,3 +786,23 @@ def test_constrained_local_energy_and_gradient_cfg2():
             # and it differs from the unconstrained gradient (the flag is really in effect)
             gun, _ = ograd.energy_gradient(params, samples, counts, e64)
             assert np.abs(gun - gref).max() > 1e-4 * np.abs(gref).max()
+
+
+def test_sampler_takes_the_constraint_of_the_handle():
+    """A handle with a constraint samples that constraint: (-1, -1) means the handle's pair, the same pair explicitly gives
+    the same buffer, a different pair is refused (include/nqs.h) — samples, log psi, E_loc and gradient share one pi_hat."""
+    p = wl.make_made_params(12, 32, 55)
+    M = nqs.made_create(p)
+    M.set_constraint(3, 2)
+    s0, c0 = nqs.made_sample(M, 3000, 11, device=DEV)
+    s1, c1 = nqs.made_sample(M, 3000, 11, 3, 2, device=DEV)
+    assert torch.equal(s0, s1) and torch.equal(c0, c1)
+    bits = wl.unpack_bits(s0.cpu().numpy().view(np.uint64), 12)
+    assert np.all(bits[:, 0::2].sum(axis=1) == 3) and np.all(bits[:, 1::2].sum(axis=1) == 2)
+    with pytest.raises(nqs.NqsError) as ei:
+        nqs.made_sample(M, 3000, 11, 2, 3, device=DEV)
+    assert ei.value.status == -1
+    M.set_constraint(-1, -1)                                   # no constraint on the handle: the pair clamps the sampler alone
+    s2, _ = nqs.made_sample(M, 3000, 11, 2, 3, device=DEV)
+    bits = wl.unpack_bits(s2.cpu().numpy().view(np.uint64), 12)
+    assert np.all(bits[:, 0::2].sum(axis=1) == 2) and np.all(bits[:, 1::2].sum(axis=1) == 3)
