@@ -228,7 +228,7 @@ def main():
     flush = torch.empty(256 * 1024 * 1024, dtype=torch.uint8, device=dev)      # > 126 MB L2
     stream = torch.cuda.current_stream()
 
-    from paper_2208_05637_b200.distributed import minibatch_of_step, max_over_ranks
+    from paper_2208_05637_b200.distributed import minibatch_of_step, max_over_ranks, all_reduce_stats
 
     def step(k):
         b = minibatch_of_step(k, rank, world, n_mb)
@@ -248,14 +248,21 @@ def main():
     launches0 = nqs.kernel_launch_count()
     ev = [(torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)) for _ in range(args.steps)]
     chain_ms, chain_launches = 0.0, 0
+    job_stats = torch.zeros(5, dtype=torch.float64, device=dev)
     for k in range(args.steps):
         flush.fill_(k & 0xFF)                                                   # L2 flush between timed iterations
         ev[k][0].record(stream)
-        step(args.warmup + k)
+        _, st_k = step(args.warmup + k)
         ev[k][1].record(stream)
         ms_k, nl = M.last_chain_kernel_ms()
         chain_ms += ms_k
         chain_launches += nl
+        st_k = torch.from_numpy(st_k).to(dev)
+        job_stats[:4] += st_k[:4]
+        job_stats[4] = torch.maximum(job_stats[4], st_k[4])
+    # the one exchange of the data-parallel design: the statistics of the mini-batches every rank
+    # processed, 4 sums + 1 max, once per accumulation round -- inside the barrier-bracketed region, outside the events
+    all_reduce_stats(job_stats)
     barrier()
     launches = nqs.kernel_launch_count() - launches0
     clocks = sampler.stop()
@@ -342,7 +349,10 @@ def main():
             "cpu_baseline": cpu_baseline, "cpu_baseline_1thread": cpu_baseline_1,
             "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": mb * 16 + mb * 8,
                     "d2h_bytes_per_step": mb * 8 + 5 * 8},
-            "gpu_launches": int(launches), "clocks": clocks}
+            "gpu_launches": int(launches), "clocks": clocks,
+            "job_stats": {"sum_n": job_stats[0].item(), "mean_E": [(job_stats[1] / job_stats[0]).item(), (job_stats[2] / job_stats[0]).item()],
+                          "note": "count-weighted mean of E_loc over every mini-batch of every rank in the timed steps "
+                                  "(all_reduce_stats: 4 sums + 1 max over ranks)"}}
     print(json.dumps(line))
     if world > 1:
         dist.destroy_process_group()
