@@ -64,6 +64,59 @@ def test_compile_bit_exact_workloads(cfg):
     _assert_same(Hp.export(), H.export())
 
 
+def _check_compiled_invariants(t, n, exact):
+    """SURVEY 8(c) pins of the compiled tensors that need no second implementation: CSR covers every term, flips strictly
+    ascending as 128-bit integers (word 1 major), ycount = popcount(flip & zy), and the group sizes of a JW chemistry
+    Hamiltonian: 1 + n + C(n,2) diagonal strings, 2(n-1) per same-spin two-flip, 4 per aabb four-flip, 6 per aaaa / bbbb
+    four-flip (exactly when nothing fell under the generator's 1e-8 drop, at most that otherwise)."""
+    from math import comb
+    flips, off, zy, yc = t["flips"], t["offsets"].astype(np.int64), t["zy"], t["ycount"]
+    K, G, N = zy.shape[0], flips.shape[0], n // 2
+    assert off[0] == 0 and off[-1] == K and np.all(np.diff(off) > 0)
+    hi, lo = flips[:, 1], flips[:, 0]
+    assert np.all((hi[1:] > hi[:-1]) | ((hi[1:] == hi[:-1]) & (lo[1:] > lo[:-1])))
+    grp = np.repeat(np.arange(G), np.diff(off))
+    pc = lambda a: np.bitwise_count(a).astype(np.int64)
+    assert np.array_equal(pc(flips[grp, 0] & zy[:, 0]) + pc(flips[grp, 1] & zy[:, 1]), yc.astype(np.int64))
+    # within a group the sign masks ascend strictly (rule 4; equal masks were merged by rule 2)
+    same = grp[1:] == grp[:-1]
+    zhi, zlo = zy[:, 1], zy[:, 0]
+    assert np.all(~same | (zhi[1:] > zhi[:-1]) | ((zhi[1:] == zhi[:-1]) & (zlo[1:] > zlo[:-1])))
+    nflip = pc(flips[:, 0]) + pc(flips[:, 1])
+    sizes = np.diff(off)
+    assert set(np.unique(nflip)) <= {0, 2, 4} and np.all(yc % 2 == 0)          # real integrals: even Y counts
+    even = np.uint64(0x5555555555555555)
+    n_even = pc(flips[:, 0] & even) + pc(flips[:, 1] & even)                   # flipped alpha (even) spin-orbitals
+    cap = np.where(nflip == 0, 1 + n + comb(n, 2), np.where(nflip == 2, 2 * (n - 1), np.where(n_even == 2, 4, 6)))
+    assert np.all(sizes <= cap)
+    assert np.all((nflip != 2) | (n_even != 1)) and np.all((nflip != 4) | (n_even % 2 == 0))   # S_z is conserved
+    if exact:
+        assert np.array_equal(sizes, cap)
+        assert G == 1 + 2 * comb(N, 2) + comb(N, 2) ** 2 + 2 * comb(N, 4)
+        assert K == 1 + n + comb(n, 2) + 4 * (n - 1) * comb(N, 2) + 4 * comb(N, 2) ** 2 + 12 * comb(N, 4)
+    else:
+        assert G <= 1 + 2 * comb(N, 2) + comb(N, 2) ** 2 + 2 * comb(N, 4)
+
+
+@pytest.mark.parametrize("cfg", [3, pytest.param(4, marks=pytest.mark.slow), pytest.param(5, marks=pytest.mark.slow)])
+def test_compile_bit_exact_at_the_benchmarked_sizes(cfg):
+    """north_star: "grouped tensors and flip masks must match bit-exactly" -- at the sizes that are benchmarked, not only
+    cfg 1-2: 73,126 terms (cfg 3), ~0.67 M (cfg 4), ~2.8 M (cfg 5, the bench workload; about 100 s here, most of it
+    the dict-based oracle).  PAPER.md:154-156, Fig. 1 (:101)."""
+    w = wl.WORKLOADS[cfg]
+    h, g = wl.make_integrals(w.n_spatial, w.seed_integrals)
+    x, z, c = wl.jw_pauli_terms(h, g)
+    H = nqs.ham_compile_packed(w.n_qubits, x, z, c)
+    t = H.export()
+    ora = ocomp.compile_hamiltonian(wl.masks_to_codes(x, z, w.n_qubits), c)
+    _assert_same(t, ora)
+    assert (H.K, H.G) == (ora["zy"].shape[0], ora["flips"].shape[0])
+    assert abs(H.sum_abs_coeff - ora["sum_abs_coeff"]) <= 1e-12 * ora["sum_abs_coeff"]
+    _check_compiled_invariants(t, w.n_qubits, exact=(cfg == 3))
+    if cfg == 3:
+        assert (H.K, H.G) == (73126, 13966)                                 # closed forms K(15), G(15), SURVEY 8
+
+
 def test_compile_edge_cases_and_errors():
     L = nqs.lib()
     out = ctypes.c_void_p()
