@@ -105,23 +105,8 @@ struct TcParams {
     long long g_begin;                   // first group that needs a forward pass (1 if group 0 is f = 0)
     int n_up, n_down;                    // Hamming-weight constraint (Eq. 14), n_up < 0 = off
     unsigned long long spin_lo, spin_hi; // bit d = 1: position d is a down spin
-#ifdef TC_PROF
-    long long *prof;                     // [grid][32] cycle counters (instrumented build only)
-    int test_mode;                       // 1: issuer waits for the weight ring only; 2: for nothing (timing probes, results are garbage)
-#endif
 };
 
-#ifdef TC_PROF
-#define PROF_T0() const long long _t0 = clock64()
-#define PROF_ADD(v) (v) += clock64() - _t0
-#define PROF_SITE(x) pw_site = (x)
-#define TESTMODE (p.test_mode)
-#else
-#define PROF_SITE(x) do {} while (0)
-#define TESTMODE 0
-#define PROF_T0() do {} while (0)
-#define PROF_ADD(v) do {} while (0)
-#endif
 
 __device__ __forceinline__ unsigned long long shr128(ulonglong2 a, int s) {      // low 64 bits of a >> s, 0 <= s < 128
     if (s == 0) return a.x;
@@ -218,21 +203,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             const long long total = ntl * (long long)p.nfills;
             const uint8_t *img = p.wimg + (size_t)rank * p.img_stride;
             uint32_t e = (uint32_t)lane % (uint32_t)p.nfills, slot = (uint32_t)lane, par = 1u;   // a fresh barrier passes a parity-1 wait
-            long long pp_wait = 0; (void)pp_wait;
             for (long long q = lane; q < total; q += nprod) {
                 const uint2 pe = __ldg(&p.fills[e]);
-                { PROF_T0(); mbar_wait(&bars[BAR_WEMPTY + slot], par); PROF_ADD(pp_wait); }
-                if (TESTMODE & 128) mbar_arrive_addr(BAR_ADDR(BAR_WFULL + slot));        // probe: no weight traffic at all
-                else {
+                mbar_wait(&bars[BAR_WEMPTY + slot], par);
                 mbar_arrive_expect_tx(&bars[BAR_WFULL + slot], pe.y);
                 bulk_g2s(smem + SL.slots + slot * p.slot_bytes, img + pe.x, pe.y, &bars[BAR_WFULL + slot]);
-                }
                 e += nprod; while (e >= (uint32_t)p.nfills) e -= (uint32_t)p.nfills;
                 slot += nprod; while (slot >= (uint32_t)p.nslots) { slot -= (uint32_t)p.nslots; par ^= 1u; }
             }
-#ifdef TC_PROF
-            if (p.prof && lane == 0) p.prof[(size_t)blockIdx.x * 32 + 21] = pp_wait;
-#endif
         }
     } else if (warp == W_ISSUE && rank != 0) {
         // =========================== peer CTA: ring forwarder ===========================
@@ -241,15 +219,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
         if (elect_one()) {
             const long long total = ntl * (long long)p.nfills;
             uint32_t slot = 0, par = 0;
-            long long pf_wait = 0; (void)pf_wait;
             for (long long q = 0; q < total; ++q) {
-                { PROF_T0(); mbar_wait(&bars[BAR_WFULL + slot], par); PROF_ADD(pf_wait); }
+                mbar_wait(&bars[BAR_WFULL + slot], par);
                 mbar_arrive_cluster(BAR_ADDR(BAR_WFULL + slot), 0);
                 if (++slot == (uint32_t)p.nslots) { slot = 0; par ^= 1u; }
             }
-#ifdef TC_PROF
-            if (p.prof) p.prof[(size_t)blockIdx.x * 32 + 22] = pf_wait;
-#endif
         }
         __syncwarp();
     } else if (warp == W_ISSUE) {
@@ -271,12 +245,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             const uint32_t tm_d3 = tmem + p.tm_d3, tm_ph = tm_d3 + (uint32_t)KO - 16, tm_a0 = tmem + p.tm_a0;
             uint32_t slot = 0, wpar = 0, slot_lo = slots_lo;
             uint32_t ph = 0;                             // parity of the next phase to wait for, one bit per barrier id
-#ifdef TC_PROF
-            long long pw_wait = 0, pw_wf = 0, pw_tot = clock64(), pw_cls[4] = {0, 0, 0, 0};
-            int pw_site = 0;                             // 0 = A0FULL, 1 = prewait (accumulator / A1 chunk), 2 = consumer EDONE, 3 = D3EMPTY
-#endif
-#define WAIT(id) do { PROF_T0(); if (!(TESTMODE & 3)) mbar_spin(BAR_ADDR(id), (ph >> (id)) & 1u); ph ^= 1u << (id); tc_fence_after(); PROF_ADD(pw_wait); PROF_ADD(pw_cls[pw_site]); } while (0)
-#define SLOT_ACQUIRE(w) do { if ((w) & SUB_NEW) { PROF_T0(); if ((TESTMODE & 3) < 2) mbar_spin(BAR_ADDR(BAR_WFULL + slot), wpar); tc_fence_after(); PROF_ADD(pw_wf); } } while (0)
+#define WAIT(id) do { mbar_spin(BAR_ADDR(id), (ph >> (id)) & 1u); ph ^= 1u << (id); tc_fence_after(); } while (0)
+#define SLOT_ACQUIRE(w) do { if ((w) & SUB_NEW) { mbar_spin(BAR_ADDR(BAR_WFULL + slot), wpar); tc_fence_after(); } } while (0)
 #define SLOT_RELEASE(w) do { if ((w) & SUB_END) { mma_commit_cg2(BAR_ADDR(BAR_WEMPTY + slot)); slot_lo += slot_step; \
                              if (++slot == nslots) { slot = 0; wpar ^= 1u; slot_lo = slots_lo; } } } while (0)
             for (long long ti = 0; ti < ntl; ++ti) {
@@ -285,7 +255,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                 uint32_t si = 0;
                 asm volatile("" : "+r"(si));
                 uint32_t w = p.sub[si];                      // current table word; the next one is always loaded one step ahead
-                PROF_SITE(0); WAIT(BAR_A0FULL);
+                WAIT(BAR_A0FULL);
                 // consumer of tile-local op jc (jc is a compile-time constant after unrolling)
                 auto consume = [&](const int jc) {
                     const int type = S::type(jc);
@@ -297,12 +267,12 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                     // [32 pc + 16, 32 pc + 32) of every 32-column piece; D3 += Ahi.Bhi + Alo.Bhi + Ahi.Blo
                     if (type == T_P) {                                          // resident P2 tile of this chunk, N = 16
                         const uint32_t b_lo = (res_lo + (uint32_t)S::chunk(jc) * ((SPLIT ? 4096u : 2048u) >> 4)) | lo_sw128;
-                        PROF_SITE(2); WAIT(BAR_EDONE + jc % NACC);
-                        if (jc == S::FIRST_INPLACE) { PROF_SITE(3); WAIT(BAR_D3EMPTY); }          // first write into D3 of this tile
+                        WAIT(BAR_EDONE + jc % NACC);
+                        if (jc == S::FIRST_INPLACE) { WAIT(BAR_D3EMPTY); }          // first write into D3 of this tile
 #pragma unroll
                         for (uint32_t ks = 0; ks < 8; ++ks) {
                             const uint32_t a_k = a_t + 32 * (ks >> 1) + 8 * (ks & 1), b_k = b_lo + (ks >> 2) * (1024u >> 4) + 2 * (ks & 3);
-                            if (!(TESTMODE & 8)) mma_ts_cg2(tm_ph, a_k, b_k, hi_sw128, id16, 1u);
+                            mma_ts_cg2(tm_ph, a_k, b_k, hi_sw128, id16, 1u);
                             if (SPLIT) {
                                 mma_ts_cg2(tm_ph, a_k + 16, b_k, hi_sw128, id16, 1u);
                                 mma_ts_cg2(tm_ph, a_k, b_k + (2048u >> 4), hi_sw128, id16, 1u);
@@ -314,8 +284,8 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                         const uint32_t N = (uint32_t)KO - nlo, kb_step = (N >> 1) * (128u >> 4);
                         const uint32_t b_lo = (slot_lo + (w & SUB_OFF_MASK)) | lo_sw128, idesc = id0 | ((N >> 3) << 17);
                         SLOT_ACQUIRE(w);
-                        PROF_SITE(2); WAIT(BAR_EDONE + jc % NACC);
-                        if (jc == S::FIRST_INPLACE) { PROF_SITE(3); WAIT(BAR_D3EMPTY); }          // first write into D3 of this tile
+                        WAIT(BAR_EDONE + jc % NACC);
+                        if (jc == S::FIRST_INPLACE) { WAIT(BAR_D3EMPTY); }          // first write into D3 of this tile
 #pragma unroll
                         for (uint32_t ks = 0; ks < 8; ++ks) {
                             const uint32_t a_k = a_t + 32 * (ks >> 1) + 8 * (ks & 1), b_k = b_lo + (ks >> 2) * kb_step + 2 * (ks & 3);
@@ -335,7 +305,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                     uint32_t jj = (uint32_t)j;
                     asm volatile("" : "+r"(jj));
                     const uint32_t pw = p.prewait[jj];      // pending chunk epilogues this op depends on (accumulator reuse, A1 chunks)
-                    PROF_SITE(1);
                     if (pw & 1u) WAIT(BAR_EDONE + 0);
                     if (NACC > 1 && (pw & 2u)) WAIT(BAR_EDONE + 1);
                     if (NACC > 2 && (pw & 4u)) WAIT(BAR_EDONE + 2);
@@ -345,7 +314,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                         {   // D = [1 1 x'..] . [b2_hi b2_lo 0..]^T: the bias, and the overwrite of the accumulator
                             const uint32_t wn = p.sub[++si];
                             SLOT_ACQUIRE(w);
-                            if (!(TESTMODE & 4)) mma_ts_cg2(d, tm_a0, (slot_lo + (w & SUB_OFF_MASK)) | lo_noswz, hi_noswz16, id128, 0u);
+                            mma_ts_cg2(d, tm_a0, (slot_lo + (w & SUB_OFF_MASK)) | lo_noswz, hi_noswz16, id128, 0u);
                             SLOT_RELEASE(w);
                             w = wn;
                         }
@@ -405,9 +374,6 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                 for (int m = S::LAG; m >= 1; --m) consume(S::NOPS - m);                       // consumers of the last ops
                 mma_commit_cg2(BAR_ADDR(BAR_D3FULL));
             }
-#ifdef TC_PROF
-            if (p.prof) { long long *pr = p.prof + (size_t)blockIdx.x * 32; pr[0] = clock64() - pw_tot; pr[1] = pw_wait; pr[3] = pw_wf; pr[5] = ntl; pr[28] = pw_cls[0]; pr[29] = pw_cls[1]; pr[30] = pw_cls[2]; pr[31] = pw_cls[3]; }
-#endif
 #undef WAIT
 #undef SLOT_ACQUIRE
 #undef SLOT_RELEASE
@@ -423,33 +389,25 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
         const uint32_t lane_base = (uint32_t)((warp & 3) * 32) << 16;     // TMEM lane quadrant of this warp
         const uint32_t a1_row = smem_base + SL.a1 + (row >> 3) * 1024u + (row & 7u) * 128u, sw = row & 7u;
         uint32_t fb = 0;                                   // bit a: parity of accumulator a's first FULL phase of this tile
-        long long pe_wait = 0, pe_a1 = 0, pe_tot = clock64(), pe_fence = 0, pe_arr = 0, pe_ld = 0, pe_ldi = 0, pe_cvt = 0;
-        (void)pe_wait; (void)pe_a1; (void)pe_tot; (void)pe_fence; (void)pe_arr; (void)pe_ld; (void)pe_ldi; (void)pe_cvt;
-        if (!(TESTMODE & 3))
         for (long long ti = 0; ti < ntl; ++ti, fb ^= p.cntmask) {
         bool a1_waited = false;
         uint32_t acc = 0, q = 0;                           // j % NACC, j / NACC
         for (uint32_t j = 0; j < nops; ++j) {
             const uint32_t type = p.optype[j], c = p.opchunk[j];
-            { PROF_T0(); mbar_wait(&bars[BAR_FULL + acc], ((fb >> acc) ^ q) & 1u); PROF_ADD(pe_wait); }
+            mbar_wait(&bars[BAR_FULL + acc], ((fb >> acc) ^ q) & 1u);
             tc_fence_after();
             // before the first write into A1: the previous tile's layer-2 MMAs have read it
             if (L == 2 && ti > 0 && type == T_L1S && !a1_waited) {
-                PROF_T0(); mbar_wait(&bars[BAR_A1FREE], (uint32_t)(ti - 1) & 1u); PROF_ADD(pe_a1);
+                mbar_wait(&bars[BAR_A1FREE], (uint32_t)(ti - 1) & 1u);
                 a1_waited = true;
             }
             const uint32_t d_addr = tmem + lane_base + acc * CN + 64u * grp;
             uint32_t va[32], vb[32];
-            { PROF_T0();
             tmem_ld32p(d_addr, va);
             tmem_ld32p(d_addr + 32, vb);
-            PROF_ADD(pe_ldi); }
-            { PROF_T0(); tmem_wait_ld(); PROF_ADD(pe_ld); }
-#ifdef TC_PROF
-            const long long _tc0 = clock64();
-#endif
+            tmem_wait_ld();
 #pragma unroll
-            for (int pp = 0; pp < ((TESTMODE & 64) ? 0 : 2); ++pp) {     // probe bit 64: no conversion, no store
+            for (int pp = 0; pp < 2; ++pp) {
                 const uint32_t *v = pp ? vb : va;
                 uint32_t w[16], wl[16];                        // the bias is already in the accumulator (constant input columns)
 #pragma unroll
@@ -475,22 +433,14 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                     if (SPLIT) tmem_st16p(d_addr + 32 * pp + 16, wl);
                 }
             }
-#ifdef TC_PROF
-            pe_cvt += clock64() - _tc0;
-#endif
-            { PROF_T0();
             if (type == T_L1S) fence_proxy_async(); else tmem_wait_st();
             tc_fence_before();
-            __syncwarp(); PROF_ADD(pe_fence); }
-            { PROF_T0();
+            __syncwarp();
             if (lane == 0) mbar_arrive_leader(BAR_ADDR(BAR_EDONE + acc), rank);
-            __syncwarp(); PROF_ADD(pe_arr); }
+            __syncwarp();
             if (++acc == (uint32_t)NACC) { acc = 0; ++q; }
         }
         }
-#ifdef TC_PROF
-        if (p.prof && lane == 0 && (warp & 3) == 0) { long long *pr = p.prof + (size_t)blockIdx.x * 32 + (grp == 0 ? 6 : 11); pr[0] = clock64() - pe_tot; pr[1] = pe_wait; pr[2] = pe_ld; pr[3] = pe_fence; pr[4] = pe_arr; long long *pa = p.prof + (size_t)blockIdx.x * 32 + (grp == 0 ? 23 : 25); pa[0] = pe_ldi; pa[1] = pe_cvt; }
-#endif
     } else {
         // =========================== tile warps: A0 of the next tile, contraction, final epilogue ===========================
         const int q = warp & 3;
@@ -552,9 +502,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
         };
         float2 E = make_float2(0.f, 0.f);
         float mr = (p.mode == 1 && p.hm.has_diag) ? 1.0f : 0.0f;     // the f = 0 group has ratio exactly 1
-        long long pt_a0 = 0, pt_d3 = 0, pt_tot = clock64(), pt_s = 0, pt_fin = 0;
-        (void)pt_a0; (void)pt_d3; (void)pt_tot; (void)pt_s; (void)pt_fin;
-        if (ntl > 0 && !(TESTMODE & 3)) {
+        if (ntl > 0) {
             const long long t = 2 * q_lo + rank;
             const bool valid = t < ntiles;
             load_row(t / Gnd, valid, cur);
@@ -563,7 +511,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             clamp_of(zp, fm, inval);
             build_a0(zp);
         }
-        for (long long ti = 0; ti < ((TESTMODE & 3) ? 0 : ntl); ++ti) {
+        for (long long ti = 0; ti < ntl; ++ti) {
             const long long t = 2 * (q_lo + ti) + rank;
             const bool valid = t < ntiles;
             const long long g = p.g_begin + (t % Gnd);
@@ -579,10 +527,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             }
             // ---- (a3) S = sum_{t in g} c_t (-i)^{r_t} (-1)^{popcount(x & s_t)}: independent of the MMAs, done while they run ----
             float2 S = make_float2(0.f, 0.f);
-#ifdef TC_PROF
-            const long long _ts = clock64();
-#endif
-            if (p.mode == 1 && valid && cur.i < p.B && !(TESTMODE & 32)) {
+            if (p.mode == 1 && valid && cur.i < p.B) {
                 const uint32_t t1 = __ldg(&p.hm.offsets[g + 1]);
                 for (uint32_t tt = __ldg(&p.hm.offsets[g]); tt < t1; ++tt) {
                     const ulonglong2 zy = __ldg(&p.hm.zy[tt]);
@@ -592,21 +537,15 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                     S.y += cs.y;
                 }
             }
-#ifdef TC_PROF
-            pt_s += (long long)__float_as_int(S.x) * 0 + clock64() - _ts;
-#endif
             // ---- operand tile of the NEXT tile, once the last MMA that reads the current one has completed ----
             if (has_next) {
-                { PROF_T0(); mbar_wait(&bars[BAR_A0FREE], (uint32_t)ti & 1u); PROF_ADD(pt_a0); }
+                mbar_wait(&bars[BAR_A0FREE], (uint32_t)ti & 1u);
                 tc_fence_after();
                 build_a0(zp_n);
             }
             // ---- final epilogue: log|psi| = 1/2 sum_d log sigmoid(+-a_d), phi = o[2 z_{n-2} + z_{n-1}] ----
-            { PROF_T0(); mbar_wait(&bars[BAR_D3FULL], (uint32_t)ti & 1u); PROF_ADD(pt_d3); }
+            mbar_wait(&bars[BAR_D3FULL], (uint32_t)ti & 1u);
             tc_fence_after();
-#ifdef TC_PROF
-            const long long _tf = clock64();
-#endif
             // sum_d log sigmoid(t_d) = sum_d min(t_d, 0) - ln prod_d (1 + exp(-|t_d|)): every factor is in (1, 2], so a
             // 16-term product cannot overflow and costs one LG2 per 16 conditionals; the 16 chains are independent (ILP).
             float msum = 0.0f, lg = 0.0f, phi = 0.0f;
@@ -626,7 +565,7 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                 const float4 *bp = reinterpret_cast<const float4 *>(s_b3 + c0);
                 float prod0 = 1.0f, prod1 = 1.0f, m0 = 0.0f, m1 = 0.0f;
 #pragma unroll
-                for (int k4 = 0; k4 < ((TESTMODE & 16) ? 0 : 4); ++k4) {
+                for (int k4 = 0; k4 < 4; ++k4) {
                     const float4 bb = bp[k4];
                     const float bk[4] = {bb.x, bb.y, bb.z, bb.w};
 #pragma unroll
@@ -668,15 +607,9 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
                 }
                 E = make_float2(0.f, 0.f);
             }
-#ifdef TC_PROF
-            pt_fin += clock64() - _tf;
-#endif
             cur = nxt; zp = zp_n; fm = fm_n; inval = inval_n;
         }
         if (p.mode == 1) atomicMax(p.max_ratio_bits, __float_as_uint(mr));
-#ifdef TC_PROF
-        if (p.prof && lane == 0 && warp == 0) { long long *pr = p.prof + (size_t)blockIdx.x * 32 + 16; pr[0] = clock64() - pt_tot; pr[1] = pt_a0; pr[2] = pt_d3; pr[3] = pt_s; pr[4] = pt_fin; }
-#endif
     }
 #undef BAR_ADDR
     tc_fence_before();
@@ -768,10 +701,6 @@ static bool tc_shape(const nqs_made *M, TcShape *out) {
     uint32_t slot = (ring / ns) / 1024 * 1024;
     if (slot < need) return false;
     if (slot > 0x1FFFu * 16u) slot = 0x1FFFu * 16u / 1024 * 1024;
-#ifdef TC_PROF
-    if (const char *e = getenv("NQS_TC_SLOT_KB")) { slot = (uint32_t)atoi(e) * 1024; }
-    if (const char *e = getenv("NQS_TC_NSLOTS")) { ns = atoi(e); }
-#endif
     s.slot = slot; s.nslots = ns;
     *out = s;
     return true;
@@ -1074,9 +1003,6 @@ static void fill_common(const nqs_made *M, TcParams &p) {
     p.resimg = (const uint8_t *)P->d_res; p.res_bytes = P->res_bytes;
     p.slot_bytes = P->slot_bytes; p.nslots = P->nslots;
     p.nprod = P->nslots < NPROD ? P->nslots : NPROD;
-#ifdef TC_PROF
-    if (const char *e = getenv("NQS_TC_NPROD")) { p.nprod = atoi(e); if (p.nprod > p.nslots) p.nprod = p.nslots; }
-#endif
     p.bias = (const float *)P->d_bias;
     p.n_up = M->dev.n_up; p.n_down = M->dev.n_down; p.spin_lo = M->dev.spin_lo; p.spin_hi = M->dev.spin_hi;
 }
@@ -1096,10 +1022,6 @@ static int permuted(const nqs_made *M, const ulonglong2 *in, long long N, ulongl
     return cudaGetLastError() == cudaSuccess ? NQS_OK : NQS_ECUDA;
 }
 
-#ifdef TC_PROF
-long long *g_tc_prof = nullptr;   // [148][16], set by the profiling harness through nqs_tc_prof_buffer()
-extern "C" void nqs_tc_prof_buffer(long long *dev_buf) { g_tc_prof = dev_buf; }
-#endif
 
 template <int NC, int L, int NACC, bool SPLIT, bool SEQ>
 static int launch_inst(const TcParams &p, int grid, uint32_t smem_bytes, cudaStream_t st) {
@@ -1117,10 +1039,6 @@ static int launch_inst(const TcParams &p, int grid, uint32_t smem_bytes, cudaStr
 }
 
 static int launch_chain(const TcPack *P, TcParams &p, long long ntiles, cudaStream_t st) {
-#ifdef TC_PROF
-    p.prof = g_tc_prof;
-    p.test_mode = getenv("NQS_TC_TESTMODE") ? atoi(getenv("NQS_TC_TESTMODE")) : 0;
-#endif
     const long long npairs = (ntiles + 1) / 2;
     const long long ncl_max = P->sms / 2;
     const int grid = 2 * (int)(npairs < ncl_max ? npairs : ncl_max);

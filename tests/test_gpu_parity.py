@@ -342,10 +342,12 @@ def test_empty_hamiltonian():
 # ---- the tensor-core path in the launch configuration bench.py times: many sample blocks per launch ---------
 def _spread_rows(B, n_oracle, seed):
     """Oracle rows spread over the 128-row sample blocks of a launch: first block, last (ragged) block, and
-    the rest drawn from distinct blocks in between."""
+    the rest drawn from distinct blocks in between; with more rows than blocks, further rounds over the blocks."""
     nsb = (B + 127) // 128
     rng = np.random.default_rng(seed)
     blocks = [0, nsb - 1] + list(rng.permutation(np.arange(1, max(nsb - 1, 1)))[: max(n_oracle - 2, 0)])
+    while len(blocks) < n_oracle:
+        blocks += list(rng.permutation(nsb))
     rows = []
     for k, sb in enumerate(blocks[:n_oracle]):
         lo, hi = sb * 128, min(B, sb * 128 + 128)
@@ -357,8 +359,8 @@ def _check_eloc_tc_blocks(cfg, B, n_oracle, minibatch):
     w, (x, z, c), params, H, M = workload(cfg)
     assert M.resolved_path(nqs.PATH_TC) == nqs.PATH_TC
     samples, counts = wl.make_samples(w.n_spatial, w.n_alpha, w.n_beta, B, w.max_count, w.seed_samples, w.unique)
-    pick = _spread_rows(min(B, minibatch) if minibatch else B, n_oracle, cfg)
-    if minibatch and minibatch < B:                      # also rows of the second mini-batch
+    pick = _spread_rows(B, n_oracle, cfg)
+    if minibatch and minibatch < B:                      # also the first and last row of the second mini-batch
         pick = np.unique(np.concatenate([pick, [minibatch, B - 1]]))
     ref = oeloc.local_energy(wl.masks_to_codes(x, z, w.n_qubits), c, params, samples[pick], memo=True)
     e, stats = nqs.local_energy(H, M, _dev_u64(samples), torch.from_numpy(counts).to(DEV), minibatch=minibatch,
@@ -381,16 +383,61 @@ def test_eloc_cfg5_tc_many_sample_blocks_ragged():
     _check_eloc_tc_blocks(5, 1101, 8, 8192)
 
 
+def _all_rows_vs_fp32_path(H, M, samples, rows, ec_tc, tag):
+    """Every row in `rows` of a tensor-core launch against the fp32 CUDA-core path run on exactly those samples (the
+    fp32 path is itself within ~0.04 x the bound of the oracle and costs ~30 x the tensor-core time per row): the
+    GPU-side reference that reaches rows the oracle cannot.  Asserted at 1 x the north_star bound."""
+    tol = 1e-5 * H.sum_abs_coeff
+    e_si, _ = nqs.local_energy(H, M, _dev_u64(samples[rows]), None, path=nqs.PATH_SIMT)
+    e_si = e_si.cpu().numpy().astype(np.float64)
+    d = np.abs(ec_tc[rows] - (e_si[:, 0] + 1j * e_si[:, 1]))
+    print(f"[parity] {tag}: max|TC - fp32 path|/tol = {d.max() / tol:.4f} (mean {d.mean() / tol:.4f}) over all {len(rows)} rows compared")
+    assert d.max() <= tol, (tag, d.max() / tol)
+
+
 def test_eloc_cfg5_literal_bench_call():
-    """The call bench.py times: 8,192 cfg-5 samples, minibatch = 8192, NQS_PATH_AUTO -> tensor cores; 4 oracle
-    rows from blocks spread over the 64 sample blocks."""
+    """The call bench.py times: 8,192 cfg-5 samples, minibatch = 8192, NQS_PATH_AUTO -> tensor cores.  32 oracle rows
+    from 32 distinct sample blocks, and every row of 8 whole sample blocks spread over the 64 plus 77 more
+    rows (1,101 in all) against the fp32 path."""
     w, (x, z, c), params, H, M = workload(5)
     assert M.resolved_path(nqs.PATH_AUTO) == nqs.PATH_TC
-    _check_eloc_tc_blocks(5, 8192, 4, 8192)
+    ec, samples, counts = _check_eloc_tc_blocks(5, 8192, 32, 8192)
+    rows = np.concatenate([np.arange(sb * 128, sb * 128 + 128) for sb in (0, 9, 18, 27, 36, 45, 54, 63)] + [np.arange(4000, 4077)])
+    _all_rows_vs_fp32_path(H, M, samples, rows, ec, "cfg 5 bench launch (B = 8192)")
+
+
+def test_eloc_cfg5_two_full_minibatches_in_one_call():
+    """Row a7 at the configured slice size: ONE nqs_local_energy call over 16,384 cfg-5 samples with
+    minibatch = 8192 = two full gradient-accumulation slices.  The second slice must equal a direct call on those rows
+    (same kernel, so only the order of the float atomics differs), the statistics must be those of all 16,384 rows, and two
+    rows of the second slice are checked against the oracle."""
+    w, (x, z, c), params, H, M = workload(5)
+    B = 16384
+    samples, counts = wl.make_samples(w.n_spatial, w.n_alpha, w.n_beta, B, w.max_count, w.seed_samples, w.unique)
+    xs, cn = _dev_u64(samples), torch.from_numpy(counts).to(DEV)
+    e, st = nqs.local_energy(H, M, xs, cn, minibatch=8192)
+    e2, st2 = nqs.local_energy(H, M, xs[8192:].contiguous(), cn[8192:].contiguous(), minibatch=8192)
+    tol = 1e-5 * H.sum_abs_coeff
+    d = (e[8192:] - e2).cpu().numpy().astype(np.float64)
+    en = e.cpu().numpy().astype(np.float64)
+    ec = en[:, 0] + 1j * en[:, 1]
+    pick = np.array([8192, 16383])
+    ref = oeloc.local_energy(wl.masks_to_codes(x, z, w.n_qubits), c, params, samples[pick], memo=True)
+    err = np.abs(ec[pick] - ref).max()
+    print(f"[parity] cfg 5, B = 16384 as 2 x 8192 in one call: second slice vs direct call max|d|/tol = "
+          f"{np.hypot(d[:, 0], d[:, 1]).max() / tol:.5f}; max|dE_loc|/tol = {err / tol:.4f} over oracle rows {pick.tolist()}")
+    assert np.hypot(d[:, 0], d[:, 1]).max() <= 0.01 * tol
+    assert err <= tol
+    np.testing.assert_allclose(st[:4], oeloc.weighted_stats(ec, counts)[:4], rtol=1e-9)
+    assert st[0] == counts.sum() and st[4] >= st2[4] >= 1.0
 
 
 def test_eloc_cfg4_tc_many_sample_blocks_two_minibatches():
-    _check_eloc_tc_blocks(4, 1024 + 333, 16, 1024)       # 8 blocks, then a second mini-batch of 333 (3 blocks, ragged)
+    """cfg 4: 8 blocks, then a second mini-batch of 333 (3 blocks, ragged); 64 oracle rows and every one of
+    the 1,357 rows against the fp32 path."""
+    w, (x, z, c), params, H, M = workload(4)
+    ec, samples, counts = _check_eloc_tc_blocks(4, 1024 + 333, 64, 1024)
+    _all_rows_vs_fp32_path(H, M, samples, np.arange(1024 + 333), ec, "cfg 4 (B = 1357, minibatch 1024)")
 
 
 def test_eloc_cfg3_tc_vs_simt_all_rows_and_oracle():
