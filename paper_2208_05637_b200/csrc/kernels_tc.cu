@@ -22,6 +22,7 @@
 // leader when the peer's half of a ring slot has landed; 4-7 / 8-11 = two chunk-epilogue groups, each serving one
 // 64-column half of every op; 0-3 = tile warps (A0 of the NEXT tile, contraction, final epilogue).  DESIGN.md 6-7.
 // PAPER.md:122-134 (Alg. 1), :84-96 (architecture, Eq. 8-10), :152-158 (Eq. 15-16).
+#include <algorithm>
 #include <cstdlib>
 #include <cstring>
 #include <new>
@@ -100,7 +101,8 @@ struct TcParams {
     const ulonglong2 *x;                 // [B] samples in qubit order (contraction parity)
     HamDev hm;
     const float2 *base;                  // [B] (log|psi|, phi) of the samples
-    float *eloc;                         // [B][2], pre-initialised with the f = 0 group; atomically accumulated
+    float2 *epart;                       // [nsb][eslots][TILE_M] per-CTA partial sums of E (slot = 2 * (cluster - first cluster of the block) + rank)
+    int eslots;                          // slots per sample block (host: 2 * the largest number of clusters that share a block)
     unsigned *max_ratio_bits;
     long long g_begin;                   // first group that needs a forward pass (1 if group 0 is f = 0)
     int n_up, n_down;                    // Hamming-weight constraint (Eq. 14), n_up < 0 = off
@@ -602,8 +604,11 @@ __global__ void __cluster_dims__(2, 1, 1) __launch_bounds__(NTHREADS, 1) eloc_tc
             }
             if (!has_next || nxt.sb != cur.sb || nxt.i != cur.i) {
                 if (p.mode == 1 && cur.i < p.B) {
-                    atomicAdd(&p.eloc[2 * cur.i], E.x);
-                    atomicAdd(&p.eloc[2 * cur.i + 1], E.y);
+                    // One slot per (sample block, CTA): every row's partial is WRITTEN once and eloc_finish_kernel adds
+                    // the slots in order, so E_loc does not depend on how the CTAs were scheduled (no float atomics).
+                    // The clusters that share block sb are consecutive; the first is the one holding tile pair sb*Gnd/2.
+                    const long long k_first = ((((cur.sb * Gnd) >> 1) + 1) * ncl - 1) / npairs;
+                    p.epart[((size_t)cur.sb * p.eslots + 2 * (size_t)(cl - k_first) + rank) * TILE_M + row] = E;
                 }
                 E = make_float2(0.f, 0.f);
             }
@@ -632,8 +637,11 @@ __global__ void permute_bits_kernel(const ulonglong2 *__restrict__ in, long long
     out[i] = make_ulonglong2(lo, hi);
 }
 
-// eloc[i] = S[i, group 0] when group 0 is the f = 0 group (psi ratio == 1), else 0.
-__global__ void diag_init_kernel(HamDev hm, const ulonglong2 *__restrict__ x, long long B, float2 *__restrict__ eloc) {
+// eloc[i] = S[i, group 0] (when group 0 is the f = 0 group: psi ratio == 1) + the per-CTA partial sums of the chain
+// kernel, added in slot order = cluster order, rank 0 before rank 1: a fixed order, so the result is bit-reproducible.
+// Slots no CTA owns were zeroed before the chain kernel ran.
+__global__ void eloc_finish_kernel(HamDev hm, const ulonglong2 *__restrict__ x, long long B, const float2 *__restrict__ epart,
+                                   int eslots, float2 *__restrict__ eloc) {
     const long long i = (long long)blockIdx.x * blockDim.x + threadIdx.x;
     if (i >= B) return;
     float2 S = make_float2(0.f, 0.f);
@@ -648,6 +656,12 @@ __global__ void diag_init_kernel(HamDev hm, const ulonglong2 *__restrict__ x, lo
             S.y += cs.y;
         }
     }
+    const float2 *pp = epart + (size_t)(i / TILE_M) * eslots * TILE_M + (i % TILE_M);
+    for (int j = 0; j < eslots; ++j) {
+        const float2 e = pp[(size_t)j * TILE_M];
+        S.x += e.x;
+        S.y += e.y;
+    }
     eloc[i] = S;
 }
 
@@ -659,6 +673,7 @@ struct TcPack {
     uint32_t slot_bytes = 0, res_bytes = 0, img_stride = 0, tm_d3 = 0, tm_a0 = 0;
     void *d_wimg = nullptr, *d_fills = nullptr, *d_res = nullptr, *d_bias = nullptr;
     void *d_fpos = nullptr; size_t fpos_cap = 0;
+    void *d_epart = nullptr; size_t epart_cap = 0;   // per-CTA partial sums of E (launch_eloc_tc)
     void *d_xpos = nullptr; size_t xpos_cap = 0;
     SmemLayout L{};
     uint32_t sub[MAX_SUB + 1] = {0};
@@ -981,6 +996,7 @@ void tc_pack_free(const nqs_made *M) {
     TcPack *P = M->tc;
     cudaFree(P->d_wimg); cudaFree(P->d_fills); cudaFree(P->d_res); cudaFree(P->d_bias);
     if (P->d_fpos) cudaFree(P->d_fpos);
+    if (P->d_epart) cudaFree(P->d_epart);
     if (P->d_xpos) cudaFree(P->d_xpos);
     delete P;
     M->tc = nullptr;
@@ -1089,16 +1105,38 @@ int launch_eloc_tc(const HamDev &hm, const nqs_made *M, const ulonglong2 *x, con
     if (hm.G > 0 && (rc = permuted(M, hm.flips, hm.G, (ulonglong2 *)P->d_fpos, st))) return rc;
     if ((rc = ensure(&P->d_xpos, &P->xpos_cap, sizeof(ulonglong2) * (size_t)B))) return rc;
     if ((rc = permuted(M, x, B, (ulonglong2 *)P->d_xpos, st))) return rc;
-    diag_init_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(hm, x, B, eloc);
-    ++g_launch_count;
-    if (cudaGetLastError() != cudaSuccess) return NQS_ECUDA;
     TcParams p{};
     fill_common(M, p);
     p.mode = 1; p.xpos = (const ulonglong2 *)P->d_xpos; p.B = B; p.fpos = (const ulonglong2 *)P->d_fpos; p.x = x;
-    p.hm = hm; p.base = base; p.eloc = (float *)eloc; p.max_ratio_bits = max_ratio_bits;
+    p.hm = hm; p.base = base; p.max_ratio_bits = max_ratio_bits;
     p.g_begin = hm.has_diag ? 1 : 0;
     const long long nsb = (B + TILE_M - 1) / TILE_M;
-    const long long ntiles = nsb * (hm.G - p.g_begin);
-    if (ntiles > 0) return launch_chain(P, p, ntiles, st);
-    return NQS_OK;
+    const long long Gnd = hm.G - p.g_begin;
+    const long long ntiles = nsb * Gnd;
+    // Partial-sum slots (see the flush in the kernel): walk the kernel's own static schedule -- cluster k owns tile pairs
+    // [npairs k / ncl, npairs (k+1) / ncl) -- and take the largest number of clusters that share one sample block.
+    int eslots = 0;
+    if (ntiles > 0) {
+        const long long npairs = (ntiles + 1) / 2, ncl_max = P->sms / 2, ncl = npairs < ncl_max ? npairs : ncl_max;
+        long long cur_sb = -1, cnt = 0, most = 0;
+        for (long long k = 0; k < ncl; ++k) {
+            const long long t_lo = 2 * (npairs * k / ncl), t_hi = std::min(2 * (npairs * (k + 1) / ncl), ntiles);
+            if (t_hi <= t_lo) continue;
+            const long long sb_lo = t_lo / Gnd, sb_hi = (t_hi - 1) / Gnd;
+            cnt = (sb_lo == cur_sb) ? cnt + 1 : 1;                 // clusters on block sb_lo so far
+            most = std::max(most, cnt);
+            if (sb_hi != sb_lo) cnt = 1;                           // this cluster is the first on block sb_hi (blocks between are its own)
+            cur_sb = sb_hi;
+        }
+        eslots = (int)(2 * most);
+        const size_t bytes = sizeof(float2) * (size_t)nsb * eslots * TILE_M;
+        if ((rc = ensure(&P->d_epart, &P->epart_cap, bytes))) return rc;
+        if (cudaMemsetAsync(P->d_epart, 0, bytes, st) != cudaSuccess) { cudaGetLastError(); return NQS_ECUDA; }
+        p.epart = (float2 *)P->d_epart; p.eslots = eslots;
+        if ((rc = launch_chain(P, p, ntiles, st))) return rc;
+    }
+    eloc_finish_kernel<<<(unsigned)((B + 255) / 256), 256, 0, st>>>(hm, x, B, (const float2 *)P->d_epart, eslots, eloc);
+    ++g_launch_count;
+    return cudaGetLastError() == cudaSuccess ? NQS_OK : NQS_ECUDA;
 }
+

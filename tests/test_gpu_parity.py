@@ -853,3 +853,21 @@ def test_sampler_takes_the_constraint_of_the_handle():
     s2, _ = nqs.made_sample(M, 3000, 11, 2, 3, device=DEV)
     bits = wl.unpack_bits(s2.cpu().numpy().view(np.uint64), 12)
     assert np.all(bits[:, 0::2].sum(axis=1) == 2) and np.all(bits[:, 1::2].sum(axis=1) == 3)
+
+
+@pytest.mark.parametrize("cfg,B,mb", [(1, 256, 0), (3, 1101, 0), (3, 1101, 512), (4, 300, 0)])
+def test_tc_eloc_is_bit_reproducible(cfg, B, mb):
+    """The tensor-core path adds each row's per-CTA partial sums in a fixed order (no float atomics): the same call gives
+    the same bytes, whatever the order the CTAs ran in.  cfg 1 puts 25 clusters on one sample block (50 slots per row),
+    cfg 3 / 4 have clusters that straddle sample blocks; the mini-batch variant reuses the partial buffer at another size."""
+    w, (x, z, c), params, H, M = workload(cfg)
+    samples, counts = wl.make_samples(w.n_spatial, w.n_alpha, w.n_beta, B, w.max_count, w.seed_samples, w.unique)
+    xs = _dev_u64(samples)
+    e0, s0 = nqs.local_energy(H, M, xs, None, minibatch=mb, path=nqs.PATH_TC)
+    e0 = e0.clone()
+    junk, _ = nqs.local_energy(H, M, xs[: B // 3].contiguous(), None, path=nqs.PATH_TC)      # another shape in between
+    e1, s1 = nqs.local_energy(H, M, xs, None, minibatch=mb, path=nqs.PATH_TC)
+    assert torch.equal(e0, e1) and np.array_equal(s0, s1)
+    e_si, _ = nqs.local_energy(H, M, xs, None, path=nqs.PATH_SIMT)
+    d = (e0 - e_si).cpu().numpy().astype(np.float64)
+    assert np.hypot(d[:, 0], d[:, 1]).max() <= 1e-5 * H.sum_abs_coeff
