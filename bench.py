@@ -119,17 +119,42 @@ def time_oracle(w, ham, params, samples, n_samples, one_thread=False):
     return n_samples * len(c) / dt, dt, threads
 
 
-# DRAM bytes (read + write) of ONE eloc_tc_kernel launch from the `ncu --set full` capture summarised in
-# profiles/r2_final_summary.md, keyed by (cfg, samples per launch).  A constant of that capture, not measured live: the
-# full-size launch (8,192 samples, 2.4 s x ~45 replay passes) did not finish under ncu, the 2,048-sample launch did.
-NCU_DRAM_BYTES_PER_LAUNCH = {(5, 2048): 326464000 + 7157248}
+# Constants read from ncu captures (profiles/r3_ncu_counters.md gives the commands).  They describe the kernel SOURCE they
+# were captured on: each carries the sha256 (first 16 hex) of the .cu files it depends on, and bench.py reports a constant
+# only while those files are unchanged -- a stale capture is omitted, not repeated.
+NCU_CAPTURES = {
+    # DRAM bytes (read + write) of ONE eloc_tc_kernel launch, keyed by (cfg, samples per launch)
+    "eloc_tc_dram_bytes": {"files": ["kernels_tc.cu", "tc_ptx.cuh"], "sha16": None, "values": {}},
+    # warp instructions executed per (sample, term) pair by contract_kernel over all groups of cfg 5 (8,192 samples)
+    "contract_warp_inst_per_pair": {"files": ["kernels_simt.cu", "nqs_internal.h"], "sha16": None, "values": {}},
+}
+
+
+def _source_sha16(files):
+    import hashlib
+    h = hashlib.sha256()
+    for f in files:
+        with open(os.path.join(ROOT, "paper_2208_05637_b200", "csrc", f), "rb") as fh:
+            h.update(fh.read())
+    return h.hexdigest()[:16]
+
+
+def ncu_constant(name, key):
+    """The captured value, or None when there is no capture for `key` or the kernel source changed since."""
+    c = NCU_CAPTURES[name]
+    if key not in c["values"] or c["sha16"] != _source_sha16(c["files"]):
+        return None
+    return c["values"][key]
 
 
 def time_contraction(nqs, torch, H, xs, stream, clocks_mhz):
     """Standalone Pauli contraction (a3, nqs_pauli_contract) of one mini-batch against ALL groups, in group chunks
     that reuse one output buffer (S is never materialised whole: B x G x 8 bytes would be 38 GB at cfg 5).
-    ALU roofline: 148 SM x 128 INT/FP32 lanes x SM clock; 7 lane-operations per (sample, term) pair for n <= 128
-    (2 AND + 2 POPC + parity add/select + 2 sign-injected FP32 adds)."""
+    ALU roofline: SMs (device attribute) x 128 INT/FP32 lanes x SM clock.  Two per-pair operation counts are reported:
+    the model count of SURVEY.md 8(d) (7 lane-operations: AND, popcount, parity, sign inject, 2 FP32 adds, select), and --
+    when a capture of the current kernel source exists -- the warp instructions ncu counted per pair (loads, address
+    arithmetic and loop overhead included), which is what the issue slots actually saw.  The sweep writes B x G x 8 bytes
+    of S to HBM, so for groups of ~5 terms the figure is as much a store rate as a popcount rate (hbm_write_gbs)."""
     B, G, K = xs.shape[0], H.G, H.K
     chunk = max(1, min(G, (256 << 20) // (B * 8)))
     out = torch.empty((chunk, B, 2), dtype=torch.float32, device=xs.device)
@@ -149,9 +174,13 @@ def time_contraction(nqs, torch, H, xs, stream, clocks_mhz):
     torch.cuda.synchronize()
     ms = e0.elapsed_time(e1)
     pairs_s = B * K / (ms / 1e3)
-    peak = 148 * 128 * clocks_mhz * 1e6
-    return {"value": pairs_s, "unit": "pairs/s", "ms": ms, "launches": (G + chunk - 1) // chunk,
-            "lane_ops_per_pair": 7, "alu_peak_lane_ops_per_s": peak, "alu_frac": 7 * pairs_s / peak,
+    sms = torch.cuda.get_device_properties(xs.device).multi_processor_count
+    peak = sms * 128 * clocks_mhz * 1e6
+    counted = ncu_constant("contract_warp_inst_per_pair", 5) if (B, K) == (8192, 2802815) else None
+    return {"value": pairs_s, "unit": "pairs/s", "ms": ms, "launches": (G + chunk - 1) // chunk, "sms": sms,
+            "lane_ops_per_pair_model": 7, "alu_peak_lane_ops_per_s": peak, "alu_frac_model": 7 * pairs_s / peak,
+            "warp_inst_per_pair_counted": counted,
+            "issue_frac_counted": (counted * pairs_s / (sms * 4 * clocks_mhz * 1e6)) if counted else None,
             "hbm_write_gbs": B * G * 8 / (ms / 1e3) / 1e9,
             "note": "standalone nqs_pauli_contract over all groups; S chunks are written to HBM (the fused path keeps them in registers)"}
 
@@ -167,6 +196,10 @@ def main():
     ap.add_argument("--oracle-samples", type=int, default=0, help="samples for the cpu_baseline leg (0 = auto)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-contraction", action="store_true", help="skip the standalone contraction figure")
+    ap.add_argument("--no-full-config", action="store_true",
+                    help="skip the one call over all 65,536 samples as 8 mini-batches (cfg 5: ~20 s)")
+    ap.add_argument("--iteration", action="store_true",
+                    help="also time one whole VMC iteration through the ABI: sampler -> E_loc -> gradient")
     ap.add_argument("--mb-samples", type=int, default=0,
                     help="profiling aid: samples per step instead of the configured mini-batch (labelled in config)")
     args = ap.parse_args()
@@ -290,6 +323,48 @@ def main():
     e2e_ms = max_over_ranks(e2e_ms, dev)
     e2e_val = pairs_per_step / (e2e_ms / 1e3)
 
+    # ---- the configuration as BASELINE.json states it: every sample of the batch in ONE call, processed as
+    # gradient-accumulation mini-batches (row a7), host buffers in, host buffers out, wall clock ----
+    full_config = None
+    if not args.no_full_config and not args.mb_samples:
+        Bfull = wq.batch
+        hof = np.zeros((Bfull, 2), np.float32)
+        barrier()
+        t0 = time.perf_counter()
+        _, st_full = nqs.local_energy_host(H, M, samples, counts, minibatch=mb, path=path, want_stats=True, out=hof)
+        full_s = max_over_ranks(time.perf_counter() - t0, dev)
+        full_config = {"samples": Bfull, "minibatches": (Bfull + mb - 1) // mb, "seconds": full_s,
+                       "value": Bfull * K * world / full_s, "unit": UNIT,
+                       "mean_E": [st_full[1] / st_full[0], st_full[2] / st_full[0]],
+                       "note": "one nqs_local_energy_host call over the whole configured batch; H2D, all mini-batches, "
+                               "statistics and D2H inside the wall-clock region"}
+
+    # ---- one whole iteration through the ABI: sampler -> E_loc -> gradient, each wall-clocked ----
+    iteration = None
+    if args.iteration:
+        M.set_constraint(wq.n_alpha, wq.n_beta)
+        n_draws = 1 << 20
+        barrier()
+        t0 = time.perf_counter()
+        s_dev, c_dev = nqs.made_sample(M, n_draws, 2024, max_unique=mb, device=dev)
+        torch.cuda.synchronize()
+        t_sample = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        e_it, st_it = nqs.local_energy(H, M, s_dev, c_dev, minibatch=mb, path=path)
+        torch.cuda.synchronize()
+        t_eloc = time.perf_counter() - t0
+        t0 = time.perf_counter()
+        g_it, b_it = nqs.energy_grad(M, s_dev, c_dev, e_it, minibatch=mb)
+        torch.cuda.synchronize()
+        t_grad = time.perf_counter() - t0
+        M.set_constraint(-1, -1)
+        iteration = {"n_draws": n_draws, "unique_samples": int(s_dev.shape[0]), "constraint": [wq.n_alpha, wq.n_beta],
+                     "sample_s": t_sample, "eloc_s": t_eloc, "grad_s": t_grad,
+                     "sample_over_eloc": t_sample / t_eloc, "grad_over_eloc": t_grad / t_eloc,
+                     "mean_E": [st_it[1] / st_it[0], st_it[2] / st_it[0]], "grad_finite": bool(torch.isfinite(g_it).all().item()),
+                     "note": "nqs_made_sample (first call: includes its per-call buffer allocation) -> nqs_local_energy -> "
+                             "nqs_energy_grad on the sampler's output, constrained model, wall clock with a synchronise after each"}
+
     if rank != 0:
         if world > 1:
             dist.destroy_process_group()
@@ -308,18 +383,17 @@ def main():
                 "peak_source": f"{peaks['src']} bf16 dense, sustained (fp16 operands run at the bf16 rate)"}
     else:
         clk = (clocks["sm_mhz"] or peaks["sm_max_mhz"]) * 1e6
-        alu_peak = 148 * 128 * 2 * clk / 1e12             # FFMA lanes x 2 flop x measured clock
+        sms = torch.cuda.get_device_properties(dev).multi_processor_count
+        alu_peak = sms * 128 * 2 * clk / 1e12             # FFMA lanes x 2 flop x measured clock
         roof = {"bound": "alu", "achieved": achieved, "peak": alu_peak, "unit": "TFLOP/s", "frac": achieved / alu_peak,
-                "traffic": None, "peak_source": "148 SM x 128 FFMA lanes x 2 flop x median SM clock under load"}
+                "traffic": None, "peak_source": f"{sms} SM x 128 FFMA lanes x 2 flop x median SM clock under load"}
     roof.update({"kernel": "eloc_tc_kernel" if used_tc else "eloc_simt_kernel", "kernel_ms_per_launch": k_ms,
                  "algorithmic_flops_per_eval": flops_eval, "evals_per_launch": evals_per_launch,
                  "kernel_share_of_step": chain_ms / total_ms})
 
-    roof["traffic"] = NCU_DRAM_BYTES_PER_LAUNCH.get((args.cfg, mb)) if used_tc else None
-    if used_tc and roof["traffic"] is None and (args.cfg, 2048) in NCU_DRAM_BYTES_PER_LAUNCH:
-        roof["traffic_reduced_launch"] = {"bytes": NCU_DRAM_BYTES_PER_LAUNCH[(args.cfg, 2048)], "samples": 2048,
-                                          "note": "ncu capture of a 2,048-sample launch (the full-size launch does not finish "
-                                                  "under ncu); algorithmic bytes = the term tensors once, 79 MB"}
+    roof["traffic"] = ncu_constant("eloc_tc_dram_bytes", (args.cfg, mb)) if used_tc else None
+    roof["traffic_source"] = ("ncu dram__bytes_read.sum + dram__bytes_write.sum of one launch of this kernel source "
+                              "(profiles/r3_ncu_counters.md)") if roof["traffic"] else "no ncu capture of the current kernel source"
     if used_tc:
         issued, dense = M.tc_flops()
         roof["issued_flops_per_eval"] = issued                # what the kernel sends to the tensor cores (overhead included)
@@ -349,6 +423,7 @@ def main():
             "cpu_baseline": cpu_baseline, "cpu_baseline_1thread": cpu_baseline_1,
             "e2e": {"value": e2e_val, "unit": UNIT, "ms_per_step": e2e_ms, "h2d_bytes_per_step": mb * 16 + mb * 8,
                     "d2h_bytes_per_step": mb * 8 + 5 * 8},
+            "full_config": full_config, "iteration": iteration,
             "gpu_launches": int(launches), "clocks": clocks,
             "job_stats": {"sum_n": job_stats[0].item(), "mean_E": [(job_stats[1] / job_stats[0]).item(), (job_stats[2] / job_stats[0]).item()],
                           "note": "count-weighted mean of E_loc over every mini-batch of every rank in the timed steps "

@@ -61,8 +61,15 @@ enum nqs_status {
  *                  so round16(n+2) <= 128 input columns; TMEM holds two 128-column accumulators + round16(n+4)
  *                  output columns + round16(n+2)/2 input columns <= 512 (three accumulators when n <= 76).  Other
  *                  shapes (n = 127, 128 included) return NQS_EUNSUPPORTED; NQS_PATH_AUTO then takes NQS_PATH_SIMT.
- *                  Precision: hidden (padded) >= 384 runs one fp16 pass (|dE_loc| 0.1-0.2 x 1e-5 sum|c| on the chemistry
- *                  workloads); hidden (padded) <= 256 runs in SPLIT precision — every fp16 operand as hi + lo parts, three MMA
+ *                  Precision: hidden (padded) >= 384 runs ONE fp16 pass (10-bit mantissa, the TF32 mantissa): every psi
+ *                  ratio carries a relative error of a few 1e-4, so |dE_loc| is bounded by ~8e-3 sum|c| max|ratio| and
+ *                  meets 1e-5 sum|c| only where the terms of a row largely cancel — measured on the Jordan-Wigner
+ *                  chemistry Hamiltonians of the five configured workloads: max 0.14 x the bound over 32 oracle rows and 0.31 x
+ *                  over 1,101 rows against the fp32 path at 76 qubits, 0.42 x / 0.66 x at 52 qubits.  On other
+ *                  Hamiltonians at hidden >= 384 it does NOT meet that bound (measured 1.5 x on a symmetry-sparse
+ *                  20-qubit Hamiltonian with a one-hidden-layer net, 2-3 x on generic Pauli lists): a caller who needs
+ *                  1e-5 sum|c| there passes NQS_PATH_SIMT (fp32, ~30 x slower) and can check stats[4] = max|ratio|.
+ *                  hidden (padded) <= 256 runs in SPLIT precision — every fp16 operand as hi + lo parts, three MMA
  *                  passes (hi.hi + lo.hi + hi.lo) — because a single fp16 pass misses the bound there (2 x); split
  *                  results are as accurate as the fp32 path (0.03 x the bound) at 3 x the tensor work.
  *  NQS_PATH_AUTO : TC when the shape supports it, else SIMT.  If the tensor-core weight pack of a supported shape cannot be
@@ -279,7 +286,8 @@ int nqs_energy_grad(const nqs_made_t *made, const uint64_t *samples_dev, const i
  *     without one the pair clamps the sampler alone.
  * samples_out_dev : device uint64 [cap][2], counts_out_dev : device int64 [cap], cap = max_unique if 0 < max_unique <
  *   n_draws else n_draws; the first *n_unique_out_host rows are written, in buffer order (unique, bit j = qubit j).
- * Synchronous (n readbacks of the buffer size); allocates and frees its buffers per call.  n_draws < 2^30
+ * Synchronous (n readbacks of the buffer size); its buffers live in the model handle and grow on demand (a handle
+ * serves one nqs_made_sample call at a time).  n_draws < 2^30
  * (buffer indices are 32-bit; more: NQS_ERANGE). */
 int nqs_made_sample(const nqs_made_t *made, int64_t n_draws, uint64_t seed, int n_up, int n_down,
                     int64_t max_unique, uint64_t *samples_out_dev, int64_t *counts_out_dev,

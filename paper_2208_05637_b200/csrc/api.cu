@@ -194,6 +194,7 @@ extern "C" void nqs_made_free(nqs_made_t *M) {
     if (M->hx) cudaFree(M->hx);
     if (M->hc) cudaFree(M->hc);
     if (M->he) cudaFree(M->he);
+    if (M->samp_ws) cudaFree(M->samp_ws);
     if (M->h_stream) cudaStreamDestroy(M->h_stream);
     for (cudaEvent_t e : M->ev) cudaEventDestroy(e);
     tc_pack_free(M);

@@ -173,16 +173,27 @@ extern "C" int nqs_made_sample(const nqs_made_t *M, int64_t n_draws, uint64_t se
     if (rc) return rc;
     cudaStream_t st = (cudaStream_t)cuda_stream;
     const long long emax = max_unique > 0 && max_unique < n_draws ? max_unique : n_draws;     // buffer entries after a step
-    void *d_cfg[2] = {nullptr, nullptr}, *d_cnt = nullptr, *d_cc = nullptr, *d_ni = nullptr, *d_entry = nullptr, *d_p1 = nullptr, *d_n = nullptr;
-    auto cleanup = [&]() {
-        cudaFree(d_cfg[0]); cudaFree(d_cfg[1]); cudaFree(d_cnt); cudaFree(d_cc); cudaFree(d_ni); cudaFree(d_entry); cudaFree(d_p1); cudaFree(d_n);
-    };
-    if (cudaMalloc(&d_cfg[0], 16 * (size_t)emax) != cudaSuccess || cudaMalloc(&d_cfg[1], 16 * (size_t)emax) != cudaSuccess ||
-        cudaMalloc(&d_cnt, 8 * (size_t)emax) != cudaSuccess || cudaMalloc(&d_cc, 16 * (size_t)emax) != cudaSuccess ||
-        cudaMalloc(&d_ni, 8 * (size_t)emax) != cudaSuccess || cudaMalloc(&d_entry, 4 * (size_t)n_draws) != cudaSuccess ||
-        cudaMalloc(&d_p1, 4 * (size_t)emax) != cudaSuccess || cudaMalloc(&d_n, 8) != cudaSuccess) {
-        cudaGetLastError(); cleanup(); return NQS_ENOMEM;
+    // buffers: one arena in the model handle, grown on demand and kept (a handle serves one call at a time), so a
+    // training loop that samples every iteration allocates on its first iteration only
+    auto al = [](size_t b) { return (b + 255) & ~(size_t)255; };
+    const size_t sz_cfg = al(16 * (size_t)emax), sz_cnt = al(8 * (size_t)emax), sz_cc = al(16 * (size_t)emax),
+                 sz_ni = al(8 * (size_t)emax), sz_entry = al(4 * (size_t)n_draws), sz_p1 = al(4 * (size_t)emax), sz_n = 256;
+    const size_t need = 2 * sz_cfg + sz_cnt + sz_cc + sz_ni + sz_entry + sz_p1 + sz_n;
+    if (M->samp_ws_bytes < need) {
+        if (M->samp_ws) cudaFree(M->samp_ws);
+        M->samp_ws = nullptr; M->samp_ws_bytes = 0;
+        if (cudaMalloc(&M->samp_ws, need) != cudaSuccess) { cudaGetLastError(); return NQS_ENOMEM; }
+        M->samp_ws_bytes = need;
     }
+    unsigned char *wsp = (unsigned char *)M->samp_ws;
+    void *d_cfg[2];
+    d_cfg[0] = wsp; wsp += sz_cfg; d_cfg[1] = wsp; wsp += sz_cfg;
+    void *d_cnt = wsp; wsp += sz_cnt;
+    void *d_cc = wsp; wsp += sz_cc;
+    void *d_ni = wsp; wsp += sz_ni;
+    void *d_entry = wsp; wsp += sz_entry;
+    void *d_p1 = wsp; wsp += sz_p1;
+    void *d_n = wsp;
     rc = NQS_ECUDA;
     long long E = 1;
     int cur = 0;
@@ -214,7 +225,6 @@ extern "C" int nqs_made_sample(const nqs_made_t *M, int64_t n_draws, uint64_t se
              cudaMemcpyAsync(counts_out_dev, d_cnt, 8 * (size_t)E, cudaMemcpyDeviceToDevice, st) == cudaSuccess &&
              cudaStreamSynchronize(st) == cudaSuccess;
     }
-    cleanup();
     if (!ok) { cudaGetLastError(); return rc; }
     *n_unique_out_host = E;
     return NQS_OK;

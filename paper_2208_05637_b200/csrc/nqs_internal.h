@@ -118,6 +118,9 @@ struct nqs_made {
     mutable void *hx = nullptr, *hc = nullptr, *he = nullptr;
     mutable size_t h_rows = 0;
     mutable cudaStream_t h_stream = nullptr;
+    // buffers of nqs_made_sample: one arena, grown on demand, reused across calls
+    mutable void  *samp_ws = nullptr;
+    mutable size_t samp_ws_bytes = 0;
     // timing of the chain kernel (nqs_last_chain_kernel_ms)
     mutable std::vector<cudaEvent_t> ev;        // pairs (start, stop)
     mutable int ev_used = 0;
