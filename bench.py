@@ -124,9 +124,12 @@ def time_oracle(w, ham, params, samples, n_samples, one_thread=False):
 # only while those files are unchanged -- a stale capture is omitted, not repeated.
 NCU_CAPTURES = {
     # DRAM bytes (read + write) of ONE eloc_tc_kernel launch, keyed by (cfg, samples per launch)
-    "eloc_tc_dram_bytes": {"files": ["kernels_tc.cu", "tc_ptx.cuh"], "sha16": None, "values": {}},
-    # warp instructions executed per (sample, term) pair by contract_kernel over all groups of cfg 5 (8,192 samples)
-    "contract_warp_inst_per_pair": {"files": ["kernels_simt.cu", "nqs_internal.h"], "sha16": None, "values": {}},
+    "eloc_tc_dram_bytes": {"files": ["kernels_tc.cu", "tc_ptx.cuh"], "sha16": "c59e0af701c9581a",
+                           "values": {(5, 8192): 1067126912}},      # mean of two launches: 1.046 GB read + 21 MB written
+    # thread-level instructions executed per (sample, term) pair by contract_kernel, summed over the 144 launches of one
+    # sweep over all groups of cfg 5 (8,192 samples): smsp__thread_inst_executed.sum / (B * K)
+    "contract_thread_inst_per_pair": {"files": ["kernels_simt.cu", "nqs_internal.h"], "sha16": "75b0c7f177203c5c",
+                                      "values": {5: 23.71}},
 }
 
 
@@ -152,8 +155,8 @@ def time_contraction(nqs, torch, H, xs, stream, clocks_mhz):
     that reuse one output buffer (S is never materialised whole: B x G x 8 bytes would be 38 GB at cfg 5).
     ALU roofline: SMs (device attribute) x 128 INT/FP32 lanes x SM clock.  Two per-pair operation counts are reported:
     the model count of SURVEY.md 8(d) (7 lane-operations: AND, popcount, parity, sign inject, 2 FP32 adds, select), and --
-    when a capture of the current kernel source exists -- the warp instructions ncu counted per pair (loads, address
-    arithmetic and loop overhead included), which is what the issue slots actually saw.  The sweep writes B x G x 8 bytes
+    when a capture of the current kernel source exists -- the thread-level instructions ncu counted per pair (loads,
+    address arithmetic, the per-group prologue and store amortised over ~4.8 terms), which is what the lanes actually saw.  The sweep writes B x G x 8 bytes
     of S to HBM, so for groups of ~5 terms the figure is as much a store rate as a popcount rate (hbm_write_gbs)."""
     B, G, K = xs.shape[0], H.G, H.K
     chunk = max(1, min(G, (256 << 20) // (B * 8)))
@@ -176,11 +179,11 @@ def time_contraction(nqs, torch, H, xs, stream, clocks_mhz):
     pairs_s = B * K / (ms / 1e3)
     sms = torch.cuda.get_device_properties(xs.device).multi_processor_count
     peak = sms * 128 * clocks_mhz * 1e6
-    counted = ncu_constant("contract_warp_inst_per_pair", 5) if (B, K) == (8192, 2802815) else None
+    counted = ncu_constant("contract_thread_inst_per_pair", 5) if (B, K) == (8192, 2802815) else None
     return {"value": pairs_s, "unit": "pairs/s", "ms": ms, "launches": (G + chunk - 1) // chunk, "sms": sms,
             "lane_ops_per_pair_model": 7, "alu_peak_lane_ops_per_s": peak, "alu_frac_model": 7 * pairs_s / peak,
-            "warp_inst_per_pair_counted": counted,
-            "issue_frac_counted": (counted * pairs_s / (sms * 4 * clocks_mhz * 1e6)) if counted else None,
+            "thread_inst_per_pair_counted": counted,
+            "lane_frac_counted": (counted * pairs_s / peak) if counted else None,
             "hbm_write_gbs": B * G * 8 / (ms / 1e3) / 1e9,
             "note": "standalone nqs_pauli_contract over all groups; S chunks are written to HBM (the fused path keeps them in registers)"}
 
